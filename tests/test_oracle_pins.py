@@ -1,0 +1,258 @@
+"""Pins P2-P4, P6-P10: the oracle's whole step against what the method and the mathematics fix.
+
+Nothing here compares the oracle with itself on the same path: expected values are invariants of Eq. 10/13/16
+(PAPER.md:90-95, :131-139, :163-168), symmetries of Eq. 1-4, the decomposition property of the patch-group
+contract, the closed-form exact Euler Riemann solution (Sod), and convergence rates.
+"""
+import numpy as np
+import pytest
+
+from paper_1804_03479_b200 import inputs
+import harness as H
+
+G = 5.0 / 3.0
+SCHEMES = [("vl_plm", 0, 0, 3), ("ctu_plm", 1, 0, 3), ("ctu_ppm", 1, 1, 4)]
+
+
+def mk(oracle, scheme, recon, g, N=16, riemann=1, limvar=None):
+    cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon, riemann=riemann, limvar=limvar)
+    return cfg, (lambda Ui, Bi, dt, dh: oracle.advance(cfg, Ui, Bi, dt, dh))
+
+
+# ------------------------------------------------------------------------------------------------
+# P2 uniform state: nothing changes, bitwise, for every scheme and solver
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,scheme,recon,g", SCHEMES)
+@pytest.mark.parametrize("riemann", [0, 1, 2])
+def test_p2_uniform_state_is_a_fixed_point(oracle, name, scheme, recon, g, riemann):
+    n = 16
+    rho, v, p, B = 1.3, (0.4, -0.7, 0.2), 0.8, (0.5, -0.3, 0.9)
+    bx = np.full((n, n, n + 1), B[0]); by = np.full((n, n + 1, n), B[1]); bz = np.full((n + 1, n, n), B[2])
+    o = np.ones((n, n, n))
+    U = inputs.conserved(rho * o, v[0] * o, v[1] * o, v[2] * o, p * o, bx, by, bz, G)
+    cfg, adv = mk(oracle, scheme, recon, g, riemann=riemann)
+    Un, bxn, byn, bzn, out, _ = H.step_grid(adv, U, bx, by, bz, 0.01, 1.0 / n, 16, g)
+    # rho and B are reproduced bitwise (their fluxes/EMFs are exact products of the uniform values);
+    # M and e to round-off of the flux differences
+    assert np.array_equal(bxn, bx) and np.array_equal(byn, by) and np.array_equal(bzn, bz)
+    assert np.abs(Un - U).max() < 1e-14
+    assert out["stats"] == (0, 0, 0)
+
+
+# ------------------------------------------------------------------------------------------------
+# P3 conservation + P4 div B + shared faces bitwise, 10 steps on a generic periodic state cut into 8 groups
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,scheme,recon,g", SCHEMES)
+def test_p3_p4_conservation_and_divb(oracle, name, scheme, recon, g):
+    n = 32
+    U, bx, by, bz, dh = inputs.random_group_grid(n, 77)
+    cfg, adv = mk(oracle, scheme, recon, g)
+    t0 = H.totals(U)
+    assert H.rel_divb(bx, by, bz, dh) < 1e-13
+    mean_b0 = [bx.mean(), by.mean(), bz.mean()]
+    for _ in range(10):
+        Ui, Bi = inputs.pack_groups(U, bx, by, bz, n, 0)
+        c0 = oracle.make_config(N=n, g=3)
+        dt, _ = oracle.dt_reduce(c0, Ui, Bi, 0, dh, 0.3)
+        U, bx, by, bz, out, mism = H.step_grid(adv, U, bx, by, bz, dt, dh, 16, g)
+        assert mism == 0.0                       # faces shared by two groups come out bitwise equal
+        assert H.rel_divb(bx, by, bz, dh) < 1e-13
+    t1 = H.totals(U)
+    scale = np.array([t0[0], np.abs(U[1:4]).sum(), np.abs(U[1:4]).sum(), np.abs(U[1:4]).sum(), t0[4]])
+    assert np.all(np.abs(t1 - t0) / scale < 1e-13), (t1 - t0) / scale
+    # the volume-averaged field is conserved too (Eq. 13 is a discrete curl)
+    for a, m0 in zip((bx, by, bz), mean_b0):
+        assert abs(a[..., :, :, :].mean() - m0) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
+# P9 decomposition: monolithic 32^3 vs 8 groups of 16^3 with g ghosts: bitwise; one ghost fewer: not
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,scheme,recon,g", SCHEMES)
+def test_p9_decomposition_is_bitwise_and_ghost_width_is_minimal(oracle, name, scheme, recon, g):
+    n = 32
+    U, bx, by, bz, dh = inputs.random_group_grid(n, 5)
+    dt = 0.2 * dh
+    cfgM, advM = mk(oracle, scheme, recon, g, N=32)
+    cfgD, advD = mk(oracle, scheme, recon, g, N=16)
+    a = H.step_grid(advM, U, bx, by, bz, dt, dh, 32, g)
+    b = H.step_grid(advD, U, bx, by, bz, dt, dh, 16, g)
+    for x, y in zip(a[:4], b[:4]):
+        assert np.array_equal(x, y)
+    # extra garbage layer beyond g must not matter: g+1 ghosts, outermost layer overwritten with junk
+    cfgE = oracle.make_config(N=16, g=g + 1, scheme=scheme, recon=recon)
+    Ui, Bi = inputs.pack_groups(U, bx, by, bz, 16, g + 1)
+    out0 = oracle.advance(cfgE, Ui, Bi, dt, dh)
+    T = 16 + 2 * (g + 1)
+    Uj = Ui.reshape(-1, 5, T, T, T).copy()
+    mask = np.ones((T, T, T), bool); mask[1:-1, 1:-1, 1:-1] = False
+    Uj[:, 0][:, mask] = 7.0; Uj[:, 4][:, mask] = 99.0
+    out1 = oracle.advance(cfgE, Uj.reshape(Ui.shape), Bi, dt, dh)
+    assert np.array_equal(out0["U"], out1["U"]) and np.array_equal(out0["B"], out1["B"])
+    # one ghost cell fewer than required changes the answer (forced past the config check)
+    cfgS = oracle.make_config(N=16, g=g - 1, scheme=scheme, recon=recon)
+    Ui, Bi = inputs.pack_groups(U, bx, by, bz, 16, g - 1)
+    outS = oracle.advance(cfgS, Ui, Bi, dt, dh, force_ghost_ok=True)
+    Us, bxs, bys, bzs, _ = inputs.unpack_groups(outS["U"], outS["B"], n, 16)
+    differs = (not np.array_equal(np.nan_to_num(Us), a[0])) or (not np.array_equal(np.nan_to_num(bxs), a[1]))
+    assert differs
+    with pytest.raises(ValueError):
+        oracle.advance(cfgS, Ui, Bi, dt, dh)
+
+
+# ------------------------------------------------------------------------------------------------
+# P8 symmetry: cyclic axis permutation and x-mirror commute with the step
+# ------------------------------------------------------------------------------------------------
+def _permute(U, bx, by, bz):
+    """Relabel axes cyclically: new (x,y,z) = old (y,z,x), i.e. new_x-component = old_y-component etc.
+    Arrays are [z][y][x]; new array index (k',j',i') = old (z=j', y=i', x=k') -> transpose (1,2,0) of [z,y,x]->[?]."""
+    # old array a[z][y][x]; new coordinates x'=y, y'=z, z'=x  =>  new[z'][y'][x'] = old[z=y'][y=x'][x=z'] = a.transpose(2,0,1)
+    tr = lambda a: np.ascontiguousarray(a.transpose(2, 0, 1))
+    Un = np.stack([tr(U[0]), tr(U[2]), tr(U[3]), tr(U[1]), tr(U[4])])
+    return Un, tr(by), tr(bz), tr(bx)
+
+
+def _mirror_x(U, bx, by, bz):
+    f = lambda a: np.ascontiguousarray(a[..., ::-1])
+    Un = np.stack([f(U[0]), -f(U[1]), f(U[2]), f(U[3]), f(U[4])])
+    return Un, -f(bx), f(by), f(bz)
+
+
+@pytest.mark.parametrize("name,scheme,recon,g", [SCHEMES[0], SCHEMES[2]])
+@pytest.mark.parametrize("riemann", [1, 2])
+def test_p8_axis_permutation_and_mirror(oracle, name, scheme, recon, g, riemann):
+    n = 16
+    U, bx, by, bz, dh = inputs.random_group_grid(n, 11)
+    dt = 0.25 * dh
+    cfg, adv = mk(oracle, scheme, recon, g, riemann=riemann)
+    ref = H.step_grid(adv, U, bx, by, bz, dt, dh, 16, g)[:4]
+    for tf in (_permute, _mirror_x):
+        got = H.step_grid(adv, *tf(U, bx, by, bz), dt, dh, 16, g)[:4]
+        exp = tf(*ref)
+        for a, b in zip(got, exp):
+            assert np.abs(a - b).max() / np.abs(b).max() < 1e-13, tf.__name__
+    # and the transforms are not trivial on this input
+    assert np.abs(_permute(*ref)[0] - ref[0]).max() > 1e-3
+
+
+# ------------------------------------------------------------------------------------------------
+# P6 ABC force-free equilibrium with uniform pressure: the residual of one step converges at 2nd order
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,scheme,recon,g", [SCHEMES[0], SCHEMES[2]])
+def test_p6_abc_equilibrium_residual_converges(oracle, name, scheme, recon, g):
+    res = []
+    for n in (16, 32):
+        U, bx, by, bz, dh = inputs.abc_grid(n, 0, p0=1.0, vamp=0.0)
+        cfg, adv = mk(oracle, scheme, recon, g, N=n)
+        c0 = oracle.make_config(N=n, g=3)
+        Ui, Bi = inputs.pack_groups(U, bx, by, bz, n, 0)
+        dt, _ = oracle.dt_reduce(c0, Ui, Bi, 0, dh, 0.3)
+        Un, bxn, byn, bzn, _, _ = H.step_grid(adv, U, bx, by, bz, dt, dh, n, g)
+        # rate of change (divide by dt: dt itself halves with dh)
+        res.append((np.abs(Un[1:4] - U[1:4]).mean() / dt, np.abs(bxn - bx).mean() / dt, np.abs(Un[0] - U[0]).max()))
+    assert res[0][0] / res[1][0] > 3.0 and res[0][1] / res[1][1] > 3.0, res
+    assert res[0][0] < 1.0      # a mis-signed tension/pressure term would leave a force ~ k B^2 ~ 12
+    assert res[1][2] < 3e-3 and res[1][2] < res[0][2]
+
+
+# ------------------------------------------------------------------------------------------------
+# P7 field loop: the out-of-plane field of an advected in-plane loop stays at round-off (CTU source terms)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,scheme,recon,g", SCHEMES)
+@pytest.mark.parametrize("cdir", [2, 0])
+def test_p7_field_loop_out_of_plane_field(oracle, name, scheme, recon, g, cdir):
+    n, nc = 32, 16
+    a, b = (cdir + 1) % 3, (cdir + 2) % 3
+    shape_xyz = [n, n, n]; shape_xyz[cdir] = nc
+    nx, ny, nz = shape_xyz
+    dh = 1.0 / n
+    f = [np.arange(m + 1) * dh - 0.5 * m * dh for m in (nx, ny, nz)]
+    c = [(np.arange(m) + 0.5) * dh - 0.5 * m * dh for m in (nx, ny, nz)]
+    # potential along cdir lives on cdir-edges: face coords in a and b, centre coord along cdir
+    co = [None, None, None]; co[cdir] = c[cdir]; co[a] = f[a]; co[b] = f[b]
+    Z, Y, X = np.meshgrid(co[2], co[1], co[0], indexing="ij")
+    XYZ = (X, Y, Z)
+    r = np.sqrt(XYZ[a] ** 2 + XYZ[b] ** 2)
+    Ac = 1e-3 * np.maximum(0.3 - r, 0.0)
+    A = [np.zeros((nz + 1, ny + 1, nx)), np.zeros((nz + 1, ny, nx + 1)), np.zeros((nz, ny + 1, nx + 1))]
+    A[cdir] = Ac
+    bx, by, bz = inputs.faces_from_potential(A[0], A[1], A[2], dh)
+    v = [0.0, 0.0, 0.0]; v[a] = 1.0; v[b] = 0.5; v[cdir] = 1.0
+    o = np.ones((nz, ny, nx))
+    U = inputs.conserved(o, v[0] * o, v[1] * o, v[2] * o, o, bx, by, bz, G)
+    cfg, adv = mk(oracle, scheme, recon, g)
+    dt = 0.3 * dh / (1.0 + np.sqrt(G))
+    for _ in range(10):
+        U, bx, by, bz, _, _ = H.step_grid(adv, U, bx, by, bz, dt, dh, 16, g)
+    bc = (bx, by, bz)[cdir]
+    assert np.abs(bc).max() < 1e-16, np.abs(bc).max()
+    assert np.abs((bx, by, bz)[a]).max() > 5e-4     # the loop is still there
+
+
+# ------------------------------------------------------------------------------------------------
+# P10 B = 0: Sod tube against the exact Euler Riemann solution (closed form + one Newton solve for p*)
+# ------------------------------------------------------------------------------------------------
+def _sod_exact(x, t, gam, L=(1.0, 0.0, 1.0), R=(0.125, 0.0, 0.1)):
+    """Exact solution of the Euler Riemann problem (textbook: left rarefaction, contact, right shock for Sod)."""
+    rl, ul, pl = L; rr, ur, pr = R
+    al, ar = np.sqrt(gam * pl / rl), np.sqrt(gam * pr / rr)
+    g1, g2 = (gam - 1) / (2 * gam), (gam + 1) / (2 * gam)
+
+    def fK(p, rk, pk, ak):
+        if p > pk:   # shock
+            A, B = 2 / ((gam + 1) * rk), (gam - 1) / (gam + 1) * pk
+            return (p - pk) * np.sqrt(A / (p + B))
+        return 2 * ak / (gam - 1) * ((p / pk) ** g1 - 1)
+
+    lo, hi = 1e-8, 10.0
+    for _ in range(200):
+        mid = 0.5 * (lo + hi)
+        if fK(mid, rl, pl, al) + fK(mid, rr, pr, ar) + ur - ul > 0: hi = mid
+        else: lo = mid
+    ps = 0.5 * (lo + hi)
+    us = 0.5 * (ul + ur) + 0.5 * (fK(ps, rr, pr, ar) - fK(ps, rl, pl, al))
+    rsl = rl * (ps / pl) ** (1 / gam); asl = al * (ps / pl) ** g1
+    rsr = rr * ((ps / pr + (gam - 1) / (gam + 1)) / ((gam - 1) / (gam + 1) * ps / pr + 1))
+    S = ur + ar * np.sqrt(g2 * ps / pr + g1)
+    xi = x / t
+    rho = np.where(xi < ul - al, rl, np.where(xi < us - asl,
+          rl * (2 / (gam + 1) + (gam - 1) / ((gam + 1) * al) * (ul - xi)) ** (2 / (gam - 1)),
+          np.where(xi < us, rsl, np.where(xi < S, rsr, rr))))
+    return rho
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("name,scheme,recon,g,riemann", [("vl", 0, 0, 3, 1), ("ctu_ppm_roe", 1, 1, 4, 2), ("vl_hlle", 0, 0, 3, 0)])
+def test_p10_sod_tube_hydro_limit(oracle, axis, name, scheme, recon, g, riemann):
+    gam = 1.4
+    errs = []
+    for n in (32, 64):
+        NT = 4
+        shape = [NT, NT, NT]; shape[2 - axis] = 2 * n          # periodic double tube: [-1,1), discontinuities at 0 and +-1
+        nz, ny, nx = shape
+        dh = 2.0 / (2 * n)
+        xc = -1.0 + (np.arange(2 * n) + 0.5) * dh
+        bs = [1, 1, 1]; bs[2 - axis] = 2 * n
+        left = (np.abs(xc) < 0.5).reshape(bs) & np.ones(shape, bool)   # high-pressure state inside |x|<0.5 -> Sod tube at x=+0.5, mirrored one at -0.5
+        rho = np.where(left, 1.0, 0.125); p = np.where(left, 1.0, 0.1)
+        z = np.zeros(shape)
+        bx = np.zeros((nz, ny, nx + 1)); by = np.zeros((nz, ny + 1, nx)); bz = np.zeros((nz + 1, ny, nx))
+        U = inputs.conserved(rho, z, z, z, p, bx, by, bz, gam)
+        cfg = oracle.make_config(N=4, g=g, gamma=gam, scheme=scheme, recon=recon, riemann=riemann)
+        adv = lambda Ui, Bi, dt, dh_: oracle.advance(cfg, Ui, Bi, dt, dh_)
+        t, tend = 0.0, 0.15
+        while t < tend * (1 - 1e-12):
+            dt = min(0.3 * dh / 2.3, tend - t)            # max |v|+c ~ 2.2 in Sod
+            U, bx, by, bz, _, _ = H.step_grid(adv, U, bx, by, bz, dt, dh, 4, g)
+            t += dt
+        sl = [0, 0, 0]; sl[2 - axis] = slice(None)
+        rho_num = U[0][tuple(sl)]
+        m = (xc > 0.05) & (xc < 0.95)                     # the tube centred at x = +0.5
+        ex = _sod_exact(xc[m] - 0.5, tend, gam)
+        errs.append(np.mean(np.abs(rho_num[m] - ex)))
+        assert rho_num.min() > 0.124 and rho_num.max() < 1.0 + 1e-2      # no oscillation > 1 %
+        assert np.abs(bx).max() == 0 and np.abs(by).max() == 0 and np.abs(bz).max() == 0
+        # transverse invariance
+        assert np.ptp(U[0], axis=tuple(a for a in range(3) if a != 2 - axis)).max() < 1e-14
+    print(name, axis, errs)
+    assert errs[1] < 0.012 and errs[0] / errs[1] > 1.6, errs

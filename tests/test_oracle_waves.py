@@ -1,0 +1,76 @@
+"""Pin P5: second-order convergence of small-amplitude linear waves (Fig. 4).
+
+The eigenvectors come from tests/golden/linear_wave_modes.txt, not from the oracle; they are checked here against
+the finite-difference Jacobian of Eq. 7 typed out below, so that a wrong fixture cannot hide a bug.
+"""
+import numpy as np
+import pytest
+
+from paper_1804_03479_b200 import inputs
+import harness as H
+import waves
+
+G = 5.0 / 3.0
+
+
+def _flux_cons(U, Bn):
+    rho = U[0]; v = U[1:4] / rho; B = np.array([Bn, U[5], U[6]])
+    P = (G - 1) * (U[4] - 0.5 * rho * v @ v - 0.5 * B @ B)
+    pt = P + 0.5 * B @ B
+    return np.array([rho * v[0], rho * v[0] * v[0] + pt - Bn * Bn, rho * v[0] * v[1] - Bn * B[1], rho * v[0] * v[2] - Bn * B[2],
+                     (U[4] + pt) * v[0] - Bn * (B @ v), B[1] * v[0] - Bn * v[1], B[2] * v[0] - Bn * v[2]])
+
+
+def test_fixture_vectors_are_eigenvectors_of_eq7():
+    m = waves.load_modes()
+    W0 = m["background"]
+    U0 = np.array([W0[0], 0, 0, 0, W0[4] / (G - 1) + 0.5 * (W0[5] ** 2 + W0[6] ** 2 + W0[7] ** 2), W0[6], W0[7]])
+    J = np.empty((7, 7))
+    for c in range(7):
+        h = 1e-6
+        Up = U0.copy(); Um = U0.copy(); Up[c] += h; Um[c] -= h
+        J[:, c] = (_flux_cons(Up, W0[5]) - _flux_cons(Um, W0[5])) / (2 * h)
+    for name in ("fast", "alfven", "slow"):
+        spd, R = m[name][0], m[name][1:]
+        assert np.abs(J @ R - spd * R).max() < 1e-8, name
+
+
+CASES = [("vl_plm", 0, 0, 3, 1), ("vl_plm_roe", 0, 0, 3, 2), ("ctu_plm", 1, 0, 3, 1), ("ctu_ppm", 1, 1, 4, 1), ("ctu_ppm_roe", 1, 1, 4, 2)]
+
+
+def _run_axis(oracle, scheme, recon, g, riemann, mode, axis, N):
+    U, bx, by, bz, dh, spd = waves.axis_wave(N, axis, mode, NT=4)
+    cfg = oracle.make_config(N=4, g=g, scheme=scheme, recon=recon, riemann=riemann)
+    adv = lambda Ui, Bi, dt, dh_: oracle.advance(cfg, Ui, Bi, dt, dh_)
+    dt_fn = lambda U_, a, b, c, dh_, cfl: cfl * dh_ / 2.0          # c_f = 2 is the largest speed of the background
+    return waves.run_period(adv, dt_fn, U, bx, by, bz, dh, 1.0 / spd, 4, g)
+
+
+@pytest.mark.parametrize("name,scheme,recon,g,riemann", CASES)
+@pytest.mark.parametrize("mode", ["fast", "alfven", "slow"])
+def test_p5_axis_waves_converge_at_second_order(oracle, name, scheme, recon, g, riemann, mode):
+    axis = {"fast": 0, "alfven": 1, "slow": 2}[mode]
+    e16 = _run_axis(oracle, scheme, recon, g, riemann, mode, axis, 16)[0]
+    e32 = _run_axis(oracle, scheme, recon, g, riemann, mode, axis, 32)[0]
+    order = np.log2(e16 / e32)
+    assert order > 1.5, (e16, e32, order)
+    assert e32 < 6e-8           # amplitude 1e-6: a first-order scheme leaves ~2e-7 at N = 32
+
+
+def test_p5_axes_are_equivalent(oracle):
+    e = [_run_axis(oracle, 0, 0, 3, 1, "slow", ax, 16)[0] for ax in range(3)]
+    assert max(e) - min(e) < 1e-7 * max(e) + 1e-15
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name,scheme,recon,g,riemann", [CASES[0], CASES[3]])
+def test_p5_diagonal_fast_wave(oracle, name, scheme, recon, g, riemann):
+    errs = []
+    for N in (16, 32):
+        U, bx, by, bz, dh, spd, lam = waves.diagonal_wave(N, "fast")
+        assert H.rel_divb(bx, by, bz, dh) < 1e-13
+        cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon, riemann=riemann)
+        adv = lambda Ui, Bi, dt, dh_: oracle.advance(cfg, Ui, Bi, dt, dh_)
+        dt_fn = lambda U_, a, b, c, dh_, cfl: cfl * dh_ / 2.0
+        errs.append(waves.run_period(adv, dt_fn, U, bx, by, bz, dh, lam / spd, N, g)[0])
+    assert np.log2(errs[0] / errs[1]) > 1.5, errs
