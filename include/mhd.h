@@ -1,0 +1,115 @@
+/* =====================================================================================
+ * mhd.h -- C ABI of the B200 patch-group MHD solver (libmhd.so).
+ *
+ * The hot path of GAMER-MHD (Zhang, Schive & Chiueh 2018; citations are PAPER.md:<line>):
+ * the unsplit second-order Godunov update of a batch of ghost-zoned patch groups
+ * by the VL / MUSCL-Hancock scheme (7 steps) or the CTU
+ * scheme (8 steps), with PLM/PPM reconstruction, an HLLE/HLLD/Roe Riemann
+ * solver and constrained transport of the face-centred magnetic field
+ * (Eq. 13), plus the CFL time-step reduction.
+ * Where the paper is silent the readings R1-R18 of DESIGN.md apply.
+ *
+ * Every step runs in hand-written CUDA kernels for sm_100a.  There is no CPU fallback: every
+ * call fails with MHD_ECUDA when no CUDA device is usable.
+ *
+ * ---- array layouts (per group, contiguous; groups outermost; SoA; index order [k][j][i], x fastest) ----
+ * N = ps2 interior cells per side, g = nghost, T = N + 2g.  Real = float (MHD_FP32) or double (MHD_FP64).
+ *   U_in  [G][5][T][T][T]      (rho, Mx, My, Mz, e); e includes 1/2 Bc^2, Bc = mean of the two faces (Eq. 5)
+ *   B_in  [G]{ Bx[T][T][T+1] | By[T][T+1][T] | Bz[T+1][T][T] }   Bx[k][j][i] = field on face i-1/2 of cell (i,j,k) (Fig. 1)
+ *   U_out [G][5][N][N][N]
+ *   B_out [G]{ Bx[N][N][N+1] | By[N][N+1][N] | Bz[N+1][N][N] }   interior faces incl. both boundary planes
+ *   flux_out [G][9][5][N][N]   plane p = 3*d + s; d = normal (x,y,z); s = 0 lower boundary face plane (face index 0),
+ *                              1 mid plane (index N/2, boundary between the two patches), 2 upper boundary (index N);
+ *                              5 = time-centred fluxes of (rho,Mx,My,Mz,e) used in the final update, NOT multiplied
+ *                              by dt or area; [N][N] = (t2,t1) transverse cell indices, t1 fastest, (d,t1,t2) cyclic
+ *   emf_out  [G][9][2][(N+1)*N] same 9 planes; component 0 = E_t1 on the plane's edges along t1, [N+1 in t2][N in t1];
+ *                              component 1 = E_t2 on edges along t2, [N in t2][N+1 in t1]
+ * ===================================================================================== */
+#ifndef MHD_B200_H
+#define MHD_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mhd_solver mhd_solver; /* opaque; owns the device workspace, streams and staging buffers */
+
+typedef enum { MHD_FP32 = 0, MHD_FP64 = 1 } mhd_precision;
+typedef enum { MHD_VL = 0, MHD_CTU = 1 } mhd_scheme;            /* PAPER.md:191-197 / :176-183 */
+typedef enum { MHD_PLM = 0, MHD_PPM = 1 } mhd_recon;
+typedef enum { MHD_HLLE = 0, MHD_HLLD = 1, MHD_ROE = 2 } mhd_riemann;
+typedef enum { MHD_LIM_PRIM = 0, MHD_LIM_CHAR = 1 } mhd_limvar; /* limiter in primitive / characteristic variables */
+
+typedef struct {
+  int ps2;          /* N: interior cells per side of a patch group; 16 = 2 patches of 8; even, 8..64 */
+  int nghost;       /* g: >= 3 for PLM, >= 4 for PPM (R8); exactly the ghost width of the arrays passed in */
+  double gamma;     /* ratio of specific heats, > 1 (5/3 in every paper test) */
+  int scheme;       /* mhd_scheme; VL+PPM is rejected */
+  int recon;        /* mhd_recon */
+  int riemann;      /* mhd_riemann */
+  int limvar;       /* mhd_limvar */
+  int prec;         /* mhd_precision: element type of every array argument */
+  double min_dens;  /* floors applied to DERIVED primitive states only (R9); conserved output is never floored */
+  double min_pres;
+  double emf_tie;   /* CT upwinding tie (R7a): a face mass flux m with |m| dt/dh <= emf_tie * (mean density of the
+                       two cells) counts as zero and takes the centred average; <= 0 selects 1e-12 (FP64) / 1e-5 (FP32) */
+  int max_groups;   /* largest ngroups of one mhd_advance call (bounds nothing but argument checking) */
+  int device;       /* CUDA device ordinal */
+} mhd_config;
+
+enum { MHD_OK = 0, MHD_EINVAL = -1, MHD_ECUDA = -2, MHD_ENOMEM = -3 };
+
+/* Create a solver.  Allocates the device workspace (sized for an L2-resident slice of groups, not for
+ * max_groups).  Returns MHD_EINVAL for a bad configuration (incl. too small a ghost width), MHD_ECUDA /
+ * MHD_ENOMEM for device errors.  *out is NULL on failure. */
+int mhd_create(const mhd_config* cfg, mhd_solver** out);
+int mhd_destroy(mhd_solver* s);
+
+/* Element counts PER GROUP of the six arrays (any pointer may be NULL). */
+int mhd_sizes(const mhd_solver* s, size_t* n_U_in, size_t* n_B_in, size_t* n_U_out, size_t* n_B_out,
+              size_t* n_flux, size_t* n_emf);
+
+/* Advance ngroups patch groups by dt with cell size dh (one pass of the whole scheme, PAPER.md:176-183 / :191-197).
+ * All array pointers are DEVICE pointers owned by the caller, laid out as above in the solver's precision.
+ * flux_out and emf_out may each be NULL.  Asynchronous on cuda_stream (a cudaStream_t; NULL = default stream);
+ * allocates nothing and never synchronises.  Outputs must not alias inputs.  ngroups = 0 is a no-op.
+ * Errors: MHD_EINVAL (null pointer, ngroups < 0 or > max_groups, dt or dh not finite/positive), MHD_ECUDA (launch). */
+int mhd_advance(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out,
+                void* flux_out, void* emf_out, int ngroups, double dt, double dh, void* cuda_stream);
+
+/* Same update with HOST pointers (pinned memory gives the overlap; pageable memory works but serialises).
+ * The batch is cut into chunks of chunk_groups; chunk c runs H2D -> kernels -> D2H on stream c % nstreams so that
+ * copy-in, compute and copy-out of successive chunks overlap.  Blocking.  1 <= nstreams <= 8,
+ * 1 <= chunk_groups <= max_groups.  flux_out / emf_out may be NULL. */
+int mhd_advance_host(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out,
+                     void* flux_out, void* emf_out, int ngroups, double dt, double dh,
+                     int chunk_groups, int nstreams);
+
+/* CFL time step (R13): dt = cfl * dh / max over interior cells and directions d of
+ * (|v_d| + c_f,d), cell-centred B = face mean.  U, B: DEVICE arrays of ngroups groups whose ghost width is
+ * nghost_of_arrays (0: the U_out/B_out layout; cfg.nghost: the U_in/B_in layout).  dt_out (required) and
+ * maxspeed_out (nullable) are HOST pointers; the call synchronises cuda_stream. */
+int mhd_dt_reduce(mhd_solver* s, const void* U, const void* B, int ngroups, int nghost_of_arrays,
+                  double dh, double cfl, double* dt_out, double* maxspeed_out, void* cuda_stream);
+
+/* Cumulative event counters since creation (density floors, pressure floors, Roe->HLLE fallbacks).
+ * Synchronises the device; asynchronous kernel faults surface here as MHD_ECUDA. */
+int mhd_get_stats(mhd_solver* s, unsigned long long* n_floor_dens, unsigned long long* n_floor_pres,
+                  unsigned long long* n_riemann_fallback);
+
+/* Number of kernel launches issued by this solver since creation (bench.py's gpu_launches). */
+unsigned long long mhd_launch_count(const mhd_solver* s);
+
+/* Register-only FMA-chain micro-kernel: measured FP32 (prec=0) or FP64 (prec=1) FMA peak of this device in
+ * TFLOP/s (2 flop per FMA), used as the ALU roofline denominator beside the nominal figure. */
+int mhd_measure_fma_peak(int device, int prec, double* tflops_out);
+
+/* Message for a return code; for MHD_ECUDA the last CUDA error string seen by this thread. */
+const char* mhd_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MHD_B200_H */

@@ -39,6 +39,7 @@ typedef struct {
   int riemann;  // 0 HLLE, 1 HLLD, 2 ROE
   int limvar;   // 0 primitive, 1 characteristic
   double min_dens, min_pres;
+  double emf_tie;  // reading R7a: width of the linear blend of the CT upwind switch, in units of (mean cell density) * dh/dt
 } mhdref_config;
 }
 
@@ -417,7 +418,22 @@ struct Group {
       auto Ea = [&](size_t q) { return -F[a][5][q]; };
       auto Eb = [&](size_t q) { return F[bdir][6][q]; };
       auto ec = [&](size_t q) { return Wc[1 + bdir][q] * Wc[5 + a][q] - Wc[1 + a][q] * Wc[5 + bdir][q]; };  // -(v x B)_c
-      auto up = [](double m, double qm, double qp) { return m > 0.0 ? qm : (m < 0.0 ? qp : 0.5 * (qm + qp)); };
+      // upwinding by the sign of the face mass flux m (reading R7): q- if m > 0, q+ if m < 0, the mean if m = 0.
+      // Reading R7a: "m = 0" means |m| <= m0 = emf_tie * (mean density of the two cells) * dh/dt, i.e. less than emf_tie
+      // of the cell mass crosses the face in dt (zero at working precision); between m0 and 2 m0 the switch ramps
+      // linearly from the mean to the upwind value, so that the EMF is a continuous function of m.
+      const double tie = c.emf_tie * dh / dt;
+      auto up = [tie](double m, double rm, double rp, double qm, double qp) {
+        double m0 = tie * 0.5 * (rm + rp), am = std::fabs(m);
+        if (am <= m0) return 0.5 * (qm + qp);
+        if (am < 2.0 * m0) {
+          double w = (am - m0) / m0;                       // 0..1: weight of the upwind value
+          double qu = m > 0.0 ? qm : qp;
+          return w * qu + (1.0 - w) * (0.5 * (qm + qp));
+        }
+        return m > 0.0 ? qm : qp;
+      };
+      const Arr& rho = Wc[0];
       int idx[3];
       for (idx[cdir] = clo; idx[cdir] < chi; ++idx[cdir])
         for (idx[bdir] = alo; idx[bdir] <= ahi; ++idx[bdir])
@@ -427,8 +443,8 @@ struct Group {
             double e = 0.25 * (Ea(q) + Ea(qb) + Eb(q) + Eb(qa));
             double ma_lo = F[a][0][qb], ma_hi = F[a][0][q];       // mass flux through a-face (a-1/2, b-1) and (a-1/2, b)
             double mb_lo = F[bdir][0][qa], mb_hi = F[bdir][0][q]; // through b-face (a-1, b-1/2) and (a, b-1/2)
-            e += 0.25 * (up(ma_lo, Eb(qa) - ec(qab), Eb(q) - ec(qb)) - up(ma_hi, ec(qa) - Eb(qa), ec(q) - Eb(q)));
-            e += 0.25 * (up(mb_lo, Ea(qb) - ec(qab), Ea(q) - ec(qa)) - up(mb_hi, ec(qb) - Ea(qb), ec(q) - Ea(q)));
+            e += 0.25 * (up(ma_lo, rho[qab], rho[qb], Eb(qa) - ec(qab), Eb(q) - ec(qb)) - up(ma_hi, rho[qa], rho[q], ec(qa) - Eb(qa), ec(q) - Eb(q)));
+            e += 0.25 * (up(mb_lo, rho[qab], rho[qa], Ea(qb) - ec(qab), Ea(q) - ec(qa)) - up(mb_hi, rho[qb], rho[q], ec(qb) - Ea(qb), ec(q) - Ea(q)));
             E[cdir][q] = e;
           }
     }
@@ -724,6 +740,7 @@ int check_cfg(const mhdref_config* c) {
   int need = c->recon == 1 ? 4 : 3;                        // reading R8
   if (c->nghost < need) return -1;
   if (!(c->gamma > 1.0)) return -1;
+  if (!(c->emf_tie >= 0.0)) return -1;
   return 0;
 }
 

@@ -1,0 +1,136 @@
+// mhd_kernels3.cuh -- full update, coarse-fine boundary planes and the
+// CFL reduction.  See mhd_kernels.cuh for the layout.
+#pragma once
+#include "mhd_kernels2.cuh"
+
+namespace mhd {
+
+// ---- S8: U^{n+1} = U^n - dt/dh sum dF2 (Eq. 10) on the N^3 interior cells, b^{n+1} by Eq. 13 on their faces -------
+template <class R>
+__global__ void __launch_bounds__(256) k_final(const KParams<R> p) {
+  Ctx<R> c(p);
+  if (!c.valid()) return;
+  const int g = p.g, N = p.N;
+  const int ii = c.i - g, jj = c.j - g, kk = c.k - g;
+  if (ii < 0 || ii >= N || jj < 0 || jj >= N || kk < 0 || kk >= N) return;
+  const R qh = p.dt / p.dh;
+  R u[5], dU[5];
+  load_U_in(p, c, u);
+  flux_div(c, dU);
+  R* Uo = p.Uout + (size_t)c.grp * p.nUo;
+  const size_t N3 = (size_t)N * N * N, cq = ((size_t)kk * N + jj) * N + ii;
+#pragma unroll
+  for (int v = 0; v < 5; ++v) Uo[v * N3 + cq] = u[v] - qh * dU[v];
+  R* Bx = p.Bout + (size_t)c.grp * p.nBo;
+  R* By = Bx + (size_t)N * N * (N + 1);
+  R* Bz = By + (size_t)N * N * (N + 1);
+  const int q = c.q;
+  Bx[((size_t)kk * N + jj) * (N + 1) + ii] = ct_face<R, 0>(c, c.arr(A_B + 0), q, qh);
+  By[((size_t)kk * (N + 1) + jj) * N + ii] = ct_face<R, 1>(c, c.arr(A_B + 1), q, qh);
+  Bz[((size_t)kk * N + jj) * N + ii] = ct_face<R, 2>(c, c.arr(A_B + 2), q, qh);
+  if (ii == N - 1) Bx[((size_t)kk * N + jj) * (N + 1) + N] = ct_face<R, 0>(c, c.arr(A_B + 0), q + 1, qh);
+  if (jj == N - 1) By[((size_t)kk * (N + 1) + N) * N + ii] = ct_face<R, 1>(c, c.arr(A_B + 1), q + p.S, qh);
+  if (kk == N - 1) Bz[((size_t)N * N + jj) * N + ii] = ct_face<R, 2>(c, c.arr(A_B + 2), q + p.S2, qh);
+}
+
+// ---- epilogue: time-centred fluxes and edge EMFs on the lower / mid / upper face planes of each direction ----------
+// one thread per (plane, a2, a1) with a1, a2 in [0, N]
+template <class R>
+__global__ void __launch_bounds__(256) k_planes(const KParams<R> p) {
+  const int N = p.N, M = N + 1, g = p.g;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= 9 * M * M) return;
+  const int grp = blockIdx.z;
+  const int a1 = t % M, a2 = (t / M) % M, pl = t / (M * M);
+  const int d = pl / 3, s = pl % 3, t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+  int id[3];
+  id[d] = (s == 0 ? 0 : (s == 1 ? N / 2 : N)) + g; id[t1] = a1 + g; id[t2] = a2 + g;
+  const int q = (id[2] * p.S + id[1]) * p.S + id[0];
+  const R* w = p.ws + (size_t)grp * p.narr * p.S3;
+  if (p.fout && a1 < N && a2 < N) {
+    const R* F = w + (size_t)(A_F + 7 * d) * p.S3;
+    R fg[5];
+    fg[0] = F[q]; fg[1 + d] = F[(size_t)p.S3 + q]; fg[1 + t1] = F[(size_t)2 * p.S3 + q]; fg[1 + t2] = F[(size_t)3 * p.S3 + q];
+    fg[4] = F[(size_t)4 * p.S3 + q];
+    R* fo = p.fout + (size_t)grp * p.nF + (size_t)pl * 5 * N * N + (size_t)a2 * N + a1;
+#pragma unroll
+    for (int v = 0; v < 5; ++v) fo[(size_t)v * N * N] = fg[v];
+  }
+  if (p.eout) {
+    R* e0 = p.eout + (size_t)grp * p.nE + (size_t)pl * 2 * M * N;
+    R* e1 = e0 + (size_t)M * N;
+    if (a1 < N) e0[(size_t)a2 * N + a1] = w[(size_t)(A_E + t1) * p.S3 + q];
+    if (a2 < N) e1[(size_t)a2 * M + a1] = w[(size_t)(A_E + t2) * p.S3 + q];
+  }
+}
+
+// ---- S9: CFL (R13): max over interior cells and directions of |v_d| + c_f,d -------------------
+// speeds are >= 0, so their IEEE bit patterns order like unsigned integers: one atomicMax per block.
+template <class R> struct Bits;
+template <> struct Bits<float> {
+  typedef unsigned int U;
+  static __device__ __forceinline__ U enc(float x) { return __float_as_uint(x); }
+};
+template <> struct Bits<double> {
+  typedef unsigned long long U;
+  static __device__ __forceinline__ U enc(double x) { return (U)__double_as_longlong(x); }
+};
+
+template <class R>
+__global__ void __launch_bounds__(256) k_dt(const R* __restrict__ U, const R* __restrict__ B, int N, int ng, long long nU,
+                                            long long nB, R gam, R min_dens, R min_pres, unsigned long long* out) {
+  const int T = N + 2 * ng;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  R smax = R(0);
+  if (t < N * N * N) {
+    const int i = t % N + ng, j = (t / N) % N + ng, k = t / (N * N) + ng;
+    const R* u = U + (size_t)blockIdx.z * nU;
+    const R* bx = B + (size_t)blockIdx.z * nB;
+    const R* by = bx + (size_t)T * T * (T + 1);
+    const R* bz = by + (size_t)T * T * (T + 1);
+    const size_t T3 = (size_t)T * T * T, cq = ((size_t)k * T + j) * T + i;
+    const size_t qx = ((size_t)k * T + j) * (T + 1) + i, qy = ((size_t)k * (T + 1) + j) * T + i;
+    const R Bc[3] = { R(0.5) * (bx[qx] + bx[qx + 1]), R(0.5) * (by[qy] + by[qy + T]), R(0.5) * (bz[cq] + bz[cq + (size_t)T * T]) };
+    const R rho = Num<R>::max(u[cq], min_dens);
+    const R v[3] = { u[T3 + cq] / rho, u[2 * T3 + cq] / rho, u[3 * T3 + cq] / rho };
+    const R b2 = Bc[0] * Bc[0] + Bc[1] * Bc[1] + Bc[2] * Bc[2];
+    R P = (gam - R(1)) * (u[4 * T3 + cq] - R(0.5) * rho * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) - R(0.5) * b2);
+    P = Num<R>::max(P, min_pres);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const R bn2 = Bc[d] * Bc[d];
+      smax = Num<R>::max(smax, Num<R>::abs(v[d]) + fast_speed(rho, P, bn2, b2 - bn2, gam));
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) smax = Num<R>::max(smax, __shfl_xor_sync(0xffffffffu, smax, o));
+  __shared__ R red[8];
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = smax;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    R m = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : R(0);
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) m = Num<R>::max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (threadIdx.x == 0) atomicMax(reinterpret_cast<typename Bits<R>::U*>(out), Bits<R>::enc(m));
+  }
+}
+
+// ---- register-only FMA chains: measured FP32 / FP64 FMA peak (ALU roofline denominator) ----------------
+template <class R>
+__global__ void __launch_bounds__(256) k_fma_peak(R* out, int iters) {
+  R a[8], x = R(1.0000001), y = R(1e-9) * threadIdx.x;
+#pragma unroll
+  for (int v = 0; v < 8; ++v) a[v] = R(v) + y;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+      for (int v = 0; v < 8; ++v) a[v] = a[v] * x + y;
+  }
+  R s = R(0);
+#pragma unroll
+  for (int v = 0; v < 8; ++v) s += a[v];
+  if (s == R(-1)) out[0] = s;
+}
+
+}  // namespace mhd

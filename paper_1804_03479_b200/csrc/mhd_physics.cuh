@@ -1,0 +1,185 @@
+// mhd_physics.cuh -- per-face / per-cell device arithmetic of the patch-group MHD update (sm_100a).
+//
+// Register-resident formulations of: the ideal-MHD flux (Eq. 7), the gamma-law total energy
+// (Eq. 5), the HLLE / HLLD / Roe Riemann solvers the paper names, the MC-limited
+// PLM and PPM reconstructions in primitive or characteristic variables, and the CTU
+// characteristic tracing in matrix form (R5).  The formulas the paper leaves to its references are
+// the readings of DESIGN.md (R1-R18).  Everything is a template on Real (float / double); divisions are
+// turned into shared reciprocals and all branches of a solver are evaluated and selected at the end so that
+// a warp never diverges on the wave pattern.
+//
+// Generic 1-D state of direction n: W = (rho, vn, vt1, vt2, P, Bt1, Bt2) with the normal field Bn passed
+// separately; conserved U = (rho, Mn, Mt1, Mt2, e, Bt1, Bt2).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace mhd {
+
+enum : int { kHLLE = 0, kHLLD = 1, kROE = 2 };
+enum : int { kPLM = 0, kPPM = 1 };
+enum : int { kLimPrim = 0, kLimChar = 1 };
+
+template <class R> struct Num;
+template <> struct Num<float> {
+  static __device__ __forceinline__ float sqrt(float x) { return sqrtf(x); }
+  static __device__ __forceinline__ float abs(float x) { return fabsf(x); }
+  static __device__ __forceinline__ float min(float a, float b) { return fminf(a, b); }
+  static __device__ __forceinline__ float max(float a, float b) { return fmaxf(a, b); }
+};
+template <> struct Num<double> {
+  static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
+  static __device__ __forceinline__ double abs(double x) { return fabs(x); }
+  static __device__ __forceinline__ double min(double a, double b) { return fmin(a, b); }
+  static __device__ __forceinline__ double max(double a, double b) { return fmax(a, b); }
+};
+
+template <class R> __device__ __forceinline__ R sqr(R x) { return x * x; }
+
+// monotonised-central limiter (R5)
+template <class R> __device__ __forceinline__ R lim_mc(R a, R b) {
+  R s = a + b;
+  R m = Num<R>::min(R(0.5) * Num<R>::abs(s), R(2) * Num<R>::min(Num<R>::abs(a), Num<R>::abs(b)));
+  m = (s > R(0)) ? m : -m;
+  return (a * b <= R(0)) ? R(0) : m;
+}
+// minmod of the CTU multidimensional MHD source terms (R6)
+template <class R> __device__ __forceinline__ R lim_minmod(R a, R b) {
+  R m = Num<R>::min(Num<R>::abs(a), Num<R>::abs(b));
+  m = (a > R(0)) ? m : -m;
+  return (a * b <= R(0)) ? R(0) : m;
+}
+
+// ---- one side of a face: everything the solvers need from a primitive state -------------------------------
+template <class R> struct Side {
+  R U[7];   // conserved (Eq. 5)
+  R F[7];   // physical flux (Eq. 7)
+  R pT;     // P + B^2/2
+  R vB;     // v.B
+  R cf;     // fast speed along n
+  R g;      // cf^2 - ca^2 >= 0, evaluated without cancellation (HLLD star-state denominators)
+};
+
+template <class R>
+__device__ __forceinline__ void side_setup(const R (&w)[7], R bn, R bn2, R gm1inv, R gam, Side<R>& s) {
+  R bt2 = w[5] * w[5] + w[6] * w[6];
+  R pmag = R(0.5) * (bn2 + bt2);
+  R v2 = w[1] * w[1] + w[2] * w[2] + w[3] * w[3];
+  s.pT = w[4] + pmag;
+  s.vB = bn * w[1] + w[5] * w[2] + w[6] * w[3];
+  R mn = w[0] * w[1];
+  s.U[0] = w[0]; s.U[1] = mn; s.U[2] = w[0] * w[2]; s.U[3] = w[0] * w[3];
+  s.U[4] = w[4] * gm1inv + R(0.5) * w[0] * v2 + pmag;
+  s.U[5] = w[5]; s.U[6] = w[6];
+  s.F[0] = mn;
+  s.F[1] = mn * w[1] + s.pT - bn2;
+  s.F[2] = mn * w[2] - bn * w[5];
+  s.F[3] = mn * w[3] - bn * w[6];
+  s.F[4] = (s.U[4] + s.pT) * w[1] - bn * s.vB;
+  s.F[5] = w[5] * w[1] - bn * w[2];
+  s.F[6] = w[6] * w[1] - bn * w[3];
+  // c_f^2 = 1/2 [ (a^2+ca^2+ct^2) + sqrt( (ca^2+ct^2-a^2)^2 + 4 a^2 ct^2 ) ]   (R1, R18)
+  R ir = R(1) / w[0];
+  R a2 = gam * w[4] * ir, ca2 = bn2 * ir, ct2 = bt2 * ir;
+  R sum = a2 + ca2 + ct2, dif = ca2 + ct2 - a2;
+  R root = Num<R>::sqrt(dif * dif + R(4) * a2 * ct2);
+  s.cf = Num<R>::sqrt(R(0.5) * (sum + root));
+  // cf^2 - ca^2 = 1/2 (x + root), x = a^2 + ct^2 - ca^2 (root^2 = x^2 + 4 ca^2 ct^2); rationalised where x < 0
+  R x = a2 + ct2 - ca2;
+  s.g = (x >= R(0)) ? R(0.5) * (x + root) : R(2) * ca2 * ct2 / (root - x);
+}
+
+template <class R>
+__device__ __forceinline__ R fast_speed(R rho, R P, R bn2, R bt2, R gam) {
+  R ir = R(1) / rho;
+  R a2 = gam * P * ir, ca2 = bn2 * ir, ct2 = bt2 * ir;
+  R sum = a2 + ca2 + ct2, dif = ca2 + ct2 - a2;
+  return Num<R>::sqrt(R(0.5) * (sum + Num<R>::sqrt(dif * dif + R(4) * a2 * ct2)));
+}
+
+// ---- HLLD (Miyoshi & Kusano form; R7/R12) ------------------------------------------------
+template <class R>
+__device__ __forceinline__ void riemann_hlld(const R (&wl)[7], const R (&wr)[7], R bn, R gam, R gm1inv, R (&F)[7]) {
+  const R bn2 = bn * bn;
+  Side<R> L, Rr;
+  side_setup(wl, bn, bn2, gm1inv, gam, L);
+  side_setup(wr, bn, bn2, gm1inv, gam, Rr);
+  const R uL = wl[1], uR = wr[1];
+  const bool lmax = L.cf >= Rr.cf;
+  const R cmax = lmax ? L.cf : Rr.cf;
+  const R SL = Num<R>::min(uL, uR) - cmax, SR = Num<R>::max(uL, uR) + cmax;
+  const R sL = (SL - uL) * wl[0], sR = (SR - uR) * wr[0];
+  const R idn = R(1) / (sR - sL);
+  // contact speed through the differences u_L - u_R and pT_R - pT_L taken directly from the inputs, so that slow
+  // flows in a strong field keep their significant digits (the textbook quotient subtracts O(pT) terms)
+  const R du = uL - uR;
+  const R dp = (wr[4] - wl[4]) + R(0.5) * ((wr[5] - wl[5]) * (wr[5] + wl[5]) + (wr[6] - wl[6]) * (wr[6] + wl[6]));
+  const R uLmSM = (sR * du + dp) * idn, uRmSM = (sL * du + dp) * idn;     // u_alpha - S_M
+  const R SM = uL - uLmSM;
+  const R pTs = (sR * L.pT - sL * Rr.pT + sL * sR * (uR - uL)) * idn;
+  const R tiny = R(1e-12) * pTs;
+  // rho (S-u)^2 - Bn^2 of each side without cancellation: (S-u)^2 = (cmax + delta)^2, cmax^2 = ca_m^2 + g_m
+  const R delta = Num<R>::max(du, R(0));
+  const R gm = lmax ? L.g : Rr.g, rhom = lmax ? wl[0] : wr[0];
+  const R grow = gm + delta * (R(2) * cmax + delta);
+
+  // star states of both sides (the double-star state needs both)
+  R rs[2], v1s[2], v2s[2], b1s[2], b2s[2], es[2], vBs[2], sq[2];
+#pragma unroll
+  for (int a = 0; a < 2; ++a) {
+    const R (&w)[7] = a ? wr : wl;
+    const Side<R>& s = a ? Rr : L;
+    const R Sa = a ? SR : SL, sa = a ? sR : sL, umSM = a ? uRmSM : uLmSM;
+    const R dSM = (Sa - w[1]) + umSM, idSM = R(1) / dSM;      // S_alpha - S_M
+    rs[a] = sa * idSM;
+    const R Nb = w[0] * grow + bn2 * (w[0] - rhom) / rhom;     // rho (S-u)^2 - Bn^2
+    const R D = Nb + sa * umSM;                                // rho (S-u)(S-S_M) - Bn^2
+    const bool degen = Num<R>::abs(D) < tiny;
+    const R iD = R(1) / D;
+    const R fv = degen ? R(0) : -bn * umSM * iD;
+    const R fb = degen ? R(1) : Nb * iD;
+    v1s[a] = w[2] - w[5] * fv; v2s[a] = w[3] - w[6] * fv;
+    b1s[a] = w[5] * fb; b2s[a] = w[6] * fb;
+    vBs[a] = bn * SM + b1s[a] * v1s[a] + b2s[a] * v2s[a];
+    es[a] = ((Sa - w[1]) * s.U[4] - s.pT * w[1] + pTs * SM + bn * (s.vB - vBs[a])) * idSM;
+    sq[a] = Num<R>::sqrt(rs[a]);
+  }
+  const R abn = Num<R>::abs(bn);
+  const R SsL = SM - abn / sq[0], SsR = SM + abn / sq[1];
+
+  // which side of the contact the face lies on, and in which region of that side
+  const bool left = (SL >= R(0)) || (SsL >= R(0)) || (SM >= R(0));
+  const bool outer = left ? (SL >= R(0)) : !(SR >= R(0));           // plain F_L / F_R
+  const bool star = left ? (SsL >= R(0)) : !(SsR >= R(0));          // single-star region (if not outer)
+  const R Sa = left ? SL : SR, Ssa = left ? SsL : SsR;
+  const R r_s = left ? rs[0] : rs[1], sq_a = left ? sq[0] : sq[1];
+  const R v1a = left ? v1s[0] : v1s[1], v2a = left ? v2s[0] : v2s[1];
+  const R b1a = left ? b1s[0] : b1s[1], b2a = left ? b2s[0] : b2s[1];
+  const R esa = left ? es[0] : es[1], vBa = left ? vBs[0] : vBs[1];
+  R Us[7] = { r_s, r_s * SM, r_s * v1a, r_s * v2a, esa, b1a, b2a };
+  R Uss[7];
+  if (R(0.5) * bn2 < tiny) {
+#pragma unroll
+    for (int c = 0; c < 7; ++c) Uss[c] = Us[c];
+  } else {
+    const R sg = bn > R(0) ? R(1) : R(-1);
+    const R ir = R(1) / (sq[0] + sq[1]);
+    const R v1 = (sq[0] * v1s[0] + sq[1] * v1s[1] + (b1s[1] - b1s[0]) * sg) * ir;
+    const R v2 = (sq[0] * v2s[0] + sq[1] * v2s[1] + (b2s[1] - b2s[0]) * sg) * ir;
+    const R b1 = (sq[0] * b1s[1] + sq[1] * b1s[0] + sq[0] * sq[1] * (v1s[1] - v1s[0]) * sg) * ir;
+    const R b2 = (sq[0] * b2s[1] + sq[1] * b2s[0] + sq[0] * sq[1] * (v2s[1] - v2s[0]) * sg) * ir;
+    const R vBss = bn * SM + b1 * v1 + b2 * v2;
+    const R pm = left ? R(-1) : R(1);
+    Uss[0] = Us[0]; Uss[1] = Us[1]; Uss[2] = r_s * v1; Uss[3] = r_s * v2;
+    Uss[4] = esa + pm * sq_a * (vBa - vBss) * sg;
+    Uss[5] = b1; Uss[6] = b2;
+  }
+#pragma unroll
+  for (int c = 0; c < 7; ++c) {
+    const R Fa = left ? L.F[c] : Rr.F[c], Ua = left ? L.U[c] : Rr.U[c];
+    const R f_star = Fa + Sa * (Us[c] - Ua);
+    const R f_dstar = Fa + Ssa * Uss[c] - (Ssa - Sa) * Us[c] - Sa * Ua;
+    F[c] = outer ? Fa : (star ? f_star : f_dstar);
+  }
+}
+
+}  // namespace mhd

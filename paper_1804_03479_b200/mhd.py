@@ -1,0 +1,172 @@
+"""Thin Python binding of libmhd.so (include/mhd.h).  Argument marshalling only.
+
+Every step of the update runs in the CUDA kernels behind the C ABI; this module owns no arithmetic and has no
+fallback: if the library is missing or no CUDA device is usable it raises.  torch is used for device memory
+and streams only (tensor.data_ptr(), torch.cuda.current_stream()).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "libmhd.so")
+
+FP32, FP64 = 0, 1
+VL, CTU = 0, 1
+PLM, PPM = 0, 1
+HLLE, HLLD, ROE = 0, 1, 2
+LIM_PRIM, LIM_CHAR = 0, 1
+OK, EINVAL, ECUDA, ENOMEM = 0, -1, -2, -3
+
+EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance_host", "mhd_dt_reduce",
+           "mhd_get_stats", "mhd_launch_count", "mhd_measure_fma_peak", "mhd_strerror"]
+
+
+class Config(C.Structure):
+    _fields_ = [("ps2", C.c_int), ("nghost", C.c_int), ("gamma", C.c_double), ("scheme", C.c_int),
+                ("recon", C.c_int), ("riemann", C.c_int), ("limvar", C.c_int), ("prec", C.c_int),
+                ("min_dens", C.c_double), ("min_pres", C.c_double), ("emf_tie", C.c_double), ("max_groups", C.c_int), ("device", C.c_int)]
+
+
+class MHDError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libmhd error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libmhd.so (built by paper_1804_03479_b200.build); fail loudly if it is not there."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIBPATH):
+            raise ImportError(f"{_LIBPATH} not found: run `python -m paper_1804_03479_b200.build` (needs nvcc); "
+                              "there is no CPU fallback")
+        L = C.CDLL(_LIBPATH)
+        vp, sp = C.c_void_p, C.POINTER(C.c_size_t)
+        L.mhd_create.argtypes = [C.POINTER(Config), C.POINTER(vp)]
+        L.mhd_destroy.argtypes = [vp]
+        L.mhd_sizes.argtypes = [vp, sp, sp, sp, sp, sp, sp]
+        L.mhd_advance.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, vp]
+        L.mhd_advance_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int]
+        L.mhd_dt_reduce.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_double),
+                                    C.POINTER(C.c_double), vp]
+        ull = C.POINTER(C.c_ulonglong)
+        L.mhd_get_stats.argtypes = [vp, ull, ull, ull]
+        L.mhd_launch_count.argtypes = [vp]
+        L.mhd_launch_count.restype = C.c_ulonglong
+        L.mhd_measure_fma_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
+        L.mhd_strerror.argtypes = [C.c_int]
+        L.mhd_strerror.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return lib().mhd_strerror(code).decode()
+
+
+def _check(rc):
+    if rc != OK:
+        raise MHDError(rc, strerror(rc))
+
+
+def _ptr(t):
+    """Raw address of a torch tensor (device or pinned host) or numpy array; None -> NULL."""
+    if t is None:
+        return None
+    if hasattr(t, "data_ptr"):
+        assert t.is_contiguous()
+        return C.c_void_p(t.data_ptr())
+    assert t.flags["C_CONTIGUOUS"]
+    return C.c_void_p(t.ctypes.data)
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def make_config(N=16, g=3, gamma=5.0 / 3.0, scheme=VL, recon=PLM, riemann=HLLD, limvar=None, prec=FP64,
+                min_dens=1e-10, min_pres=1e-10, emf_tie=0.0, max_groups=512, device=0) -> Config:
+    if limvar is None:
+        limvar = LIM_PRIM if scheme == VL else LIM_CHAR
+    return Config(N, g, gamma, scheme, recon, riemann, limvar, prec, min_dens, min_pres, emf_tie, max_groups, device)
+
+
+class Solver:
+    """mhd_create / mhd_destroy wrapped as an object; methods carry the C-ABI names without the prefix."""
+
+    def __init__(self, cfg: Config):
+        self.cfg = cfg
+        self._h = C.c_void_p()
+        _check(lib().mhd_create(C.byref(cfg), C.byref(self._h)))
+        n = [C.c_size_t() for _ in range(6)]
+        _check(lib().mhd_sizes(self._h, *[C.byref(x) for x in n]))
+        self.n_U_in, self.n_B_in, self.n_U_out, self.n_B_out, self.n_flux, self.n_emf = [int(x.value) for x in n]
+
+    def destroy(self):
+        if self._h:
+            lib().mhd_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    @property
+    def torch_dtype(self):
+        import torch
+        return torch.float32 if self.cfg.prec == FP32 else torch.float64
+
+    def sizes(self):
+        return dict(n_U_in=self.n_U_in, n_B_in=self.n_B_in, n_U_out=self.n_U_out, n_B_out=self.n_B_out,
+                    n_flux=self.n_flux, n_emf=self.n_emf)
+
+    def alloc_outputs(self, G, planes=True, device=None):
+        import torch
+        dev = device if device is not None else f"cuda:{self.cfg.device}"
+        dt = self.torch_dtype
+        out = dict(U=torch.empty((G, self.n_U_out), dtype=dt, device=dev),
+                   B=torch.empty((G, self.n_B_out), dtype=dt, device=dev))
+        out["flux"] = torch.empty((G, self.n_flux), dtype=dt, device=dev) if planes else None
+        out["emf"] = torch.empty((G, self.n_emf), dtype=dt, device=dev) if planes else None
+        return out
+
+    def advance(self, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, stream=None):
+        """mhd_advance: DEVICE tensors, asynchronous on `stream` (default: torch's current stream)."""
+        _check(lib().mhd_advance(self._h, _ptr(U_in), _ptr(B_in), _ptr(U_out), _ptr(B_out), _ptr(flux_out),
+                                 _ptr(emf_out), int(ngroups), float(dt), float(dh), _stream_ptr(stream)))
+
+    def advance_host(self, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, chunk_groups, nstreams=3):
+        """mhd_advance_host: HOST arrays (pinned torch tensors or numpy); blocking."""
+        _check(lib().mhd_advance_host(self._h, _ptr(U_in), _ptr(B_in), _ptr(U_out), _ptr(B_out), _ptr(flux_out),
+                                      _ptr(emf_out), int(ngroups), float(dt), float(dh), int(chunk_groups),
+                                      int(nstreams)))
+
+    def dt_reduce(self, U, B, ngroups, nghost_of_arrays, dh, cfl, stream=None):
+        dt, sm = C.c_double(), C.c_double()
+        _check(lib().mhd_dt_reduce(self._h, _ptr(U), _ptr(B), int(ngroups), int(nghost_of_arrays), float(dh),
+                                   float(cfl), C.byref(dt), C.byref(sm), _stream_ptr(stream)))
+        return dt.value, sm.value
+
+    def get_stats(self):
+        a, b, c = C.c_ulonglong(), C.c_ulonglong(), C.c_ulonglong()
+        _check(lib().mhd_get_stats(self._h, C.byref(a), C.byref(b), C.byref(c)))
+        return int(a.value), int(b.value), int(c.value)
+
+    def launch_count(self) -> int:
+        return int(lib().mhd_launch_count(self._h))
+
+
+def measure_fma_peak(device=0, prec=FP64) -> float:
+    v = C.c_double()
+    _check(lib().mhd_measure_fma_peak(int(device), int(prec), C.byref(v)))
+    return v.value

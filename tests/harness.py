@@ -35,3 +35,26 @@ def field_err(a, b):
     den = float(np.max(np.abs(b)))
     num = float(np.max(np.abs(a - b)))
     return num / den if den > 0 else num
+
+
+def pack_boxes(boxes, N, g, dtype=np.float64):
+    """Batch of INDEPENDENT periodic N^3 boxes (config 2) -> one ghost-zoned group each (periodic wrap of itself)."""
+    sz = inputs.sizes(N, g)
+    G = len(boxes)
+    U_in = np.empty((G, sz["n_U_in"]), dtype=dtype)
+    B_in = np.empty((G, sz["n_B_in"]), dtype=dtype)
+    for q, (U, bx, by, bz) in enumerate(boxes):
+        u, b = inputs.pack_groups(U, bx, by, bz, N, g, dtype)
+        U_in[q], B_in[q] = u[0], b[0]
+    return U_in, B_in
+
+
+def step_boxes(advance_fn, boxes, dt, dh, N, g, dtype=np.float64):
+    """One step of a batch of independent periodic boxes through ONE advance call.  boxes: list of (U, bx, by, bz)."""
+    U_in, B_in = pack_boxes(boxes, N, g, dtype)
+    out = advance_fn(U_in, B_in, dt, dh)
+    new = []
+    for q in range(len(boxes)):
+        Un, bxn, byn, bzn, _ = inputs.unpack_groups(np.asarray(out["U"])[q:q + 1], np.asarray(out["B"])[q:q + 1], N, N)
+        new.append((Un, bxn, byn, bzn))
+    return new, out

@@ -1,0 +1,155 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances (BASELINE.json north_star; R14): per field max|gpu-oracle|/max|oracle|
+<= 1e-11 in FP64 and <= 1e-4 in FP32 after 10 steps; the FP32 path is compared with the FP64 oracle started from
+the FP32-rounded inputs and fed the oracle's dt sequence."""
+import numpy as np
+import pytest
+
+from paper_1804_03479_b200 import inputs
+import harness as H
+import gpu_util as GU
+
+pytestmark = pytest.mark.gpu
+
+TOL = {1: 1e-11, 0: 1e-4}
+TOL_ONE_STEP = {1: 2e-13, 0: 1e-4}
+SCHEMES = [("vl_plm", 0, 0, 3), ("ctu_plm", 1, 0, 3), ("ctu_ppm", 1, 1, 4)]
+
+
+EMF_TIE = {1: 1e-12, 0: 1e-5}   # DESIGN.md R7a: the tie width is part of the method and follows the working precision
+
+
+def oracle_fn(oracle, N, g, scheme, recon, riemann, limvar, prec=1):
+    cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon, riemann=riemann, limvar=limvar, emf_tie=EMF_TIE[prec])
+    return cfg, (lambda Ui, Bi, dt, dh: oracle.advance(cfg, Ui, Bi, dt, dh))
+
+
+def assert_fields(errs, tol, what):
+    bad = {k: v for k, v in errs.items() if not (v <= tol)}
+    assert not bad, f"{what}: fields over tolerance {tol:g}: {bad}; all: {errs}"
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# one step, every scheme x Riemann solver x limiter variable x precision, config-2 type groups, planes included
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,scheme,recon,g", SCHEMES)
+@pytest.mark.parametrize("riemann", [0, 1, 2])
+@pytest.mark.parametrize("limvar", [0, 1])
+@pytest.mark.parametrize("prec", [1, 0])
+def test_one_step_every_variant(oracle, name, scheme, recon, g, riemann, limvar, prec):
+    N, G = 16, 5
+    dtp = GU.np_dtype(prec)
+    U_in, B_in, dh = inputs.config2_batch(G, N=N, g=g, dtype=dtp)
+    U64, B64 = U_in.astype(np.float64), B_in.astype(np.float64)
+    cfg, adv = oracle_fn(oracle, N, g, scheme, recon, riemann, limvar, prec)
+    dt, _ = oracle.dt_reduce(cfg, U64, B64, g, dh, 0.3)
+    ref = adv(U64, B64, dt, dh)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=scheme, recon=recon, riemann=riemann, limvar=limvar, prec=prec, max_groups=G)
+    out = gpu(U_in, B_in, dt, dh)
+    assert_fields(GU.field_errors(out, ref, N), TOL_ONE_STEP[prec], f"{name} riemann={riemann} limvar={limvar}")
+    if prec == 1:
+        # same floors / fallbacks fire (same index ranges on both sides)
+        assert gpu.stats() == ref["stats"]
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# config 1: 32^3 periodic ABC grid, VL+PLM+CT, FP64, 10 steps at CFL 0.3 (8 groups of 16^3, g = 3)
+# ---------------------------------------------------------------------------------------------------------------
+def run_grid(adv, U, bx, by, bz, dts, dh, N, g, dtype=np.float64):
+    out = None
+    for dt in dts:
+        U, bx, by, bz, out, mism = H.step_grid(adv, U, bx, by, bz, dt, dh, N, g, dtype)
+        assert mism == 0.0, "faces shared by two groups must be bitwise equal"
+    return U, bx, by, bz, out
+
+
+def oracle_dt_sequence(oracle, adv, U, bx, by, bz, dh, N, g, nsteps, cfl=0.3):
+    """advance the oracle nsteps with its own CFL dt; returns (dts, final state, last output)."""
+    n = U.shape[-1]
+    c0 = oracle.make_config(N=n, g=3)
+    dts, out = [], None
+    for _ in range(nsteps):
+        Ui, Bi = inputs.pack_groups(U, bx, by, bz, n, 0)
+        dt, _ = oracle.dt_reduce(c0, Ui, Bi, 0, dh, cfl)
+        dts.append(dt)
+        U, bx, by, bz, out, _ = H.step_grid(adv, U, bx, by, bz, dt, dh, N, g)
+    return dts, (U, bx, by, bz), out
+
+
+def grid_errors(a, b):
+    names = ["rho", "Mx", "My", "Mz", "e"]
+    errs = {nm: H.field_err(a[0][v], b[0][v]) for v, nm in enumerate(names)}
+    errs.update(Bx=H.field_err(a[1], b[1]), By=H.field_err(a[2], b[2]), Bz=H.field_err(a[3], b[3]))
+    return errs
+
+
+def test_config1_abc32_vl_plm_fp64_10_steps(oracle):
+    n, N, g = 32, 16, 3
+    U, bx, by, bz, dh = inputs.abc_grid(n, seed=1804, p0=1.0, vamp=1e-3)
+    cfg, adv = oracle_fn(oracle, N, g, 0, 0, 1, 0)
+    dts, ref, ref_out = oracle_dt_sequence(oracle, adv, U, bx, by, bz, dh, N, g, 10)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=0, recon=0, riemann=1, prec=1, max_groups=8)
+    res = run_grid(gpu, U, bx, by, bz, dts, dh, N, g)
+    assert_fields(grid_errors(res, ref), TOL[1], "config 1 state")
+    assert_fields(GU.field_errors(res[4], ref_out, N), TOL[1], "config 1 planes of step 10")
+    assert H.rel_divb(res[1], res[2], res[3], dh) < 1e-13
+    t0, t1 = H.totals(U), H.totals(res[0])
+    assert abs(t1[0] - t0[0]) / t0[0] < 1e-13 and abs(t1[4] - t0[4]) / t0[4] < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# config 2: batch of independent 16^3 boxes (each its own periodic domain), VL+PLM+CT, FP64 and FP32, 10 steps
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [1, 0])
+def test_config2_batch_vl_plm_10_steps(oracle, prec):
+    N, g, G = 16, 3, 24
+    dtp = GU.np_dtype(prec)
+    boxes0 = []
+    for q in range(G):
+        U, bx, by, bz, dh = inputs.random_group_grid(N, 3479 + q)
+        # FP32 runs start from the FP32-rounded state on both sides (R14)
+        boxes0.append(tuple(a.astype(dtp).astype(np.float64) for a in (U, bx, by, bz)))
+    cfg, adv = oracle_fn(oracle, N, g, 0, 0, 1, 0, prec)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=0, recon=0, riemann=1, prec=prec, max_groups=G)
+    ref_boxes, gpu_boxes = boxes0, [tuple(a.astype(dtp) for a in b) for b in boxes0]
+    ref_out = gpu_out = None
+    for step in range(10):
+        Ui, Bi = H.pack_boxes(ref_boxes, N, g)
+        dt, _ = oracle.dt_reduce(cfg, Ui, Bi, g, dh, 0.3)
+        ref_boxes, ref_out = H.step_boxes(adv, ref_boxes, dt, dh, N, g)
+        gpu_boxes, gpu_out = H.step_boxes(gpu, gpu_boxes, dt, dh, N, g, dtype=dtp)
+    assert_fields(GU.field_errors(gpu_out, ref_out, N), TOL[prec], f"config 2 prec={prec} outputs of step 10")
+    for q in range(G):
+        bx, by, bz = (np.asarray(a, dtype=np.float64) for a in gpu_boxes[q][1:])
+        assert H.rel_divb(bx, by, bz, dh) < (1e-13 if prec == 1 else 2e-5)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# configs 3 and 4 at oracle-sized grids (64^3 -> 64 groups, g = 4): CTU+PPM+CT, 10 steps
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [1, 0])
+def test_config3_abc_ctu_ppm_10_steps(oracle, prec):
+    n, N, g = 64, 16, 4
+    dtp = GU.np_dtype(prec)
+    U, bx, by, bz, dh = inputs.abc_grid(n, seed=1805, p0=0.15, vamp=1e-2)
+    U, bx, by, bz = (a.astype(dtp).astype(np.float64) for a in (U, bx, by, bz))
+    cfg, adv = oracle_fn(oracle, N, g, 1, 1, 1, 1, prec)
+    dts, ref, ref_out = oracle_dt_sequence(oracle, adv, U, bx, by, bz, dh, N, g, 10)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=1, recon=1, riemann=1, limvar=1, prec=prec, max_groups=64)
+    res = run_grid(gpu, U.astype(dtp), bx.astype(dtp), by.astype(dtp), bz.astype(dtp), dts, dh, N, g, dtype=dtp)
+    assert_fields(grid_errors(res, ref), TOL[prec], f"config 3 prec={prec}")
+    assert H.rel_divb(*(np.asarray(a, dtype=np.float64) for a in res[1:4]), dh) < (1e-13 if prec == 1 else 2e-5)
+    assert gpu.stats() == (0, 0, 0)
+
+
+def test_config4_blast_ctu_ppm_fp64_10_steps(oracle):
+    n, N, g = 64, 16, 4
+    U, bx, by, bz, dh = inputs.blast_grid(n)
+    cfg, adv = oracle_fn(oracle, N, g, 1, 1, 1, 1)
+    dts, ref, ref_out = oracle_dt_sequence(oracle, adv, U, bx, by, bz, dh, N, g, 10)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=1, recon=1, riemann=1, limvar=1, prec=1, max_groups=64)
+    res = run_grid(gpu, U, bx, by, bz, dts, dh, N, g)
+    assert_fields(grid_errors(res, ref), TOL[1], "config 4")
+    assert H.rel_divb(res[1], res[2], res[3], dh) < 1e-13
+    t0, t1 = H.totals(U), H.totals(res[0])
+    assert abs(t1[4] - t0[4]) / t0[4] < 1e-13
