@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py -- cell-updates/sec of the patch-group MHD update on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--scheme vl|ctu] [--prec f32|f64]
+
+Workload (config.workload): BASELINE.json configs[1] -- a batch of 512 patch groups of 16^3 cells (+3 ghost cells,
+VL+PLM+HLLD+CT; flux_out and emf_out requested), seeded synthetic state of paper_1804_03479_b200.inputs.config2_batch
+(DESIGN.md "Input recipe").  One "step" = one pass of the whole hot path over the batch: mhd_advance (S0-S8) followed by
+mhd_dt_reduce (S9) on its output.  The headline line is FP32 (the paper's headline precision); the same run measures
+FP64 and reports it under "fp64".  The batch (177 MB FP32 / 355 MB FP64 of input) is larger than the 126 MB L2, so
+no explicit L2 flush is needed between iterations (config.l2: "inputs larger than L2").
+
+N > 1 (torchrun): every rank advances its own 512-group batch (weak scaling, no data-path collective; the only
+communication is the barrier around the timed region and the max-over-ranks of the device time).
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores, on the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+N_PS2, NGROUPS = 16, 512
+PAPER_P100 = {"f32": 1.2e8, "f64": 5.5e7}       # PAPER.md:12, :465-467 (Tesla P100, VL+PLM+Roe) -- context only
+# algorithmic work per Riemann solve and per group, DESIGN.md "Roofline arithmetic"
+FLOP_PER_SOLVE = {"hlld": 371, "roe": 915, "hlle": 297}   # add/mul/div/sqrt = 1 each, as the oracle states the solver
+FLOP_PLM_PER_FACE = 140     # two MC-limited primitive slopes + the two face states (VL pass 2)
+NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scheme", default="vl", choices=["vl", "ctu"])
+    ap.add_argument("--riemann", default="hlld", choices=["hlle", "hlld", "roe"])
+    ap.add_argument("--prec", default="f32", choices=["f32", "f64"], help="precision of the headline value")
+    ap.add_argument("--groups", type=int, default=NGROUPS)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def scheme_params(args):
+    from paper_1804_03479_b200 import mhd
+    if args.scheme == "vl":
+        return dict(scheme=mhd.VL, recon=mhd.PLM, g=3, name="VL+PLM")
+    return dict(scheme=mhd.CTU, recon=mhd.PPM, g=4, name="CTU+PPM")
+
+
+def faces_per_group(g, scheme):
+    """Riemann solves per group in pass 1 and pass 2 (index ranges of DESIGN.md 'Index ranges')."""
+    N, T = N_PS2, N_PS2 + 2 * g
+    if scheme == "vl":
+        return 3 * (T - 1) * T * T, 3 * (T - 5) * (T - 2) ** 2
+    r = 2
+    return 3 * (T - 2 * r - 1) * T * T, 3 * (T - 2 * r - 1) * (T - 2 * r - 2) ** 2
+
+
+class ClockSampler(threading.Thread):
+    """SM clock + throttle reasons sampled through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.05):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.stop_flag, self.max_mhz = [], set(), False, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def result(self):
+        self.stop_flag = True
+        if self.is_alive():
+            self.join(timeout=2)
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def make_batch(G, g, npdt):
+    """config-2 batch: a pool of 16 distinct seeded groups tiled to G (the kernels' work does not depend on values)."""
+    import numpy as np
+    from paper_1804_03479_b200 import inputs
+    pool = min(G, 16)
+    U, B, dh = inputs.config2_batch(pool, N=N_PS2, g=g, dtype=npdt)
+    reps = (G + pool - 1) // pool
+    return np.tile(U, (reps, 1))[:G].copy(), np.tile(B, (reps, 1))[:G].copy(), dh
+
+
+def measure(args, prec_name, rank, world, dist):
+    """Time K steps of (mhd_advance + mhd_dt_reduce) on device-resident data, then the per-stage profile, then e2e."""
+    import numpy as np
+    import torch
+    from paper_1804_03479_b200 import mhd
+    sp = scheme_params(args)
+    g, G = sp["g"], args.groups
+    prec = mhd.FP32 if prec_name == "f32" else mhd.FP64
+    npdt = np.float32 if prec_name == "f32" else np.float64
+    esz = 4 if prec_name == "f32" else 8
+    riem = {"hlle": mhd.HLLE, "hlld": mhd.HLLD, "roe": mhd.ROE}[args.riemann]
+    dev = torch.device("cuda", torch.cuda.current_device())
+    solver = mhd.Solver(mhd.make_config(N=N_PS2, g=g, scheme=sp["scheme"], recon=sp["recon"], riemann=riem, prec=prec,
+                                        max_groups=G, device=dev.index))
+    hU, hB, dh = make_batch(G, g, npdt)
+    dU, dB = torch.from_numpy(hU).to(dev), torch.from_numpy(hB).to(dev)
+    out = solver.alloc_outputs(G, planes=True, device=dev)
+    stream = torch.cuda.current_stream()
+    dt0, _ = solver.dt_reduce(dU, dB, G, g, dh, 0.3)
+
+    def step():
+        solver.advance(dU, dB, out["U"], out["B"], out["flux"], out["emf"], G, dt0, dh, stream)
+        return solver.dt_reduce(out["U"], out["B"], G, 0, dh, 0.3, stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(dev.index)
+    l0 = solver.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    clocks = sampler.result()
+    ms = e0.elapsed_time(e1)
+    launches = solver.launch_count() - l0
+    if dist is not None:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    cells = G * N_PS2 ** 3 * args.steps * world
+    res = dict(value=cells / (ms * 1e-3), ms_per_step=ms / args.steps, launches=launches, clocks=clocks)
+
+    # per-stage device time over K more steps (events around every stage launch on the launching stream)
+    solver.set_profiling(True)
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    p0.record(stream)
+    for _ in range(args.steps):
+        step()
+    p1.record(stream)
+    torch.cuda.synchronize()
+    prof = solver.get_profile()
+    solver.set_profiling(False)
+    prof_ms = p0.elapsed_time(p1)
+    stages = {k: {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps} for k, v in prof.items() if v[1]}
+    f1, f2 = faces_per_group(g, args.scheme)
+    fl = FLOP_PER_SOLVE[args.riemann]
+    top = max(stages, key=lambda k: stages[k]["ms_per_step"])
+    flops_stage = {"flux_pass1": fl * f1 * G, "flux_pass2": (fl + (FLOP_PLM_PER_FACE if args.scheme == "vl" else 0)) * f2 * G}
+    roof = None
+    if top in flops_stage:
+        n_launch = stages[top]["launches_per_step"]
+        dur = stages[top]["ms_per_step"] / n_launch * 1e-3            # average launch duration
+        ach = flops_stage[top] / n_launch / dur / 1e12
+        peak = NOMINAL_TFLOPS[prec_name]
+        roof = {"bound": "alu", "kernel": top, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                "peak_source": "nominal: 148 SMs x %d FMA lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if prec_name == "f32" else 64),
+                "peak_fma_measured": mhd.measure_fma_peak(dev.index, prec), "traffic": None,
+                "avg_launch_ms": dur * 1e3, "launches_per_step": n_launch,
+                "share_of_step": stages[top]["ms_per_step"] / (prof_ms / args.steps)}
+    # HBM view of the whole step: algorithmic bytes = read the ghost-zoned tile once, write the results once (+ dt read)
+    sz = solver.sizes()
+    bytes_step = (sz["n_U_in"] + sz["n_B_in"] + sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]
+                  + sz["n_U_out"] + sz["n_B_out"]) * esz * G
+    res.update(stages=stages, roofline=roof, profiled_ms_per_step=prof_ms / args.steps,
+               hbm={"algorithmic_GB_per_step": bytes_step / 1e9, "achieved_GBs": bytes_step / 1e9 / (res["ms_per_step"] * 1e-3)})
+
+    # end to end through mhd_advance_host: pinned host buffers, H2D + kernels + D2H inside the timed region
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    pU, pB = pin(hU), pin(hB)
+    hout = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
+    chunk = max(1, min(G, 64))
+    for _ in range(2):
+        solver.advance_host(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], G, dt0, dh, chunk, 3)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        solver.advance_host(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], G, dt0, dh, chunk, 3)
+    torch.cuda.synchronize()
+    te = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([te], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        te = float(t.item())
+    h2d = (sz["n_U_in"] + sz["n_B_in"]) * esz * G
+    d2h = (sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]) * esz * G
+    res["e2e"] = {"value": cells / te, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                  "api": "mhd_advance_host(chunk_groups=%d, nstreams=3), pinned host memory" % chunk,
+                  "h2d_plus_d2h_GBs": (h2d + d2h) * world / 1e9 / (te / args.steps)}
+    res["stats"] = solver.get_stats()
+    solver.destroy()
+    return res
+
+
+def cpu_baseline(args, groups, reps=3):
+    """The oracle, as it stands, on the host cores: best of `reps` passes over `groups` groups of the workload."""
+    import numpy as np
+    from oracle import mhdref
+    mhdref.build()
+    sp = scheme_params(args)
+    U, B, dh = make_batch(groups, sp["g"], np.float64)
+    riem = {"hlle": mhdref.HLLE, "hlld": mhdref.HLLD, "roe": mhdref.ROE}[args.riemann]
+    cfg = mhdref.make_config(N=N_PS2, g=sp["g"], scheme=sp["scheme"], recon=sp["recon"], riemann=riem)
+    dt, _ = mhdref.dt_reduce(cfg, U, B, sp["g"], dh, 0.3)
+    best = None
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        o = mhdref.advance(cfg, U, B, dt, dh)
+        mhdref.dt_reduce(cfg, o["U"], o["B"], 0, dh, 0.3)
+        t = time.perf_counter() - t0
+        best = t if best is None else min(best, t)
+    return {"value": groups * N_PS2 ** 3 / best, "unit": "cell-updates/s", "cores": os.cpu_count(), "kind": "oracle",
+            "sample": "%d of the workload's patch groups, one step (advance + dt), best of %d, FP64, OpenMP over groups"
+                      % (groups, reps), "seconds": best}
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    sp_name = "VL+PLM" if args.scheme == "vl" else "CTU+PPM"
+    g = 3 if args.scheme == "vl" else 4
+    config = {"workload": "BASELINE.json configs[1]: batch of %d patch groups of 16^3 cells + %d ghost cells, %s+%s+CT, "
+                          "flux_out and emf_out requested; per rank" % (args.groups, g, sp_name, args.riemann.upper()),
+              "groups_per_rank": args.groups, "ps2": N_PS2, "nghost": g, "scheme": sp_name, "riemann": args.riemann,
+              "step": "mhd_advance (S0-S8) + mhd_dt_reduce (S9)", "l2": "inputs larger than L2 (no flush needed)",
+              "parallelism": "independent batches per GPU (no collective)" if world > 1 else "single GPU"}
+
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        # the oracle on the host cores; each step = one pass over a bounded sample of the workload
+        sample = min(args.groups, 256)
+        for _ in range(args.warmup):
+            cpu_baseline(args, min(sample, 32), reps=1)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            cb = cpu_baseline(args, sample, reps=1)
+        t = time.perf_counter() - t0
+        val = sample * N_PS2 ** 3 * args.steps / t
+        cb.update(value=val, sample="%d of the %d patch groups per step, FP64 oracle, OpenMP over groups" % (sample, args.groups))
+        line = {"impl": "reference", "metric": "cell-updates/sec", "value": val, "unit": "cell-updates/s", "n_gpus": args.gpus,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config,
+                "cpu_baseline": cb,
+                "e2e": {"value": val, "unit": "cell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+        print(json.dumps(line))
+        return 0
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    from paper_1804_03479_b200 import build
+    build.build()
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist = dist_mod
+    main_prec = args.prec
+    other = "f64" if main_prec == "f32" else "f32"
+    r_main = measure(args, main_prec, rank, world, dist)
+    r_other = measure(args, other, rank, world, dist)
+    if rank == 0:
+        cb = None
+        if not args.no_cpu_baseline and world == 1:
+            cb = cpu_baseline(args, args.groups)
+
+        def sub(r, prec):
+            return {"value": r["value"], "unit": "cell-updates/s", "ms_per_step": r["ms_per_step"], "dtype": prec,
+                    "roofline": r["roofline"], "hbm": r["hbm"], "stages_ms_per_step": {k: round(v["ms_per_step"], 4) for k, v in r["stages"].items()},
+                    "profiled_ms_per_step": r["profiled_ms_per_step"], "e2e": r["e2e"], "clocks": r["clocks"],
+                    "stats": r["stats"], "paper_p100_context": PAPER_P100[prec]}
+
+        line = {"metric": "cell-updates/sec", "value": r_main["value"], "unit": "cell-updates/s", "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": r_main["ms_per_step"], "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": main_prec, "data": "synthetic", "config": config,
+                "clocks": r_main["clocks"], "e2e": r_main["e2e"], "gpu_launches": r_main["launches"],
+                "roofline": r_main["roofline"], "cpu_baseline": cb,
+                "hbm": r_main["hbm"], "stages_ms_per_step": {k: round(v["ms_per_step"], 4) for k, v in r_main["stages"].items()},
+                "profiled_ms_per_step": r_main["profiled_ms_per_step"],
+                "paper_p100_context": {"value": PAPER_P100[main_prec], "note": "Tesla P100, VL+PLM+Roe, PAPER.md:12,:465 -- context, not a target"},
+                {"f32": "fp32", "f64": "fp64"}[other]: sub(r_other, other)}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

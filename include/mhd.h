@@ -102,6 +102,14 @@ int mhd_get_stats(mhd_solver* s, unsigned long long* n_floor_dens, unsigned long
 /* Number of kernel launches issued by this solver since creation (bench.py's gpu_launches). */
 unsigned long long mhd_launch_count(const mhd_solver* s);
 
+/* Per-stage device timing for the roofline report: when on, every stage launch is bracketed by CUDA events on its
+ * stream (up to 16384 launches since the last mhd_set_profiling call; later ones are not recorded).
+ * mhd_get_profile synchronises the device, fills the summed milliseconds and launch counts of each stage
+ * (arrays of at least 11 entries) and returns the number of stages; mhd_profile_stage_name names stage i. */
+int mhd_set_profiling(mhd_solver* s, int on);
+int mhd_get_profile(mhd_solver* s, double* ms_per_stage, unsigned long long* launches_per_stage, int nstages);
+const char* mhd_profile_stage_name(int stage);
+
 /* Register-only FMA-chain micro-kernel: measured FP32 (prec=0) or FP64 (prec=1) FMA peak of this device in
  * TFLOP/s (2 flop per FMA), used as the ALU roofline denominator beside the nominal figure. */
 int mhd_measure_fma_peak(int device, int prec, double* tflops_out);

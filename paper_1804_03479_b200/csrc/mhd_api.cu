@@ -6,6 +6,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "../../include/mhd.h"
 #include "mhd_kernels3.cuh"
@@ -48,6 +49,11 @@ struct mhd_solver {
   unsigned long long launches = 0;
   HostLane lanes[kMaxStreams];
   int lane_groups = 0, lane_count = 0;
+  // optional per-stage timing (mhd_set_profiling): pairs of events around every stage launch
+  bool prof_on = false;
+  std::vector<cudaEvent_t> prof_ev;         // 2 per recorded launch
+  std::vector<int> prof_stage;              // stage id per recorded launch
+  size_t prof_used = 0;
 };
 
 namespace {
@@ -80,6 +86,34 @@ KParams<R> make_params(const mhd_solver* s, const void* Ui, const void* Bi, void
     default:       { constexpr int SOLVER = kROE;  CALL; } break; \
   }
 
+enum Stage : int { ST_LOAD = 0, ST_RECON, ST_FLUX1, ST_EMF1, ST_HALF, ST_CORR, ST_FLUX2, ST_EMF2, ST_FINAL, ST_PLANES, ST_DT, ST_COUNT };
+const char* const kStageNames[ST_COUNT] = { "load_prim", "recon_ctu", "flux_pass1", "emf_pass1", "half_step", "ctu_corr",
+                                            "flux_pass2", "emf_pass2", "final_update", "planes", "dt_reduce" };
+constexpr size_t kProfMaxLaunches = 16384;
+
+inline void prof_begin(mhd_solver* s, int stage, cudaStream_t st) {
+  if (!s->prof_on || s->prof_used >= kProfMaxLaunches) return;
+  if (s->prof_ev.size() < 2 * (s->prof_used + 1)) {
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    s->prof_ev.push_back(a); s->prof_ev.push_back(b); s->prof_stage.push_back(stage);
+  }
+  s->prof_stage[s->prof_used] = stage;
+  cudaEventRecord(s->prof_ev[2 * s->prof_used], st);
+}
+inline void prof_end(mhd_solver* s, cudaStream_t st) {
+  if (!s->prof_on || s->prof_used >= kProfMaxLaunches) return;
+  cudaEventRecord(s->prof_ev[2 * s->prof_used + 1], st);
+  s->prof_used++;
+}
+#define LAUNCH(stage, ...)        \
+  do {                            \
+    prof_begin(s, stage, st);     \
+    __VA_ARGS__;                  \
+    prof_end(s, st);              \
+    s->launches++;                \
+  } while (0)
+
 // all stages of one slice of groups, in the paper's step order
 template <class R>
 int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
@@ -88,36 +122,34 @@ int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
   const unsigned nb = (unsigned)((s->S3 + TPB - 1) / TPB);
   const dim3 g1(nb, 1, ng), g3(nb, 3, ng);
   const int T = s->T, sol = s->cfg.riemann, lim = s->cfg.limvar;
-  k_load_prim<R><<<g1, blk, 0, st>>>(p); s->launches++;
+  LAUNCH(ST_LOAD, (k_load_prim<R><<<g1, blk, 0, st>>>(p)));
   if (s->cfg.scheme == MHD_VL) {
-    SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER><<<g3, blk, 0, st>>>(p))); s->launches++;      // step 1
-    k_emf<R><<<g1, blk, 0, st>>>(p, A_W, 1, T - 1, 0, T); s->launches++;                      // step 2
-    k_half<R><<<g1, blk, 0, st>>>(p, 1, T - 1); s->launches++;                                // step 3
-    if (lim == MHD_LIM_PRIM) { SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, kLimPrim><<<g3, blk, 0, st>>>(p))); }
-    else { SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, kLimChar><<<g3, blk, 0, st>>>(p))); }   // steps 4+5
-    s->launches++;
-    k_emf<R><<<g1, blk, 0, st>>>(p, A_WH, 3, T - 3, 1, T - 1); s->launches++;                 // step 6
+    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER><<<g3, blk, 0, st>>>(p))));          // step 1
+    LAUNCH(ST_EMF1, (k_emf<R><<<g1, blk, 0, st>>>(p, A_W, 1, T - 1, 0, T)));                       // step 2
+    LAUNCH(ST_HALF, (k_half<R><<<g1, blk, 0, st>>>(p, 1, T - 1)));                                 // step 3
+    if (lim == MHD_LIM_PRIM) LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, kLimPrim><<<g3, blk, 0, st>>>(p))));
+    else LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, kLimChar><<<g3, blk, 0, st>>>(p))));   // steps 4+5
+    LAUNCH(ST_EMF2, (k_emf<R><<<g1, blk, 0, st>>>(p, A_WH, 3, T - 3, 1, T - 1)));                  // step 6
   } else {
     const int r = s->cfg.recon == MHD_PLM ? 1 : 2;
     if (s->cfg.recon == MHD_PLM) {
-      if (lim == MHD_LIM_PRIM) k_recon_ctu<R, kPLM, kLimPrim><<<g3, blk, 0, st>>>(p);
-      else k_recon_ctu<R, kPLM, kLimChar><<<g3, blk, 0, st>>>(p);
+      if (lim == MHD_LIM_PRIM) LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimPrim><<<g3, blk, 0, st>>>(p)));
+      else LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimChar><<<g3, blk, 0, st>>>(p)));
     } else {
-      if (lim == MHD_LIM_PRIM) k_recon_ctu<R, kPPM, kLimPrim><<<g3, blk, 0, st>>>(p);
-      else k_recon_ctu<R, kPPM, kLimChar><<<g3, blk, 0, st>>>(p);
-    }
-    s->launches++;                                                                            // step 1
-    SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<g3, blk, 0, st>>>(p, A_B, r + 1, T - r, 0, T))); s->launches++;   // step 2
-    k_emf<R><<<g1, blk, 0, st>>>(p, A_W, r + 1, T - 1 - r, 0, T); s->launches++;              // step 3
-    k_half<R><<<g1, blk, 0, st>>>(p, r + 1, T - 1 - r); s->launches++;                        // step 4
-    k_ctu_corr<R><<<g3, blk, 0, st>>>(p, r); s->launches++;                                   // step 5
-    SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<g3, blk, 0, st>>>(p, A_BH, r + 1, T - r, r + 1, T - 1 - r))); s->launches++;  // step 6
-    k_emf<R><<<g1, blk, 0, st>>>(p, A_WH, r + 2, T - 2 - r, r + 1, T - 1 - r); s->launches++; // step 7
+      if (lim == MHD_LIM_PRIM) LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, kLimPrim><<<g3, blk, 0, st>>>(p)));
+      else LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, kLimChar><<<g3, blk, 0, st>>>(p)));
+    }                                                                                              // step 1
+    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<g3, blk, 0, st>>>(p, A_B, r + 1, T - r, 0, T))));   // step 2
+    LAUNCH(ST_EMF1, (k_emf<R><<<g1, blk, 0, st>>>(p, A_W, r + 1, T - 1 - r, 0, T)));               // step 3
+    LAUNCH(ST_HALF, (k_half<R><<<g1, blk, 0, st>>>(p, r + 1, T - 1 - r)));                         // step 4
+    LAUNCH(ST_CORR, (k_ctu_corr<R><<<g3, blk, 0, st>>>(p, r)));                                    // step 5
+    LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<g3, blk, 0, st>>>(p, A_BH, r + 1, T - r, r + 1, T - 1 - r))));  // step 6
+    LAUNCH(ST_EMF2, (k_emf<R><<<g1, blk, 0, st>>>(p, A_WH, r + 2, T - 2 - r, r + 1, T - 1 - r)));  // step 7
   }
-  k_final<R><<<g1, blk, 0, st>>>(p); s->launches++;                                           // step 7 / 8
+  LAUNCH(ST_FINAL, (k_final<R><<<g1, blk, 0, st>>>(p)));                                           // step 7 / 8
   if (p.fout || p.eout) {
     const int M = s->N + 1;
-    k_planes<R><<<dim3((9 * M * M + TPB - 1) / TPB, 1, ng), blk, 0, st>>>(p); s->launches++;
+    LAUNCH(ST_PLANES, (k_planes<R><<<dim3((9 * M * M + TPB - 1) / TPB, 1, ng), blk, 0, st>>>(p)));
   }
   CU(cudaGetLastError());
   return MHD_OK;
@@ -210,6 +242,7 @@ int mhd_destroy(mhd_solver* s) {
   if (!s) return MHD_EINVAL;
   cudaSetDevice(s->cfg.device);
   free_lanes(s);
+  for (cudaEvent_t e : s->prof_ev) cudaEventDestroy(e);
   cudaFree(s->ws);
   cudaFree(s->d_stats);
   delete s;

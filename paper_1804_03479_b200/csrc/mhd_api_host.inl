@@ -76,12 +76,11 @@ int mhd_dt_reduce(mhd_solver* s, const void* U, const void* B, int ngroups, int 
   CU(cudaMemsetAsync(s->d_red, 0, sizeof(unsigned long long), st));
   const dim3 grid((N * N * N + 255) / 256, 1, ngroups), blk(256);
   if (s->cfg.prec == MHD_FP32)
-    k_dt<float><<<grid, blk, 0, st>>>(static_cast<const float*>(U), static_cast<const float*>(B), N, ng, nU, nB,
-                                       (float)s->cfg.gamma, (float)s->cfg.min_dens, (float)s->cfg.min_pres, s->d_red);
+    LAUNCH(ST_DT, (k_dt<float><<<grid, blk, 0, st>>>(static_cast<const float*>(U), static_cast<const float*>(B), N, ng, nU, nB,
+                                       (float)s->cfg.gamma, (float)s->cfg.min_dens, (float)s->cfg.min_pres, s->d_red)));
   else
-    k_dt<double><<<grid, blk, 0, st>>>(static_cast<const double*>(U), static_cast<const double*>(B), N, ng, nU, nB,
-                                        s->cfg.gamma, s->cfg.min_dens, s->cfg.min_pres, s->d_red);
-  s->launches++;
+    LAUNCH(ST_DT, (k_dt<double><<<grid, blk, 0, st>>>(static_cast<const double*>(U), static_cast<const double*>(B), N, ng, nU, nB,
+                                        s->cfg.gamma, s->cfg.min_dens, s->cfg.min_pres, s->d_red)));
   CU(cudaGetLastError());
   unsigned long long bits = 0;
   CU(cudaMemcpyAsync(&bits, s->d_red, sizeof bits, cudaMemcpyDeviceToHost, st));
@@ -105,6 +104,29 @@ int mhd_get_stats(mhd_solver* s, unsigned long long* fd, unsigned long long* fp,
 }
 
 unsigned long long mhd_launch_count(const mhd_solver* s) { return s ? s->launches : 0ULL; }
+
+int mhd_set_profiling(mhd_solver* s, int on) {
+  if (!s) return MHD_EINVAL;
+  s->prof_on = on != 0;
+  s->prof_used = 0;
+  return MHD_OK;
+}
+
+int mhd_get_profile(mhd_solver* s, double* ms_per_stage, unsigned long long* launches_per_stage, int nstages) {
+  if (!s || !ms_per_stage || !launches_per_stage || nstages < ST_COUNT) return MHD_EINVAL;
+  CU(cudaSetDevice(s->cfg.device));
+  CU(cudaDeviceSynchronize());
+  for (int i = 0; i < nstages; ++i) { ms_per_stage[i] = 0.0; launches_per_stage[i] = 0; }
+  for (size_t l = 0; l < s->prof_used; ++l) {
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, s->prof_ev[2 * l], s->prof_ev[2 * l + 1]));
+    ms_per_stage[s->prof_stage[l]] += ms;
+    launches_per_stage[s->prof_stage[l]]++;
+  }
+  return ST_COUNT;
+}
+
+const char* mhd_profile_stage_name(int stage) { return (stage >= 0 && stage < ST_COUNT) ? kStageNames[stage] : ""; }
 
 int mhd_measure_fma_peak(int device, int prec, double* tflops_out) {
   if (!tflops_out || (prec != MHD_FP32 && prec != MHD_FP64)) return MHD_EINVAL;

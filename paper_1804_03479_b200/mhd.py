@@ -20,7 +20,8 @@ LIM_PRIM, LIM_CHAR = 0, 1
 OK, EINVAL, ECUDA, ENOMEM = 0, -1, -2, -3
 
 EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance_host", "mhd_dt_reduce",
-           "mhd_get_stats", "mhd_launch_count", "mhd_measure_fma_peak", "mhd_strerror"]
+           "mhd_get_stats", "mhd_launch_count", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
+           "mhd_measure_fma_peak", "mhd_strerror"]
 
 
 class Config(C.Structure):
@@ -58,6 +59,10 @@ def lib():
         L.mhd_get_stats.argtypes = [vp, ull, ull, ull]
         L.mhd_launch_count.argtypes = [vp]
         L.mhd_launch_count.restype = C.c_ulonglong
+        L.mhd_set_profiling.argtypes = [vp, C.c_int]
+        L.mhd_get_profile.argtypes = [vp, C.POINTER(C.c_double), ull, C.c_int]
+        L.mhd_profile_stage_name.argtypes = [C.c_int]
+        L.mhd_profile_stage_name.restype = C.c_char_p
         L.mhd_measure_fma_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.mhd_strerror.argtypes = [C.c_int]
         L.mhd_strerror.restype = C.c_char_p
@@ -164,6 +169,18 @@ class Solver:
 
     def launch_count(self) -> int:
         return int(lib().mhd_launch_count(self._h))
+
+    def set_profiling(self, on: bool):
+        _check(lib().mhd_set_profiling(self._h, int(bool(on))))
+
+    def get_profile(self) -> dict:
+        """{stage name: (milliseconds summed over launches, launches)} since set_profiling(True)."""
+        n = 16
+        ms, cnt = (C.c_double * n)(), (C.c_ulonglong * n)()
+        k = lib().mhd_get_profile(self._h, ms, cnt, n)
+        if k < 0:
+            _check(k)
+        return {lib().mhd_profile_stage_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(k)}
 
 
 def measure_fma_peak(device=0, prec=FP64) -> float:
