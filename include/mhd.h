@@ -53,7 +53,7 @@ typedef struct {
   int prec;         /* mhd_precision: element type of every array argument */
   double min_dens;  /* floors applied to DERIVED primitive states only (R9); conserved output is never floored */
   double min_pres;
-  double emf_tie;   /* CT upwinding tie (R7a): a face mass flux m with |m| dt/dh <= emf_tie * (mean density of the
+  double emf_tie;   /* CT upwinding tie (R10a): a face mass flux m with |m| dt/dh <= emf_tie * (mean density of the
                        two cells) counts as zero and takes the centred average; <= 0 selects 1e-12 (FP64) / 1e-5 (FP32) */
   int max_groups;   /* largest ngroups of one mhd_advance call (bounds nothing but argument checking) */
   int device;       /* CUDA device ordinal */

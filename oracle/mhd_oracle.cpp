@@ -39,7 +39,7 @@ typedef struct {
   int riemann;  // 0 HLLE, 1 HLLD, 2 ROE
   int limvar;   // 0 primitive, 1 characteristic
   double min_dens, min_pres;
-  double emf_tie;  // reading R7a: width of the linear blend of the CT upwind switch, in units of (mean cell density) * dh/dt
+  double emf_tie;  // reading R10a: width of the linear blend of the CT upwind switch, in units of (mean cell density) * dh/dt
 } mhdref_config;
 }
 
@@ -408,7 +408,7 @@ struct Group {
     if (w[4] < c.min_pres) { w[4] = c.min_pres; if (st) st->fp++; }
   }
 
-  // C6: edge EMFs from the face fluxes F, cell-centred reference field from Wc (v, Bc).
+  // reading R10: edge EMFs from the face fluxes F, cell-centred reference field from Wc (v, Bc).
   // Edge along c=(d) at (a-1/2, b-1/2), (a,b,c) cyclic.  Range: a,b in [alo,ahi], c in [clo,chi).
   void edge_emf(const Arr Wc[8], int alo, int ahi, int clo, int chi) {
     for (int cdir = 0; cdir < 3; ++cdir) {
@@ -418,8 +418,8 @@ struct Group {
       auto Ea = [&](size_t q) { return -F[a][5][q]; };
       auto Eb = [&](size_t q) { return F[bdir][6][q]; };
       auto ec = [&](size_t q) { return Wc[1 + bdir][q] * Wc[5 + a][q] - Wc[1 + a][q] * Wc[5 + bdir][q]; };  // -(v x B)_c
-      // upwinding by the sign of the face mass flux m (reading R7): q- if m > 0, q+ if m < 0, the mean if m = 0.
-      // Reading R7a: "m = 0" means |m| <= m0 = emf_tie * (mean density of the two cells) * dh/dt, i.e. less than emf_tie
+      // upwinding by the sign of the face mass flux m (reading R10): q- if m > 0, q+ if m < 0, the mean if m = 0.
+      // Reading R10a: "m = 0" means |m| <= m0 = emf_tie * (mean density of the two cells) * dh/dt, i.e. less than emf_tie
       // of the cell mass crosses the face in dt (zero at working precision); between m0 and 2 m0 the switch ramps
       // linearly from the mean to the upwind value, so that the EMF is a continuous function of m.
       const double tie = c.emf_tie * dh / dt;

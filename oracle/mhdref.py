@@ -69,7 +69,7 @@ def _c(a):
 
 def make_config(N=16, g=3, gamma=5.0 / 3.0, scheme=VL, recon=PLM, riemann=HLLD, limvar=None,
                 min_dens=1e-10, min_pres=1e-10, emf_tie=1e-12) -> Config:
-    """emf_tie: reading R7a; 1e-12 is the FP64 value, the FP32 path is checked against the oracle run with 1e-5."""
+    """emf_tie: reading R10a; 1e-12 is the FP64 value, the FP32 path is checked against the oracle run with 1e-5."""
     if limvar is None:
         limvar = LIM_PRIM if scheme == VL else LIM_CHAR
     return Config(N, g, gamma, scheme, recon, riemann, limvar, min_dens, min_pres, emf_tie)

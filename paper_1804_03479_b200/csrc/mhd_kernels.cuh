@@ -37,7 +37,7 @@ template <class R> struct KParams {
   int N, g, T, S, S2, S3, narr;
   long long nUi, nBi, nUo, nBo, nF, nE;
   R gam, gm1, gm1inv, dt, dh, min_dens, min_pres;
-  R tie;   // emf_tie * dh / dt (R7a)
+  R tie;   // emf_tie * dh / dt (R10a)
 };
 
 struct Box { int lo[3], hi[3]; };   // half-open index box
@@ -139,9 +139,9 @@ __global__ void __launch_bounds__(256) k_flux1_vl(const KParams<R> p) {
   }
 }
 
-// ---- S3 / S7: upwinded edge EMFs (formula DESIGN.md R6) --------------------------------------
+// ---- S3 / S7: upwinded edge EMFs (formula DESIGN.md R10) -------------------------------------
 // edge along C at (a-1/2, b-1/2), (a,b,c) cyclic; face EMFs: from an a-face E_c = -F_a[B_t1], from a b-face E_c = +F_b[B_t2]
-// upwind switch on the face mass flux m (R7).  R7a: |m| <= m0 (less than emf_tie of the cell mass crosses the face
+// upwind switch on the face mass flux m (R10).  R10a: |m| <= m0 (less than emf_tie of the cell mass crosses the face
 // in dt) counts as zero -> centred mean; between m0 and 2 m0 a linear ramp to the upwind value keeps the EMF continuous
 template <class R> __device__ __forceinline__ R upwind(R m, R m0, R qm, R qp) {
   const R am = Num<R>::abs(m), mean = R(0.5) * (qm + qp), qu = m > R(0) ? qm : qp;

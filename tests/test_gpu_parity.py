@@ -16,7 +16,7 @@ TOL_ONE_STEP = {1: 2e-13, 0: 1e-4}
 SCHEMES = [("vl_plm", 0, 0, 3), ("ctu_plm", 1, 0, 3), ("ctu_ppm", 1, 1, 4)]
 
 
-EMF_TIE = {1: 1e-12, 0: 1e-5}   # DESIGN.md R7a: the tie width is part of the method and follows the working precision
+EMF_TIE = {1: 1e-12, 0: 1e-5}   # DESIGN.md R10a: the tie width is part of the method and follows the working precision
 
 
 def oracle_fn(oracle, N, g, scheme, recon, riemann, limvar, prec=1):
