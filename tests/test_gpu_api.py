@@ -1,0 +1,179 @@
+"""-m gpu tests of the boundary itself: edge cases, slicing, shapes other than 16^3, the host (stream-overlapped) path,
+the dt reduction, counters, and the full-size batch of bench.py checked on sampled groups."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1804_03479_b200 import inputs
+import harness as H
+import gpu_util as GU
+
+pytestmark = pytest.mark.gpu
+
+
+def small_batch(G, N=16, g=3, dtype=np.float64, first=0):
+    return inputs.config2_batch(G, N=N, g=g, dtype=dtype, first=first)
+
+
+def test_empty_batch_and_argument_errors():
+    import torch
+    from paper_1804_03479_b200 import mhd
+    s = mhd.Solver(mhd.make_config(max_groups=4))
+    U, B, dh = small_batch(1)
+    dU, dB = torch.from_numpy(U).cuda(), torch.from_numpy(B).cuda()
+    out = s.alloc_outputs(1)
+    out["U"].fill_(7.0)
+    s.advance(dU, dB, out["U"], out["B"], None, None, 0, 1e-3, dh)          # ngroups = 0: no-op
+    torch.cuda.synchronize()
+    assert float(out["U"].min()) == 7.0
+    for bad in (dict(ngroups=5), dict(dt=0.0), dict(dt=float("nan")), dict(dh=-1.0)):
+        kw = dict(ngroups=1, dt=1e-3, dh=dh); kw.update(bad)
+        with pytest.raises(mhd.MHDError) as ei:
+            s.advance(dU, dB, out["U"], out["B"], None, None, kw["ngroups"], kw["dt"], kw["dh"])
+        assert ei.value.code == mhd.EINVAL
+    with pytest.raises(mhd.MHDError):
+        s.advance(None, dB, out["U"], out["B"], None, None, 1, 1e-3, dh)
+    with pytest.raises(mhd.MHDError):
+        s.dt_reduce(dU, dB, 1, 2, dh, 0.3)                                   # ghost width neither 0 nor cfg.nghost
+    with pytest.raises(mhd.MHDError):
+        mhd.Solver(mhd.make_config(g=2))
+    assert s.sizes() == {k: v for k, v in inputs.sizes(16, 3).items() if k != "T"}
+
+
+@pytest.mark.parametrize("prec", [1, 0])
+def test_planes_optional_and_identical_results(oracle, prec):
+    """flux_out / emf_out NULL must not change U_out, B_out (bitwise)."""
+    dtp = GU.np_dtype(prec)
+    U, B, dh = small_batch(3, dtype=dtp)
+    a = GU.GpuRunner(prec=prec, planes=True, max_groups=3)(U, B, 2e-3, dh)
+    b = GU.GpuRunner(prec=prec, planes=False, max_groups=3)(U, B, 2e-3, dh)
+    assert b["flux"] is None and b["emf"] is None
+    assert np.array_equal(a["U"], b["U"]) and np.array_equal(a["B"], b["B"])
+
+
+@pytest.mark.parametrize("slice_groups", ["1", "3", "64"])
+def test_ragged_slices_are_bitwise_identical(slice_groups, monkeypatch):
+    """7 groups processed in slices of 1, 3 (ragged tail) and all at once give the same bits; groups are independent."""
+    U, B, dh = small_batch(7)
+    monkeypatch.setenv("MHD_SLICE_GROUPS", slice_groups)
+    a = GU.GpuRunner(max_groups=7)(U, B, 2e-3, dh)
+    monkeypatch.delenv("MHD_SLICE_GROUPS")
+    b = GU.GpuRunner(max_groups=7)(U, B, 2e-3, dh)
+    for k in ("U", "B", "flux", "emf"):
+        assert np.array_equal(a[k], b[k]), k
+    # and a group's result does not depend on its position in the batch
+    c = GU.GpuRunner(max_groups=7)(U[::-1].copy(), B[::-1].copy(), 2e-3, dh)
+    assert np.array_equal(c["U"][::-1], b["U"]) and np.array_equal(c["emf"][::-1], b["emf"])
+
+
+@pytest.mark.parametrize("N,g,scheme,recon", [(8, 3, 0, 0), (32, 3, 0, 0), (16, 4, 0, 0), (8, 4, 1, 1), (24, 5, 1, 1), (32, 3, 1, 0)])
+def test_other_group_sizes_and_wider_ghosts(oracle, N, g, scheme, recon):
+    """ps2 != 16 and ghost widths above the minimum (extra layers must not matter)."""
+    n = 2 * N if N <= 16 else N
+    U, bx, by, bz, dh = inputs.random_group_grid(n, 11)
+    cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon)
+    Ui, Bi = inputs.pack_groups(U, bx, by, bz, N, g)
+    dt = 0.2 * dh
+    ref = oracle.advance(cfg, Ui, Bi, dt, dh)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=scheme, recon=recon, max_groups=Ui.shape[0])
+    out = gpu(Ui, Bi, dt, dh)
+    errs = GU.field_errors(out, ref, N)
+    assert max(errs.values()) <= 2e-13, errs
+    assert gpu.stats() == ref["stats"]
+
+
+@pytest.mark.parametrize("prec", [1, 0])
+def test_uniform_state_is_a_fixed_point_on_the_gpu(prec):
+    N, g = 16, 3
+    dtp = GU.np_dtype(prec)
+    rho, v, p, Bv = 1.3, (0.4, -0.7, 0.2), 0.8, (0.5, -0.3, 0.9)
+    bx = np.full((N, N, N + 1), Bv[0]); by = np.full((N, N + 1, N), Bv[1]); bz = np.full((N + 1, N, N), Bv[2])
+    o = np.ones((N, N, N))
+    U = inputs.conserved(rho * o, v[0] * o, v[1] * o, v[2] * o, p * o, bx, by, bz)
+    for scheme, recon, gg in ((0, 0, 3), (1, 1, 4)):
+        gpu = GU.GpuRunner(N=N, g=gg, scheme=scheme, recon=recon, prec=prec, max_groups=1)
+        Un, bxn, byn, bzn, out, _ = H.step_grid(gpu, U.astype(dtp), bx.astype(dtp), by.astype(dtp), bz.astype(dtp), 0.01, 1.0 / N, N, gg, dtp)
+        assert np.array_equal(bxn, bx.astype(dtp)) and np.array_equal(byn, by.astype(dtp)) and np.array_equal(bzn, bz.astype(dtp))
+        assert np.abs(Un - U.astype(dtp)).max() < (1e-14 if prec == 1 else 1e-6)
+        assert gpu.stats() == (0, 0, 0)
+
+
+def test_decomposition_is_bitwise_on_the_gpu():
+    """P9 on the device: 32^3 advanced as one group of 32^3 and as 8 groups of 16^3 gives the same bits."""
+    n = 32
+    U, bx, by, bz, dh = inputs.random_group_grid(n, 5)
+    dt = 0.2 * dh
+    for scheme, recon, g in ((0, 0, 3), (1, 1, 4)):
+        a = H.step_grid(GU.GpuRunner(N=32, g=g, scheme=scheme, recon=recon, max_groups=1), U, bx, by, bz, dt, dh, 32, g)
+        b = H.step_grid(GU.GpuRunner(N=16, g=g, scheme=scheme, recon=recon, max_groups=8), U, bx, by, bz, dt, dh, 16, g)
+        for x, y in zip(a[:4], b[:4]):
+            assert np.array_equal(x, y)
+        assert b[5] == 0.0
+
+
+@pytest.mark.parametrize("prec", [1, 0])
+def test_dt_reduce_matches_the_oracle(oracle, prec):
+    dtp = GU.np_dtype(prec)
+    tol = 1e-14 if prec == 1 else 1e-6
+    U, B, dh = small_batch(9, dtype=dtp)
+    cfg = oracle.make_config()
+    gpu = GU.GpuRunner(prec=prec, max_groups=9)
+    ref_dt, ref_s = oracle.dt_reduce(cfg, U.astype(np.float64), B.astype(np.float64), 3, dh, 0.3)
+    dt, s = gpu.dt(U, B, 3, dh, 0.3)
+    assert abs(dt - ref_dt) <= tol * ref_dt and abs(s - ref_s) <= tol * ref_s
+    out = gpu(U, B, ref_dt, dh)                                   # ghost-free layout of the outputs
+    ref_dt2, _ = oracle.dt_reduce(cfg, out["U"].astype(np.float64), out["B"].astype(np.float64), 0, dh, 0.3)
+    dt2, _ = gpu.dt(out["U"], out["B"], 0, dh, 0.3)
+    assert abs(dt2 - ref_dt2) <= tol * ref_dt2
+    # the max is exact: a single group holding the fastest cell gives the same answer as the whole batch
+    per_group = [gpu.dt(U[q:q + 1], B[q:q + 1], 3, dh, 0.3)[1] for q in range(9)]
+    assert max(per_group) == s
+
+
+@pytest.mark.parametrize("prec", [1, 0])
+@pytest.mark.parametrize("chunk,nstreams", [(4, 3), (16, 1), (5, 2)])
+def test_advance_host_equals_advance_bitwise(prec, chunk, nstreams):
+    """the stream-overlapped host path (pinned or pageable host memory, ragged last chunk) returns the same bits"""
+    import torch
+    dtp = GU.np_dtype(prec)
+    G = 13
+    U, B, dh = small_batch(G, dtype=dtp)
+    gpu = GU.GpuRunner(prec=prec, max_groups=16)
+    ref = gpu(U, B, 2e-3, dh)
+    s = gpu.solver
+    tdt = s.torch_dtype
+    hU, hB = torch.from_numpy(U).pin_memory(), torch.from_numpy(B).pin_memory()
+    ho = {k: torch.empty((G, n), dtype=tdt).pin_memory() for k, n in (("U", s.n_U_out), ("B", s.n_B_out), ("flux", s.n_flux), ("emf", s.n_emf))}
+    s.advance_host(hU, hB, ho["U"], ho["B"], ho["flux"], ho["emf"], G, 2e-3, dh, chunk, nstreams)
+    for k in ("U", "B", "flux", "emf"):
+        assert np.array_equal(ho[k].numpy(), ref[k]), k
+    # pageable numpy arrays and no planes
+    oU, oB = np.empty((G, s.n_U_out), dtype=dtp), np.empty((G, s.n_B_out), dtype=dtp)
+    s.advance_host(U, B, oU, oB, None, None, G, 2e-3, dh, chunk, nstreams)
+    assert np.array_equal(oU, ref["U"]) and np.array_equal(oB, ref["B"])
+
+
+@pytest.mark.parametrize("prec,scheme,recon,g", [(0, 0, 0, 3), (1, 0, 0, 3), (0, 1, 1, 4), (1, 1, 1, 4)])
+def test_full_size_batch_on_sampled_groups(oracle, prec, scheme, recon, g):
+    """BASELINE.json configs[1] at full size (512 groups, the launch configuration bench.py times): one step, every
+    32nd group compared with the oracle (groups are independent, so the oracle can compute them one by one)."""
+    dtp = GU.np_dtype(prec)
+    G, N = 512, 16
+    pool_U, pool_B, dh = small_batch(16, g=g, dtype=dtp)
+    U = np.tile(pool_U, (G // 16, 1)); B = np.tile(pool_B, (G // 16, 1))
+    # make the sampled groups distinct from the pool so that position matters
+    sample = list(range(5, G, 32))
+    extra_U, extra_B, _ = small_batch(len(sample), g=g, dtype=dtp, first=100)
+    U[sample] = extra_U; B[sample] = extra_B
+    cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon, emf_tie=(1e-12 if prec == 1 else 1e-5))
+    dt, _ = oracle.dt_reduce(cfg, U[sample].astype(np.float64), B[sample].astype(np.float64), g, dh, 0.3)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=scheme, recon=recon, prec=prec, max_groups=G)
+    out = gpu(U, B, dt, dh)
+    ref = oracle.advance(cfg, U[sample].astype(np.float64), B[sample].astype(np.float64), dt, dh)
+    sub = {k: out[k][sample] for k in out}
+    errs = GU.field_errors(sub, ref, N)
+    assert max(errs.values()) <= (2e-13 if prec == 1 else 1e-4), errs
+    # invariants that hold at any size: div B of every group's output at round-off
+    bx, by, bz = inputs.split_B(out["B"].astype(np.float64), N)
+    assert H.rel_divb(bx, by, bz, dh) < (1e-13 if prec == 1 else 2e-5)
