@@ -1,5 +1,6 @@
-// mhd_api.cu -- the C ABI of include/mhd.h: solver object, slice scheduling, kernel dispatch, stream-overlapped
-// host path.  No CPU fallback anywhere: every entry point that computes needs a CUDA device.
+// mhd_api.cu -- the C ABI of include/mhd.h: solver object, slice scheduling over concurrent streams, kernel dispatch,
+// stream-overlapped host path.  No CPU fallback anywhere: every entry point that computes needs a CUDA device.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -34,6 +35,12 @@ struct HostLane {            // one stream of mhd_advance_host with its staging 
   void *Ui = nullptr, *Bi = nullptr, *Uo = nullptr, *Bo = nullptr, *fo = nullptr, *eo = nullptr, *ws = nullptr;
 };
 
+struct DevLane {             // one internal stream of mhd_advance with its workspace
+  cudaStream_t stream = nullptr;
+  cudaEvent_t done = nullptr;
+  void* ws = nullptr;
+};
+
 }  // namespace
 
 struct mhd_solver {
@@ -42,14 +49,17 @@ struct mhd_solver {
   size_t esz;                               // bytes per element
   size_t nUi, nBi, nUo, nBo, nF, nE;        // elements per group
   size_t S3;
-  int slice_groups;                         // groups whose working set is kept L2-resident per sweep of the stages
-  void* ws = nullptr;                       // slice_groups * narr * S3 elements
+  int slice_groups;                         // groups per slice (one slice = one pass of all stages on one lane)
+  int nlanes;                               // concurrent slices of mhd_advance
+  DevLane dev[kMaxStreams];
+  cudaEvent_t fork = nullptr;
   unsigned long long* d_stats = nullptr;    // 3 counters
   unsigned long long* d_red = nullptr;      // dt reduction cell
   unsigned long long launches = 0;
   HostLane lanes[kMaxStreams];
   int lane_groups = 0, lane_count = 0;
-  // optional per-stage timing (mhd_set_profiling): pairs of events around every stage launch
+  // optional per-stage timing (mhd_set_profiling): pairs of events around every stage launch; slices then run
+  // one after the other on the caller's stream so that the stage times do not overlap
   bool prof_on = false;
   std::vector<cudaEvent_t> prof_ev;         // 2 per recorded launch
   std::vector<int> prof_stage;              // stage id per recorded launch
@@ -86,9 +96,9 @@ KParams<R> make_params(const mhd_solver* s, const void* Ui, const void* Bi, void
     default:       { constexpr int SOLVER = kROE;  CALL; } break; \
   }
 
-enum Stage : int { ST_LOAD = 0, ST_RECON, ST_FLUX1, ST_EMF1, ST_HALF, ST_CORR, ST_FLUX2, ST_EMF2, ST_FINAL, ST_PLANES, ST_DT, ST_COUNT };
+enum Stage : int { ST_LOAD = 0, ST_RECON, ST_FLUX1, ST_EMF1, ST_HALF, ST_CORR, ST_FLUX2, ST_EMF2, ST_FINAL, ST_DT, ST_COUNT };
 const char* const kStageNames[ST_COUNT] = { "load_prim", "recon_ctu", "flux_pass1", "emf_pass1", "half_step", "ctu_corr",
-                                            "flux_pass2", "emf_pass2", "final_update", "planes", "dt_reduce" };
+                                            "flux_pass2", "emf_pass2", "final_update", "dt_reduce" };
 constexpr size_t kProfMaxLaunches = 16384;
 
 inline void prof_begin(mhd_solver* s, int stage, cudaStream_t st) {
@@ -114,55 +124,123 @@ inline void prof_end(mhd_solver* s, cudaStream_t st) {
     s->launches++;                \
   } while (0)
 
+// ---- index boxes: [lo, hi) per axis ---------------------------------------------------------
+inline Box3 box(int x0, int x1, int y0, int y1, int z0, int z1) {
+  Box3 b; b.lo[0] = x0; b.lo[1] = y0; b.lo[2] = z0; b.n[0] = x1 - x0; b.n[1] = y1 - y0; b.n[2] = z1 - z0; return b;
+}
+// per sweep direction d: normal index in [n0, n1), both transverse indices in [t0, t1)
+inline Box3x3 dir_boxes(int n0, int n1, int t0, int t1) {
+  Box3x3 bx;
+  for (int d = 0; d < 3; ++d) {
+    int lo[3] = { t0, t0, t0 }, hi[3] = { t1, t1, t1 };
+    lo[d] = n0; hi[d] = n1;
+    bx.b[d] = box(lo[0], hi[0], lo[1], hi[1], lo[2], hi[2]);
+  }
+  return bx;
+}
+// edges along c: the two transverse indices in [a0, a1], the index along the edge in [c0, c1)
+inline Box3x3 edge_boxes(int a0, int a1, int c0, int c1) {
+  Box3x3 bx;
+  for (int c = 0; c < 3; ++c) {
+    int lo[3] = { a0, a0, a0 }, hi[3] = { a1 + 1, a1 + 1, a1 + 1 };
+    lo[c] = c0; hi[c] = c1;
+    bx.b[c] = box(lo[0], hi[0], lo[1], hi[1], lo[2], hi[2]);
+  }
+  return bx;
+}
+inline unsigned blocks_for(const Box3& b, int tpb) { return (unsigned)((b.n[0] * b.n[1] * b.n[2] + tpb - 1) / tpb); }
+inline unsigned blocks_for(const Box3x3& bx, int tpb) {
+  return std::max(blocks_for(bx.b[0], tpb), std::max(blocks_for(bx.b[1], tpb), blocks_for(bx.b[2], tpb)));
+}
+
 // all stages of one slice of groups, in the paper's step order
 template <class R>
 int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
   const int TPB = 256;
   const dim3 blk(TPB);
-  const unsigned nb = (unsigned)((s->S3 + TPB - 1) / TPB);
-  const dim3 g1(nb, 1, ng), g3(nb, 3, ng);
-  const int T = s->T, sol = s->cfg.riemann, lim = s->cfg.limvar;
-  LAUNCH(ST_LOAD, (k_load_prim<R><<<g1, blk, 0, st>>>(p)));
+  const int T = s->T, S = s->S, N = s->N, g = s->g, sol = s->cfg.riemann, lim = s->cfg.limvar;
+#define GRID1(b) dim3(blocks_for(b, TPB), 1, ng)
+#define GRID3(b) dim3(blocks_for(b, TPB), 3, ng)
+  const Box3 ball = box(0, S, 0, S, 0, S);
+  LAUNCH(ST_LOAD, (k_load_prim<R><<<GRID1(ball), blk, 0, st>>>(p, ball)));
   if (s->cfg.scheme == MHD_VL) {
-    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER><<<g3, blk, 0, st>>>(p))));          // step 1
-    LAUNCH(ST_EMF1, (k_emf<R><<<g1, blk, 0, st>>>(p, A_W, 1, T - 1, 0, T)));                       // step 2
-    LAUNCH(ST_HALF, (k_half<R><<<g1, blk, 0, st>>>(p, 1, T - 1)));                                 // step 3
-    if (lim == MHD_LIM_PRIM) LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, kLimPrim><<<g3, blk, 0, st>>>(p))));
-    else LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, kLimChar><<<g3, blk, 0, st>>>(p))));   // steps 4+5
-    LAUNCH(ST_EMF2, (k_emf<R><<<g1, blk, 0, st>>>(p, A_WH, 3, T - 3, 1, T - 1)));                  // step 6
+    const Box3x3 bf1 = dir_boxes(1, T, 0, T), be1 = edge_boxes(1, T - 1, 0, T);
+    const Box3 bh = box(1, T - 1, 1, T - 1, 1, T - 1);
+    const Box3x3 bf2 = dir_boxes(3, T - 2, 1, T - 1), be2 = edge_boxes(3, T - 3, 1, T - 1);
+    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER><<<GRID3(bf1), blk, 0, st>>>(p, bf1))));          // step 1
+    LAUNCH(ST_EMF1, (k_emf<R><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 2
+    LAUNCH(ST_HALF, (k_half<R><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 3
+    if (lim == MHD_LIM_PRIM) LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, kLimPrim><<<GRID3(bf2), blk, 0, st>>>(p, bf2))));
+    else LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, kLimChar><<<GRID3(bf2), blk, 0, st>>>(p, bf2))));   // steps 4+5
+    LAUNCH(ST_EMF2, (k_emf<R><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 6
   } else {
     const int r = s->cfg.recon == MHD_PLM ? 1 : 2;
+    const Box3x3 brc = dir_boxes(r, T - r, 0, T), bf1 = dir_boxes(r + 1, T - r, 0, T), be1 = edge_boxes(r + 1, T - 1 - r, 0, T);
+    const Box3 bh = box(r + 1, T - 1 - r, r + 1, T - 1 - r, r + 1, T - 1 - r);
+    const Box3x3 bco = dir_boxes(r, T - r, r + 1, T - 1 - r), bf2 = dir_boxes(r + 1, T - r, r + 1, T - 1 - r);
+    const Box3x3 be2 = edge_boxes(r + 2, T - 2 - r, r + 1, T - 1 - r);
     if (s->cfg.recon == MHD_PLM) {
-      if (lim == MHD_LIM_PRIM) LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimPrim><<<g3, blk, 0, st>>>(p)));
-      else LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimChar><<<g3, blk, 0, st>>>(p)));
+      if (lim == MHD_LIM_PRIM) LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimPrim><<<GRID3(brc), blk, 0, st>>>(p, brc)));
+      else LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimChar><<<GRID3(brc), blk, 0, st>>>(p, brc)));
     } else {
-      if (lim == MHD_LIM_PRIM) LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, kLimPrim><<<g3, blk, 0, st>>>(p)));
-      else LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, kLimChar><<<g3, blk, 0, st>>>(p)));
-    }                                                                                              // step 1
-    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<g3, blk, 0, st>>>(p, A_B, r + 1, T - r, 0, T))));   // step 2
-    LAUNCH(ST_EMF1, (k_emf<R><<<g1, blk, 0, st>>>(p, A_W, r + 1, T - 1 - r, 0, T)));               // step 3
-    LAUNCH(ST_HALF, (k_half<R><<<g1, blk, 0, st>>>(p, r + 1, T - 1 - r)));                         // step 4
-    LAUNCH(ST_CORR, (k_ctu_corr<R><<<g3, blk, 0, st>>>(p, r)));                                    // step 5
-    LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<g3, blk, 0, st>>>(p, A_BH, r + 1, T - r, r + 1, T - 1 - r))));  // step 6
-    LAUNCH(ST_EMF2, (k_emf<R><<<g1, blk, 0, st>>>(p, A_WH, r + 2, T - 2 - r, r + 1, T - 1 - r)));  // step 7
+      const Box3x3 bsl = dir_boxes(1, T - 1, 0, T);
+      if (lim == MHD_LIM_PRIM) {
+        LAUNCH(ST_RECON, (k_slope_ctu<R, kLimPrim><<<GRID3(bsl), blk, 0, st>>>(p, bsl)));
+        LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, kLimPrim><<<GRID3(brc), blk, 0, st>>>(p, brc)));
+      } else {
+        LAUNCH(ST_RECON, (k_slope_ctu<R, kLimChar><<<GRID3(bsl), blk, 0, st>>>(p, bsl)));
+        LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, kLimChar><<<GRID3(brc), blk, 0, st>>>(p, brc)));
+      }
+    }                                                                                                          // step 1
+    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<GRID3(bf1), blk, 0, st>>>(p, bf1, A_B))));      // step 2
+    LAUNCH(ST_EMF1, (k_emf<R><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 3
+    LAUNCH(ST_HALF, (k_half<R><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 4
+    LAUNCH(ST_CORR, (k_ctu_corr<R><<<GRID3(bco), blk, 0, st>>>(p, bco, r + 1, T - 1 - r)));                    // step 5
+    LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<GRID3(bf2), blk, 0, st>>>(p, bf2, A_BH))));     // step 6
+    LAUNCH(ST_EMF2, (k_emf<R><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 7
   }
-  LAUNCH(ST_FINAL, (k_final<R><<<g1, blk, 0, st>>>(p)));                                           // step 7 / 8
-  if (p.fout || p.eout) {
-    const int M = s->N + 1;
-    LAUNCH(ST_PLANES, (k_planes<R><<<dim3((9 * M * M + TPB - 1) / TPB, 1, ng), blk, 0, st>>>(p)));
-  }
+  const Box3 bin = box(g, g + N, g, g + N, g, g + N);
+  const unsigned nbf = std::max(blocks_for(bin, TPB), (unsigned)((9 * (N + 1) * (N + 1) + TPB - 1) / TPB));
+  LAUNCH(ST_FINAL, (k_final<R><<<dim3(nbf, 1, ng), blk, 0, st>>>(p, bin)));                                    // step 7 / 8
+#undef GRID1
+#undef GRID3
   CU(cudaGetLastError());
   return MHD_OK;
 }
 
+// slices of one batch on ONE stream with ONE workspace (host path, profiling)
 template <class R>
-int advance_dev(mhd_solver* s, const void* Ui, const void* Bi, void* Uo, void* Bo, void* fo, void* eo, void* ws,
-                int ngroups, double dt, double dh, cudaStream_t st) {
+int advance_serial(mhd_solver* s, const void* Ui, const void* Bi, void* Uo, void* Bo, void* fo, void* eo, void* ws,
+                   int ngroups, double dt, double dh, cudaStream_t st) {
   for (int first = 0; first < ngroups; first += s->slice_groups) {
     const int ng = std::min(s->slice_groups, ngroups - first);
     KParams<R> p = make_params<R>(s, Ui, Bi, Uo, Bo, fo, eo, ws, first, dt, dh);
     int rc = run_slice<R>(s, p, ng, st);
     if (rc != MHD_OK) return rc;
+  }
+  return MHD_OK;
+}
+
+// slices round-robin over the internal lanes, forked from and joined back into the caller's stream
+template <class R>
+int advance_lanes(mhd_solver* s, const void* Ui, const void* Bi, void* Uo, void* Bo, void* fo, void* eo,
+                  int ngroups, double dt, double dh, cudaStream_t user) {
+  const int nslices = (ngroups + s->slice_groups - 1) / s->slice_groups;
+  const int nl = std::min(s->nlanes, nslices);
+  if (s->prof_on || nl <= 1) return advance_serial<R>(s, Ui, Bi, Uo, Bo, fo, eo, s->dev[0].ws, ngroups, dt, dh, user);
+  CU(cudaEventRecord(s->fork, user));
+  for (int l = 0; l < nl; ++l) CU(cudaStreamWaitEvent(s->dev[l].stream, s->fork, 0));
+  int i = 0;
+  for (int first = 0; first < ngroups; first += s->slice_groups, ++i) {
+    const int ng = std::min(s->slice_groups, ngroups - first);
+    DevLane& L = s->dev[i % nl];
+    KParams<R> p = make_params<R>(s, Ui, Bi, Uo, Bo, fo, eo, L.ws, first, dt, dh);
+    int rc = run_slice<R>(s, p, ng, L.stream);
+    if (rc != MHD_OK) return rc;
+  }
+  for (int l = 0; l < nl; ++l) {
+    CU(cudaEventRecord(s->dev[l].done, s->dev[l].stream));
+    CU(cudaStreamWaitEvent(user, s->dev[l].done, 0));
   }
   return MHD_OK;
 }
@@ -185,6 +263,16 @@ int check_config(const mhd_config* c) {
 }
 
 }  // namespace
+
+static void free_lanes(mhd_solver* s) {
+  for (int l = 0; l < kMaxStreams; ++l) {
+    HostLane& L = s->lanes[l];
+    if (L.stream) cudaStreamDestroy(L.stream);
+    cudaFree(L.Ui); cudaFree(L.Bi); cudaFree(L.Uo); cudaFree(L.Bo); cudaFree(L.fo); cudaFree(L.eo); cudaFree(L.ws);
+    L = HostLane();
+  }
+  s->lane_groups = 0; s->lane_count = 0;
+}
 
 extern "C" {
 
@@ -209,41 +297,47 @@ int mhd_create(const mhd_config* cfg, mhd_solver** out) {
   s->nUi = 5 * T * T * T; s->nBi = 3 * T * T * (T + 1);
   s->nUo = 5 * N * N * N; s->nBo = 3 * N * N * (N + 1);
   s->nF = 9 * 5 * N * N; s->nE = 9 * 2 * (N + 1) * N;
-  // slice = as many groups as keep workspace + their input and output inside a budget well below the 126 MB L2
-  double budget_mb = 72.0;
+  // Lanes x slice: nlanes slices are in flight at once; a slice holds as many groups as fit the per-lane share of
+  // the workspace budget (MHD_LANES / MHD_SLICE_MB / MHD_SLICE_GROUPS override for experiments)
+  int nl = 3;
+  if (const char* e = getenv("MHD_LANES")) { int v = atoi(e); if (v >= 1) nl = v; }
+  s->nlanes = std::min(nl, kMaxStreams);
+  double budget_mb = 288.0;
   if (const char* e = getenv("MHD_SLICE_MB")) { double v = atof(e); if (v > 0) budget_mb = v; }
   const size_t per_group = ((size_t)s->narr * s->S3 + s->nUi + s->nBi + s->nUo + s->nBo + s->nF + s->nE) * s->esz;
-  long sg = (long)(budget_mb * 1048576.0 / (double)per_group);
+  long sg = (long)(budget_mb * 1048576.0 / s->nlanes / (double)per_group);
   if (const char* e = getenv("MHD_SLICE_GROUPS")) { long v = atol(e); if (v > 0) sg = v; }
   if (sg < 1) sg = 1;
   if (sg > cfg->max_groups) sg = cfg->max_groups;
   s->slice_groups = (int)sg;
-  cudaError_t e = cudaMalloc(&s->ws, (size_t)s->slice_groups * s->narr * s->S3 * s->esz);
-  if (e == cudaSuccess) e = cudaMalloc((void**)&s->d_stats, 4 * sizeof(unsigned long long));
+  const size_t ws_bytes = (size_t)s->slice_groups * s->narr * s->S3 * s->esz;
+  cudaError_t e = cudaMalloc((void**)&s->d_stats, 4 * sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMemset(s->d_stats, 0, 4 * sizeof(unsigned long long));
-  if (e == cudaSuccess) e = cudaMemset(s->ws, 0, (size_t)s->slice_groups * s->narr * s->S3 * s->esz);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->fork, cudaEventDisableTiming);
+  for (int l = 0; l < s->nlanes && e == cudaSuccess; ++l) {
+    e = cudaStreamCreateWithFlags(&s->dev[l].stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->dev[l].done, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaMalloc(&s->dev[l].ws, ws_bytes);
+    if (e == cudaSuccess) e = cudaMemset(s->dev[l].ws, 0, ws_bytes);
+  }
   if (e != cudaSuccess) { int r = cuda_fail(e, "mhd_create allocation"); mhd_destroy(s); return r; }
   s->d_red = s->d_stats + 3;
   *out = s;
   return MHD_OK;
 }
 
-static void free_lanes(mhd_solver* s) {
-  for (int l = 0; l < kMaxStreams; ++l) {
-    HostLane& L = s->lanes[l];
-    if (L.stream) cudaStreamDestroy(L.stream);
-    cudaFree(L.Ui); cudaFree(L.Bi); cudaFree(L.Uo); cudaFree(L.Bo); cudaFree(L.fo); cudaFree(L.eo); cudaFree(L.ws);
-    L = HostLane();
-  }
-  s->lane_groups = 0; s->lane_count = 0;
-}
-
 int mhd_destroy(mhd_solver* s) {
   if (!s) return MHD_EINVAL;
   cudaSetDevice(s->cfg.device);
+  cudaDeviceSynchronize();
   free_lanes(s);
   for (cudaEvent_t e : s->prof_ev) cudaEventDestroy(e);
-  cudaFree(s->ws);
+  for (int l = 0; l < kMaxStreams; ++l) {
+    if (s->dev[l].stream) cudaStreamDestroy(s->dev[l].stream);
+    if (s->dev[l].done) cudaEventDestroy(s->dev[l].done);
+    cudaFree(s->dev[l].ws);
+  }
+  if (s->fork) cudaEventDestroy(s->fork);
   cudaFree(s->d_stats);
   delete s;
   return MHD_OK;
@@ -264,8 +358,8 @@ int mhd_advance(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, 
   CU(cudaSetDevice(s->cfg.device));
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   return s->cfg.prec == MHD_FP32
-             ? advance_dev<float>(s, U_in, B_in, U_out, B_out, flux_out, emf_out, s->ws, ngroups, dt, dh, st)
-             : advance_dev<double>(s, U_in, B_in, U_out, B_out, flux_out, emf_out, s->ws, ngroups, dt, dh, st);
+             ? advance_lanes<float>(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, st)
+             : advance_lanes<double>(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, st);
 }
 
 }  // extern "C"

@@ -50,8 +50,8 @@ int mhd_advance_host(mhd_solver* s, const void* U_in, const void* B_in, void* U_
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(L.Bi, hBi + f * s->nBi * e, ng * s->nBi * e, cudaMemcpyHostToDevice, L.stream);
     if (ce != cudaSuccess) { s->slice_groups = saved_slice; return cuda_fail(ce, "mhd_advance_host H2D"); }
     rc = s->cfg.prec == MHD_FP32
-             ? advance_dev<float>(s, L.Ui, L.Bi, L.Uo, L.Bo, hf ? L.fo : nullptr, he ? L.eo : nullptr, L.ws, (int)ng, dt, dh, L.stream)
-             : advance_dev<double>(s, L.Ui, L.Bi, L.Uo, L.Bo, hf ? L.fo : nullptr, he ? L.eo : nullptr, L.ws, (int)ng, dt, dh, L.stream);
+             ? advance_serial<float>(s, L.Ui, L.Bi, L.Uo, L.Bo, hf ? L.fo : nullptr, he ? L.eo : nullptr, L.ws, (int)ng, dt, dh, L.stream)
+             : advance_serial<double>(s, L.Ui, L.Bi, L.Uo, L.Bo, hf ? L.fo : nullptr, he ? L.eo : nullptr, L.ws, (int)ng, dt, dh, L.stream);
     if (rc != MHD_OK) { s->slice_groups = saved_slice; return rc; }
     ce = cudaMemcpyAsync(hUo + f * s->nUo * e, L.Uo, ng * s->nUo * e, cudaMemcpyDeviceToHost, L.stream);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(hBo + f * s->nBo * e, L.Bo, ng * s->nBo * e, cudaMemcpyDeviceToHost, L.stream);

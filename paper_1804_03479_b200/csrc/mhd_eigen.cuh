@@ -13,18 +13,18 @@ template <class R> struct WaveSet { R cf, cs, ca, af, as, b1, b2, S; };
 template <class R>
 __device__ __forceinline__ WaveSet<R> wave_set(R a2, R rho, R bn, R B1, R B2) {
   WaveSet<R> w;
-  const R ir = R(1) / rho;
+  const R ir = frcp(rho);
   const R bt2 = B1 * B1 + B2 * B2;
   const R ca2 = bn * bn * ir, ct2 = bt2 * ir;
   const R sum = a2 + ca2 + ct2, dif = ca2 + ct2 - a2;
   const R cf2 = R(0.5) * (sum + Num<R>::sqrt(dif * dif + R(4) * a2 * ct2));
-  R cs2 = (cf2 > R(0)) ? a2 * ca2 / cf2 : R(0);
+  R cs2 = (cf2 > R(0)) ? fdiv(a2 * ca2, cf2) : R(0);
   cs2 = (cs2 < R(0)) ? R(0) : cs2;
   w.cf = Num<R>::sqrt(cf2); w.cs = Num<R>::sqrt(cs2); w.ca = Num<R>::sqrt(ca2);
   const R den = cf2 - cs2;
   if (den <= R(0)) { w.af = R(1); w.as = R(0); }
   else {
-    const R iden = R(1) / den;
+    const R iden = frcp(den);
     R af2 = (a2 - cs2) * iden, as2 = (cf2 - a2) * iden;
     af2 = Num<R>::min(R(1), Num<R>::max(R(0), af2));
     as2 = Num<R>::min(R(1), Num<R>::max(R(0), as2));
@@ -32,7 +32,7 @@ __device__ __forceinline__ WaveSet<R> wave_set(R a2, R rho, R bn, R B1, R B2) {
   }
   const R bt = Num<R>::sqrt(bt2);
   if (bt == R(0)) { w.b1 = R(1); w.b2 = R(0); }
-  else { const R ibt = R(1) / bt; w.b1 = B1 * ibt; w.b2 = B2 * ibt; }
+  else { const R ibt = frcp(bt); w.b1 = B1 * ibt; w.b2 = B2 * ibt; }
   w.S = (bn >= R(0)) ? R(1) : R(-1);
   return w;
 }
@@ -45,8 +45,8 @@ __device__ __forceinline__ RoeAvg<R> roe_average(const R (&wl)[7], const R (&wr)
                                                  const Side<R>& Rr, R bn2, R gam) {
   RoeAvg<R> r;
   const R sl = Num<R>::sqrt(wl[0]), sr = Num<R>::sqrt(wr[0]);
-  const R iw = R(1) / (sl + sr);
-  const R HL = (L.U[4] + L.pT) / wl[0], HR = (Rr.U[4] + Rr.pT) / wr[0];
+  const R iw = frcp(sl + sr);
+  const R HL = fdiv(L.U[4] + L.pT, wl[0]), HR = fdiv(Rr.U[4] + Rr.pT, wr[0]);
   r.rho = sl * sr;
   r.vn = (sl * wl[1] + sr * wr[1]) * iw;
   r.v1 = (sl * wl[2] + sr * wr[2]) * iw;
@@ -55,7 +55,8 @@ __device__ __forceinline__ RoeAvg<R> roe_average(const R (&wl)[7], const R (&wr)
   r.B1 = (sr * wl[5] + sl * wr[5]) * iw;   // density weights swapped for the transverse field
   r.B2 = (sr * wl[6] + sl * wr[6]) * iw;
   r.X = (sqr(wl[5] - wr[5]) + sqr(wl[6] - wr[6])) * R(0.5) * iw * iw;
-  const R ca2 = bn2 / r.rho, ct2 = (sqr(r.B1) + sqr(r.B2)) / r.rho;
+  const R irr = frcp(r.rho);
+  const R ca2 = bn2 * irr, ct2 = (sqr(r.B1) + sqr(r.B2)) * irr;
   const R Hp = r.H - ca2 - ct2;
   const R v2 = sqr(r.vn) + sqr(r.v1) + sqr(r.v2);
   r.a2 = (gam - R(1)) * (Hp - R(0.5) * v2) - (gam - R(2)) * r.X;
@@ -68,7 +69,7 @@ __device__ __forceinline__ void hlle_flux(const R (&wl)[7], const R (&wr)[7], co
                                           bool roe_ok, R roe_vn, R roe_cf, R (&F)[7]) {
   R bp = Num<R>::max(wr[1] + Rr.cf, R(0)), bm = Num<R>::min(wl[1] - L.cf, R(0));
   if (roe_ok) { bp = Num<R>::max(bp, roe_vn + roe_cf); bm = Num<R>::min(bm, roe_vn - roe_cf); }
-  const R idb = R(1) / (bp - bm), bpm = bp * bm;
+  const R idb = frcp(bp - bm), bpm = bp * bm;
 #pragma unroll
   for (int c = 0; c < 7; ++c) F[c] = (bp * L.F[c] - bm * Rr.F[c] + bpm * (Rr.U[c] - L.U[c])) * idb;
 }
@@ -96,16 +97,17 @@ __device__ __forceinline__ bool riemann_roe(const R (&wl)[7], const R (&wr)[7], 
   side_setup(wr, bn, bn2, gm1inv, gam, Rr);
   const RoeAvg<R> r = roe_average(wl, wr, L, Rr, bn2, gam);
   const bool a2ok = r.a2 > R(0);
-  const R a2 = r.a2, a = Num<R>::sqrt(a2), srho = Num<R>::sqrt(r.rho), isrho = R(1) / srho;
+  const R a2 = r.a2, a = Num<R>::sqrt(a2), srho = Num<R>::sqrt(r.rho), isrho = frcp(srho);
   const WaveSet<R> w = wave_set(a2, r.rho, bn, r.B1, r.B2);
-  const R ca2 = bn2 / r.rho, bt2 = sqr(r.B1) + sqr(r.B2), ct2 = bt2 / r.rho;
+  const R irr = isrho * isrho;
+  const R ca2 = bn2 * irr, bt2 = sqr(r.B1) + sqr(r.B2), ct2 = bt2 * irr;
   const R Hp = r.H - ca2 - ct2;
   const R vsq = sqr(r.vn) + sqr(r.v1) + sqr(r.v2);
   const R Qf = w.cf * w.af * w.S, Qs = w.cs * w.as * w.S;
   const R Afp = a * w.af * isrho, Asp = a * w.as * isrho;
   const R vb = r.v1 * w.b1 + r.v2 * w.b2, bt = Num<R>::sqrt(bt2);
-  const R xt = (gam - R(2)) * r.X / (gam - R(1));
-  const R nn = R(0.5) / a2, g = (gam - R(1)) * nn;
+  const R xt = fdiv((gam - R(2)) * r.X, gam - R(1));
+  const R nn = fdiv(R(0.5), a2), g = (gam - R(1)) * nn;
   const R vxb = r.v1 * w.b2 - r.v2 * w.b1;
   const R lam[7] = { r.vn - w.cf, r.vn - w.ca, r.vn - w.cs, r.vn, r.vn + w.cs, r.vn + w.ca, r.vn + w.cf };
 
@@ -160,7 +162,7 @@ __device__ __forceinline__ bool riemann_roe(const R (&wl)[7], const R (&wr)[7], 
     for (int c = 0; c < 7; ++c) { diss[c] += wk * Rk[c]; Ui[c] += ak * Rk[c]; }
     if (k < 6) {
       if (lam[k + 1] > lam[k]) {
-        const R Pi = (gam - R(1)) * (Ui[4] - R(0.5) * (sqr(Ui[1]) + sqr(Ui[2]) + sqr(Ui[3])) / Ui[0]
+        const R Pi = (gam - R(1)) * (Ui[4] - R(0.5) * fdiv(sqr(Ui[1]) + sqr(Ui[2]) + sqr(Ui[3]), Ui[0])
                                       - R(0.5) * (bn2 + sqr(Ui[5]) + sqr(Ui[6])));
         bad = bad || !(Ui[0] > R(0)) || !(Pi > R(0));
       }

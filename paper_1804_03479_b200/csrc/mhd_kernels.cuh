@@ -1,16 +1,18 @@
-// mhd_kernels.cuh -- the stage kernels of the patch-group update (sm_100a).
+// mhd_kernels.cuh -- the stage kernels of the patch-group update (sm_100a), part 1: layout, staging, pass-1
+// fluxes, edge EMFs, half step.
 //
-// Work decomposition: a batch is processed in SLICES of groups whose whole working set (primitives, face
-// fluxes, edge EMFs, half-step state, CTU face states) stays resident in the B200's 126 MB L2, so that HBM
-// sees each input and output value once.  Inside a slice every stage is one
-// kernel over all cells / faces / edges of all groups of the slice: blockIdx.z = group in slice,
-// blockIdx.y = sweep direction where the stage has one, x-fastest thread order (coalesced).
+// Work decomposition: a batch is processed in SLICES of groups; inside a slice every stage of the scheme is one
+// kernel over exactly the cells / faces / edges that stage needs (a compact index box per sweep direction, no
+// masked-out threads), for all groups of the slice: blockIdx.z = group in slice, blockIdx.y = sweep direction
+// where the stage has one, x-fastest thread order (coalesced rows).  Slices run concurrently on several streams
+// (mhd_api.cu) so that the drain / ramp-up between dependent stages of one slice is filled by another slice.
 //
 // Workspace of one group: NARR arrays of S^3 Reals with the uniform strides (1, S, S^2), S = T+1, so that
 // cell (i,j,k), its lower faces and its lower edges all share the flat index q = (k*S + j)*S + i:
 //   b[d][q]  = field on the lower d-face of cell q            (Fig. 1)
 //   F[d][c][q] = flux through that face, generic component order (rho, Mn, Mt1, Mt2, e, Bt1, Bt2), (n,t1,t2) cyclic
 //   E[c][q]  = EMF on the edge along c through the cell's lowest corner, i.e. at (a-1/2, b-1/2), (a,b,c) cyclic
+//   EC[c][q] = cell-centred reference EMF -(v x Bc)_c of cell q (time n, later overwritten by the half-step one)
 #pragma once
 #include "mhd_recon.cuh"
 
@@ -23,10 +25,11 @@ enum : int {
   A_E = 32,     // 3
   A_BH = 35,    // 3: face field at t^{n+1/2}
   A_WH = 38,    // 8: half-step primitives
-  A_VL_END = 46,
-  A_LO = 46,    // 21: CTU state at the lower d-face of each cell, [d][v]
-  A_UP = 67,    // 21: CTU state at the upper d-face
-  A_CTU_END = 88
+  A_EC = 46,    // 3: cell-centred reference EMF
+  A_VL_END = 49,
+  A_LO = 49,    // 21: CTU state at the lower d-face of each cell, [d][v]
+  A_UP = 70,    // 21: CTU state at the upper d-face
+  A_CTU_END = 91
 };
 
 template <class R> struct KParams {
@@ -40,25 +43,30 @@ template <class R> struct KParams {
   R tie;   // emf_tie * dh / dt (R10a)
 };
 
-struct Box { int lo[3], hi[3]; };   // half-open index box
+// compact index box of one launch: cells lo[d] .. lo[d]+n[d]-1; Box3x3 = one box per sweep direction
+struct Box3 { int lo[3], n[3]; };
+struct Box3x3 { Box3 b[3]; };
 
 template <class R> struct Ctx {
   const KParams<R>& p;
   int q, i, j, k, grp;
+  bool ok;
   R* w;   // this group's workspace
-  __device__ __forceinline__ Ctx(const KParams<R>& p_) : p(p_) {
-    q = blockIdx.x * blockDim.x + threadIdx.x;
+  __device__ __forceinline__ Ctx(const KParams<R>& p_, const Box3& b) : p(p_) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    ok = t < b.n[0] * b.n[1] * b.n[2];
+    const int r = t / b.n[0];
+    i = b.lo[0] + (t - r * b.n[0]);
+    const int kk = r / b.n[1];
+    j = b.lo[1] + (r - kk * b.n[1]);
+    k = b.lo[2] + kk;
+    q = (k * p.S + j) * p.S + i;
     grp = blockIdx.z;
-    i = q % p.S; int t = q / p.S; j = t % p.S; k = t / p.S;
     w = p.ws + (size_t)grp * p.narr * p.S3;
   }
-  __device__ __forceinline__ bool valid() const { return q < p.S3; }
   __device__ __forceinline__ R* arr(int a) const { return w + (size_t)a * p.S3; }
   __device__ __forceinline__ int off(int d) const { return d == 0 ? 1 : (d == 1 ? p.S : p.S2); }
   __device__ __forceinline__ int idx(int d) const { return d == 0 ? i : (d == 1 ? j : k); }
-  __device__ __forceinline__ bool inside(const Box& b) const {
-    return i >= b.lo[0] && i < b.hi[0] && j >= b.lo[1] && j < b.hi[1] && k >= b.lo[2] && k < b.hi[2];
-  }
 };
 
 __device__ __forceinline__ void count_event(unsigned long long* ctr) { atomicAdd(ctr, 1ULL); }
@@ -85,17 +93,28 @@ __device__ __forceinline__ void cons_to_prim(const KParams<R>& p, const R (&u)[5
   const R bcx = R(0.5) * (bl[0] + bu[0]), bcy = R(0.5) * (bl[1] + bu[1]), bcz = R(0.5) * (bl[2] + bu[2]);
   R rho = u[0];
   if (rho < p.min_dens) { rho = p.min_dens; count_event(p.stats + 0); }
-  const R vx = u[1] / rho, vy = u[2] / rho, vz = u[3] / rho;
+  const R ir = frcp(rho);
+  const R vx = u[1] * ir, vy = u[2] * ir, vz = u[3] * ir;
   R P = p.gm1 * (u[4] - R(0.5) * rho * (vx * vx + vy * vy + vz * vz) - R(0.5) * (bcx * bcx + bcy * bcy + bcz * bcz));
   if (P < p.min_pres) { P = p.min_pres; count_event(p.stats + 1); }
   W[0] = rho; W[1] = vx; W[2] = vy; W[3] = vz; W[4] = P; W[5] = bcx; W[6] = bcy; W[7] = bcz;
 }
 
+// primitives and the cell-centred reference EMF -(v x Bc) of a cell into the workspace
+template <class R>
+__device__ __forceinline__ void store_prim(const Ctx<R>& c, int wbase, const R (&W)[8]) {
+#pragma unroll
+  for (int v = 0; v < 8; ++v) c.arr(wbase + v)[c.q] = W[v];
+  c.arr(A_EC + 0)[c.q] = W[3] * W[6] - W[2] * W[7];
+  c.arr(A_EC + 1)[c.q] = W[1] * W[7] - W[3] * W[5];
+  c.arr(A_EC + 2)[c.q] = W[2] * W[5] - W[1] * W[6];
+}
+
 // ---- S0 + S1: stage the input tile: face fields into the workspace, primitives of all T^3 cells -----------------
 template <class R>
-__global__ void __launch_bounds__(256) k_load_prim(const KParams<R> p) {
-  Ctx<R> c(p);
-  if (!c.valid()) return;
+__global__ void __launch_bounds__(256) k_load_prim(const KParams<R> p, const Box3 box) {
+  Ctx<R> c(p, box);
+  if (!c.ok) return;
   const int T = p.T, i = c.i, j = c.j, k = c.k, q = c.q;
   const R* Bx = p.Bin + (size_t)c.grp * p.nBi;
   const R* By = Bx + (size_t)T * T * (T + 1);
@@ -112,14 +131,14 @@ __global__ void __launch_bounds__(256) k_load_prim(const KParams<R> p) {
   const R u[5] = { U[cq], U[T3 + cq], U[2 * T3 + cq], U[3 * T3 + cq], U[4 * T3 + cq] };
   R W[8];
   cons_to_prim(p, u, bl, bu, W);
-#pragma unroll
-  for (int v = 0; v < 8; ++v) c.arr(A_W + v)[q] = W[v];
+  store_prim(c, A_W, W);
 }
 
 // ---- VL step 1: first-order fluxes, normal B = face value ----------------------------------------
 template <class R, int SOLVER, int D>
-__device__ __forceinline__ void flux1_dir(const KParams<R>& p, const Ctx<R>& c) {
-  if (c.idx(D) < 1 || c.i >= p.T || c.j >= p.T || c.k >= p.T) return;
+__device__ __forceinline__ void flux1_dir(const KParams<R>& p, const Box3& box) {
+  Ctx<R> c(p, box);
+  if (!c.ok) return;
   R wl[7], wr[7], F[7];
   load_gen<R, D>(c.arr(A_W), p.S3, c.q - c.off(D), wl);
   load_gen<R, D>(c.arr(A_W), p.S3, c.q, wr);
@@ -129,40 +148,35 @@ __device__ __forceinline__ void flux1_dir(const KParams<R>& p, const Ctx<R>& c) 
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[c.q] = F[v];
 }
 template <class R, int SOLVER>
-__global__ void __launch_bounds__(256) k_flux1_vl(const KParams<R> p) {
-  Ctx<R> c(p);
-  if (!c.valid()) return;
+__global__ void __launch_bounds__(256) k_flux1_vl(const KParams<R> p, const Box3x3 bx) {
   switch (blockIdx.y) {
-    case 0: flux1_dir<R, SOLVER, 0>(p, c); break;
-    case 1: flux1_dir<R, SOLVER, 1>(p, c); break;
-    default: flux1_dir<R, SOLVER, 2>(p, c); break;
+    case 0: flux1_dir<R, SOLVER, 0>(p, bx.b[0]); break;
+    case 1: flux1_dir<R, SOLVER, 1>(p, bx.b[1]); break;
+    default: flux1_dir<R, SOLVER, 2>(p, bx.b[2]); break;
   }
 }
 
-// ---- S3 / S7: upwinded edge EMFs (formula DESIGN.md R10) -------------------------------------
+// ---- S3 / S7: upwinded edge EMFs (formula DESIGN.md R10) --------------------------------------
 // edge along C at (a-1/2, b-1/2), (a,b,c) cyclic; face EMFs: from an a-face E_c = -F_a[B_t1], from a b-face E_c = +F_b[B_t2]
 // upwind switch on the face mass flux m (R10).  R10a: |m| <= m0 (less than emf_tie of the cell mass crosses the face
 // in dt) counts as zero -> centred mean; between m0 and 2 m0 a linear ramp to the upwind value keeps the EMF continuous
 template <class R> __device__ __forceinline__ R upwind(R m, R m0, R qm, R qp) {
   const R am = Num<R>::abs(m), mean = R(0.5) * (qm + qp), qu = m > R(0) ? qm : qp;
-  const R w = (am - m0) / m0;                          // weight of the upwind value on the ramp m0 < |m| < 2 m0
+  const R w = fdiv(am - m0, m0);                       // weight of the upwind value on the ramp m0 < |m| < 2 m0
   const R ramp = w * qu + (R(1) - w) * mean;
   return (am <= m0) ? mean : ((am < R(2) * m0) ? ramp : qu);
 }
 template <class R, int C>
-__device__ __forceinline__ void emf_dir(const KParams<R>& p, const Ctx<R>& c, const R* Wb, int alo, int ahi, int clo, int chi) {
+__device__ __forceinline__ void emf_dir(const KParams<R>& p, const Box3& box, int rhobase) {
   constexpr int A = (C + 1) % 3, B = (C + 2) % 3;
-  const int ia = c.idx(A), ib = c.idx(B), ic = c.idx(C);
-  if (ia < alo || ia > ahi || ib < alo || ib > ahi || ic < clo || ic >= chi) return;
-  const int S3 = p.S3, q = c.q, qa = q - c.off(A), qb = q - c.off(B), qab = qa - c.off(B);
+  Ctx<R> c(p, box);
+  if (!c.ok) return;
+  const int q = c.q, qa = q - c.off(A), qb = q - c.off(B), qab = qa - c.off(B);
   const R* Fa5 = c.arr(A_F + 7 * A + 5); const R* Fa0 = c.arr(A_F + 7 * A + 0);
   const R* Fb6 = c.arr(A_F + 7 * B + 6); const R* Fb0 = c.arr(A_F + 7 * B + 0);
-  const R* va = Wb + (size_t)(1 + A) * S3; const R* vb = Wb + (size_t)(1 + B) * S3;
-  const R* Ba = Wb + (size_t)(5 + A) * S3; const R* Bb = Wb + (size_t)(5 + B) * S3;
-  auto ec = [&](int x) { return vb[x] * Ba[x] - va[x] * Bb[x]; };   // -(v x B)_c of a cell
+  const R* ec = c.arr(A_EC + C); const R* rho = c.arr(rhobase);
   const R Ea_q = -Fa5[q], Ea_qb = -Fa5[qb], Eb_q = Fb6[q], Eb_qa = Fb6[qa];
-  const R ec_q = ec(q), ec_qa = ec(qa), ec_qb = ec(qb), ec_qab = ec(qab);
-  const R* rho = Wb;
+  const R ec_q = ec[q], ec_qa = ec[qa], ec_qb = ec[qb], ec_qab = ec[qab];
   const R ht = R(0.5) * p.tie, r_q = rho[q], r_qa = rho[qa], r_qb = rho[qb], r_qab = rho[qab];
   R e = R(0.25) * (Ea_q + Ea_qb + Eb_q + Eb_qa);
   e += R(0.25) * (upwind(Fa0[qb], ht * (r_qab + r_qb), Eb_qa - ec_qab, Eb_q - ec_qb) - upwind(Fa0[q], ht * (r_qa + r_q), ec_qa - Eb_qa, ec_q - Eb_q));
@@ -170,13 +184,12 @@ __device__ __forceinline__ void emf_dir(const KParams<R>& p, const Ctx<R>& c, co
   c.arr(A_E + C)[q] = e;
 }
 template <class R>
-__global__ void __launch_bounds__(256) k_emf(const KParams<R> p, int wbase, int alo, int ahi, int clo, int chi) {
-  Ctx<R> c(p);
-  if (!c.valid()) return;
-  const R* Wb = c.arr(wbase);
-  emf_dir<R, 0>(p, c, Wb, alo, ahi, clo, chi);
-  emf_dir<R, 1>(p, c, Wb, alo, ahi, clo, chi);
-  emf_dir<R, 2>(p, c, Wb, alo, ahi, clo, chi);
+__global__ void __launch_bounds__(256) k_emf(const KParams<R> p, const Box3x3 bx, int rhobase) {
+  switch (blockIdx.y) {
+    case 0: emf_dir<R, 0>(p, bx.b[0], rhobase); break;
+    case 1: emf_dir<R, 1>(p, bx.b[1], rhobase); break;
+    default: emf_dir<R, 2>(p, bx.b[2], rhobase); break;
+  }
 }
 
 // Eq. 13 for the lower D-face of cell x (flat index), step factor qh = tau/dh
@@ -216,10 +229,9 @@ __device__ __forceinline__ void load_U_in(const KParams<R>& p, const Ctx<R>& c, 
 
 // ---- S4: half-step state: U^{n+1/2}, b^{n+1/2} on the faces of the cells, W^{n+1/2} -------
 template <class R>
-__global__ void __launch_bounds__(256) k_half(const KParams<R> p, int lo, int hi) {
-  Ctx<R> c(p);
-  if (!c.valid()) return;
-  if (c.i < lo || c.i >= hi || c.j < lo || c.j >= hi || c.k < lo || c.k >= hi) return;
+__global__ void __launch_bounds__(256) k_half(const KParams<R> p, const Box3 box) {
+  Ctx<R> c(p, box);
+  if (!c.ok) return;
   const R qh = (R(0.5) * p.dt) / p.dh;
   R u[5], dU[5];
   load_U_in(p, c, u);
@@ -232,13 +244,12 @@ __global__ void __launch_bounds__(256) k_half(const KParams<R> p, int lo, int hi
   bl[1] = ct_face<R, 1>(c, c.arr(A_B + 1), q, qh); bu[1] = ct_face<R, 1>(c, c.arr(A_B + 1), q + p.S, qh);
   bl[2] = ct_face<R, 2>(c, c.arr(A_B + 2), q, qh); bu[2] = ct_face<R, 2>(c, c.arr(A_B + 2), q + p.S2, qh);
   c.arr(A_BH + 0)[q] = bl[0]; c.arr(A_BH + 1)[q] = bl[1]; c.arr(A_BH + 2)[q] = bl[2];
-  if (c.i == hi - 1) c.arr(A_BH + 0)[q + 1] = bu[0];
-  if (c.j == hi - 1) c.arr(A_BH + 1)[q + p.S] = bu[1];
-  if (c.k == hi - 1) c.arr(A_BH + 2)[q + p.S2] = bu[2];
+  if (c.i == box.lo[0] + box.n[0] - 1) c.arr(A_BH + 0)[q + 1] = bu[0];
+  if (c.j == box.lo[1] + box.n[1] - 1) c.arr(A_BH + 1)[q + p.S] = bu[1];
+  if (c.k == box.lo[2] + box.n[2] - 1) c.arr(A_BH + 2)[q + p.S2] = bu[2];
   R W[8];
   cons_to_prim(p, u, bl, bu, W);
-#pragma unroll
-  for (int v = 0; v < 8; ++v) c.arr(A_WH + v)[q] = W[v];
+  store_prim(c, A_WH, W);
 }
 
 }  // namespace mhd

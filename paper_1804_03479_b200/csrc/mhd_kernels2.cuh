@@ -1,5 +1,4 @@
-// mhd_kernels2.cuh -- second half of the stage kernels: VL step 4+5, CTU steps 1, 2/6 and 5, the full update
-// with the coarse-fine boundary planes, and the CFL reduction.  See mhd_kernels.cuh for the layout.
+// mhd_kernels2.cuh -- stage kernels, part 2: VL steps 4+5, CTU steps 1, 2/6 and 5.  See mhd_kernels.cuh for the layout.
 #pragma once
 #include "mhd_kernels.cuh"
 
@@ -7,10 +6,9 @@ namespace mhd {
 
 // ---- VL steps 4+5: PLM at the half step + Riemann solve, normal B = half-step face value --------
 template <class R, int SOLVER, int LIMVAR, int D>
-__device__ __forceinline__ void flux2_vl_dir(const KParams<R>& p, const Ctx<R>& c) {
-  constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
-  const int T = p.T;
-  if (c.idx(D) < 3 || c.idx(D) > T - 3 || c.idx(T1) < 1 || c.idx(T1) >= T - 1 || c.idx(T2) < 1 || c.idx(T2) >= T - 1) return;
+__device__ __forceinline__ void flux2_vl_dir(const KParams<R>& p, const Box3& box) {
+  Ctx<R> c(p, box);
+  if (!c.ok) return;
   const int o = c.off(D), q = c.q;
   const R* Wh = c.arr(A_WH);
   R wmm[7], wm[7], w0[7], wp[7], sl[7], sr[7];
@@ -30,22 +28,45 @@ __device__ __forceinline__ void flux2_vl_dir(const KParams<R>& p, const Ctx<R>& 
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[q] = F[v];
 }
 template <class R, int SOLVER, int LIMVAR>
-__global__ void __launch_bounds__(256) k_flux2_vl(const KParams<R> p) {
-  Ctx<R> c(p);
-  if (!c.valid()) return;
+__global__ void __launch_bounds__(256) k_flux2_vl(const KParams<R> p, const Box3x3 bx) {
   switch (blockIdx.y) {
-    case 0: flux2_vl_dir<R, SOLVER, LIMVAR, 0>(p, c); break;
-    case 1: flux2_vl_dir<R, SOLVER, LIMVAR, 1>(p, c); break;
-    default: flux2_vl_dir<R, SOLVER, LIMVAR, 2>(p, c); break;
+    case 0: flux2_vl_dir<R, SOLVER, LIMVAR, 0>(p, bx.b[0]); break;
+    case 1: flux2_vl_dir<R, SOLVER, LIMVAR, 1>(p, bx.b[1]); break;
+    default: flux2_vl_dir<R, SOLVER, LIMVAR, 2>(p, bx.b[2]); break;
   }
 }
 
 // ---- CTU step 1: reconstruction + half-step tracing + primitive MHD source terms ------------------
+// PPM needs the limited slope of three cells per cell: the slopes are computed once per cell and direction by
+// k_slope_ctu (parked in the flux arrays, which are free until step 2) and read back here.
+template <class R, int LIMVAR, int D>
+__device__ __forceinline__ void slope_ctu_dir(const KParams<R>& p, const Box3& box) {
+  Ctx<R> c(p, box);
+  if (!c.ok) return;
+  const int o = c.off(D), q = c.q, S3 = p.S3;
+  const R* W = c.arr(A_W);
+  R wm[7], w0[7], wp[7], dw[7];
+  load_gen<R, D>(W, S3, q - o, wm);
+  load_gen<R, D>(W, S3, q, w0);
+  load_gen<R, D>(W, S3, q + o, wp);
+  slope3<R, LIMVAR>(wm, w0, wp, W[(size_t)(5 + D) * S3 + q], p.gam, dw);
+#pragma unroll
+  for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[q] = dw[v];
+}
+template <class R, int LIMVAR>
+__global__ void __launch_bounds__(256) k_slope_ctu(const KParams<R> p, const Box3x3 bx) {
+  switch (blockIdx.y) {
+    case 0: slope_ctu_dir<R, LIMVAR, 0>(p, bx.b[0]); break;
+    case 1: slope_ctu_dir<R, LIMVAR, 1>(p, bx.b[1]); break;
+    default: slope_ctu_dir<R, LIMVAR, 2>(p, bx.b[2]); break;
+  }
+}
+
 template <class R, int RECON, int LIMVAR, int D>
-__device__ __forceinline__ void recon_ctu_dir(const KParams<R>& p, const Ctx<R>& c) {
+__device__ __forceinline__ void recon_ctu_dir(const KParams<R>& p, const Box3& box) {
   constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
-  const int T = p.T, r = (RECON == kPLM) ? 1 : 2;
-  if (c.i >= T || c.j >= T || c.k >= T || c.idx(D) < r || c.idx(D) >= T - r) return;
+  Ctx<R> c(p, box);
+  if (!c.ok) return;
   const int o = c.off(D), q = c.q, S3 = p.S3;
   const R* W = c.arr(A_W);
   const R* Bn = W + (size_t)(5 + D) * S3;
@@ -59,18 +80,19 @@ __device__ __forceinline__ void recon_ctu_dir(const KParams<R>& p, const Ctx<R>&
     slope3<R, LIMVAR>(wm, w0, wp, Bn[q], p.gam, dw);
     plm_trace(w0, Bn[q], p.gam, sig, dw, wlo, wup);
   } else {
-    R wmm[7], wpp[7], sm[7], s0[7], sp[7];
-    load_gen<R, D>(W, S3, q - 2 * o, wmm);
-    load_gen<R, D>(W, S3, q + 2 * o, wpp);
-    slope3<R, LIMVAR>(wmm, wm, w0, Bn[q - o], p.gam, sm);
-    slope3<R, LIMVAR>(wm, w0, wp, Bn[q], p.gam, s0);
-    slope3<R, LIMVAR>(w0, wp, wpp, Bn[q + o], p.gam, sp);
+    R sm[7], s0[7], sp[7];
+#pragma unroll
+    for (int v = 0; v < 7; ++v) {
+      const R* sl = c.arr(A_F + 7 * D + v);
+      sm[v] = sl[q - o]; s0[v] = sl[q]; sp[v] = sl[q + o];
+    }
     ppm_trace(wm, w0, wp, sm, s0, sp, Bn[q], p.gam, sig, wlo, wup);
   }
   const R* bn_ = c.arr(A_B + D); const R* b1_ = c.arr(A_B + T1); const R* b2_ = c.arr(A_B + T2);
-  const R dbn = (bn_[q + o] - bn_[q]) / p.dh;
-  const R db1 = (b1_[q + c.off(T1)] - b1_[q]) / p.dh;
-  const R db2 = (b2_[q + c.off(T2)] - b2_[q]) / p.dh;
+  const R idh = R(1) / p.dh;
+  const R dbn = (bn_[q + o] - bn_[q]) * idh;
+  const R db1 = (b1_[q + c.off(T1)] - b1_[q]) * idh;
+  const R db2 = (b2_[q + c.off(T2)] - b2_[q]) * idh;
   const R s1 = hdt * w0[2] * lim_minmod(dbn, -db1), s2 = hdt * w0[3] * lim_minmod(dbn, -db2);
   wlo[5] += s1; wup[5] += s1; wlo[6] += s2; wup[6] += s2;
   apply_floors(p, wlo); apply_floors(p, wup);
@@ -78,21 +100,19 @@ __device__ __forceinline__ void recon_ctu_dir(const KParams<R>& p, const Ctx<R>&
   for (int v = 0; v < 7; ++v) { c.arr(A_LO + 7 * D + v)[q] = wlo[v]; c.arr(A_UP + 7 * D + v)[q] = wup[v]; }
 }
 template <class R, int RECON, int LIMVAR>
-__global__ void __launch_bounds__(256) k_recon_ctu(const KParams<R> p) {
-  Ctx<R> c(p);
-  if (!c.valid()) return;
+__global__ void __launch_bounds__(256) k_recon_ctu(const KParams<R> p, const Box3x3 bx) {
   switch (blockIdx.y) {
-    case 0: recon_ctu_dir<R, RECON, LIMVAR, 0>(p, c); break;
-    case 1: recon_ctu_dir<R, RECON, LIMVAR, 1>(p, c); break;
-    default: recon_ctu_dir<R, RECON, LIMVAR, 2>(p, c); break;
+    case 0: recon_ctu_dir<R, RECON, LIMVAR, 0>(p, bx.b[0]); break;
+    case 1: recon_ctu_dir<R, RECON, LIMVAR, 1>(p, bx.b[1]); break;
+    default: recon_ctu_dir<R, RECON, LIMVAR, 2>(p, bx.b[2]); break;
   }
 }
 
 // ---- CTU steps 2 and 6: Riemann solve between the upper state of cell i-1 and the lower of i ----
 template <class R, int SOLVER, int D>
-__device__ __forceinline__ void flux_lr_dir(const KParams<R>& p, const Ctx<R>& c, int bbase, int nlo, int nhi, int tlo, int thi) {
-  constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
-  if (c.idx(D) < nlo || c.idx(D) >= nhi || c.idx(T1) < tlo || c.idx(T1) >= thi || c.idx(T2) < tlo || c.idx(T2) >= thi) return;
+__device__ __forceinline__ void flux_lr_dir(const KParams<R>& p, const Box3& box, int bbase) {
+  Ctx<R> c(p, box);
+  if (!c.ok) return;
   const int q = c.q, ql = q - c.off(D);
   R wl[7], wr[7], F[7];
 #pragma unroll
@@ -103,22 +123,22 @@ __device__ __forceinline__ void flux_lr_dir(const KParams<R>& p, const Ctx<R>& c
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[q] = F[v];
 }
 template <class R, int SOLVER>
-__global__ void __launch_bounds__(256) k_flux_lr(const KParams<R> p, int bbase, int nlo, int nhi, int tlo, int thi) {
-  Ctx<R> c(p);
-  if (!c.valid()) return;
+__global__ void __launch_bounds__(256) k_flux_lr(const KParams<R> p, const Box3x3 bx, int bbase) {
   switch (blockIdx.y) {
-    case 0: flux_lr_dir<R, SOLVER, 0>(p, c, bbase, nlo, nhi, tlo, thi); break;
-    case 1: flux_lr_dir<R, SOLVER, 1>(p, c, bbase, nlo, nhi, tlo, thi); break;
-    default: flux_lr_dir<R, SOLVER, 2>(p, c, bbase, nlo, nhi, tlo, thi); break;
+    case 0: flux_lr_dir<R, SOLVER, 0>(p, bx.b[0], bbase); break;
+    case 1: flux_lr_dir<R, SOLVER, 1>(p, bx.b[1], bbase); break;
+    default: flux_lr_dir<R, SOLVER, 2>(p, bx.b[2], bbase); break;
   }
 }
 
 // ---- CTU step 5: transverse flux-gradient correction + conservative MHD source terms (R6) -----------
+// flo / fhi: range of faces of direction D on which the half-step normal field exists
 template <class R, int D>
-__device__ __forceinline__ void ctu_corr_dir(const KParams<R>& p, const Ctx<R>& c, int r) {
+__device__ __forceinline__ void ctu_corr_dir(const KParams<R>& p, const Box3& box, int flo, int fhi) {
   constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
-  const int T = p.T, cn = c.idx(D);
-  if (cn < r || cn >= T - r || c.idx(T1) < r + 1 || c.idx(T1) >= T - 1 - r || c.idx(T2) < r + 1 || c.idx(T2) >= T - 1 - r) return;
+  Ctx<R> c(p, box);
+  if (!c.ok) return;
+  const int cn = c.idx(D);
   const int q = c.q, od = c.off(D), o1 = c.off(T1), o2 = c.off(T2);
   const size_t S3 = p.S3;
   const R hdt = R(0.5) * p.dt, qh = hdt / p.dh;
@@ -136,13 +156,14 @@ __device__ __forceinline__ void ctu_corr_dir(const KParams<R>& p, const Ctx<R>& 
   const R dB1 = -qh * R(0.5) * ((Emp - Emm) + (Epp - Epm));
   const R dB2 = qh * R(0.5) * ((Epm - Emm) + (Epp - Emp));
   const R* bn_ = c.arr(A_B + D); const R* b1_ = c.arr(A_B + T1); const R* b2_ = c.arr(A_B + T2);
-  const R dbn = (bn_[q + od] - bn_[q]) / p.dh, db1 = (b1_[q + o1] - b1_[q]) / p.dh, db2 = (b2_[q + o2] - b2_[q]) / p.dh;
+  const R idh = R(1) / p.dh;
+  const R dbn = (bn_[q + od] - bn_[q]) * idh, db1 = (b1_[q + o1] - b1_[q]) * idh, db2 = (b2_[q + o2] - b2_[q]) * idh;
   const R m1 = lim_minmod(dbn, -db2), m2 = lim_minmod(dbn, -db1);
   const R Bc1 = w0[5], Bc2 = w0[6], v1 = w0[2], v2 = w0[3];
 #pragma unroll
   for (int side = 0; side < 2; ++side) {
     const int face = cn + side;
-    if (face < r + 1 || face > T - 1 - r) continue;
+    if (face < flo || face > fhi) continue;
     const int qf = q + (side ? od : 0);
     const int base = (side ? A_UP : A_LO) + 7 * D;
     R w[7], u[7];
@@ -150,7 +171,7 @@ __device__ __forceinline__ void ctu_corr_dir(const KParams<R>& p, const Ctx<R>& 
     for (int v = 0; v < 7; ++v) w[v] = c.arr(base + v)[q];
     const R bnn = bn_[qf];
     u[0] = w[0]; u[1] = w[0] * w[1]; u[2] = w[0] * w[2]; u[3] = w[0] * w[3];
-    u[4] = w[4] / p.gm1 + R(0.5) * w[0] * (sqr(w[1]) + sqr(w[2]) + sqr(w[3])) + R(0.5) * (sqr(bnn) + sqr(w[5]) + sqr(w[6]));
+    u[4] = w[4] * p.gm1inv + R(0.5) * w[0] * (sqr(w[1]) + sqr(w[2]) + sqr(w[3])) + R(0.5) * (sqr(bnn) + sqr(w[5]) + sqr(w[6]));
     u[5] = w[5]; u[6] = w[6];
     u[0] -= qh * dF0; u[1] -= qh * dF1; u[2] -= qh * dF2; u[3] -= qh * dF3; u[4] -= qh * dF4;
     u[5] += dB1; u[6] += dB2;
@@ -160,7 +181,8 @@ __device__ __forceinline__ void ctu_corr_dir(const KParams<R>& p, const Ctx<R>& 
     const R bh = c.arr(A_BH + D)[qf];
     R rho = u[0];
     if (rho < p.min_dens) { rho = p.min_dens; count_event(p.stats + 0); }
-    w[0] = rho; w[1] = u[1] / rho; w[2] = u[2] / rho; w[3] = u[3] / rho; w[5] = u[5]; w[6] = u[6];
+    const R ir = frcp(rho);
+    w[0] = rho; w[1] = u[1] * ir; w[2] = u[2] * ir; w[3] = u[3] * ir; w[5] = u[5]; w[6] = u[6];
     w[4] = p.gm1 * (u[4] - R(0.5) * rho * (sqr(w[1]) + sqr(w[2]) + sqr(w[3])) - R(0.5) * (sqr(bh) + sqr(w[5]) + sqr(w[6])));
     if (w[4] < p.min_pres) { w[4] = p.min_pres; count_event(p.stats + 1); }
 #pragma unroll
@@ -168,13 +190,11 @@ __device__ __forceinline__ void ctu_corr_dir(const KParams<R>& p, const Ctx<R>& 
   }
 }
 template <class R>
-__global__ void __launch_bounds__(256) k_ctu_corr(const KParams<R> p, int r) {
-  Ctx<R> c(p);
-  if (!c.valid()) return;
+__global__ void __launch_bounds__(256) k_ctu_corr(const KParams<R> p, const Box3x3 bx, int flo, int fhi) {
   switch (blockIdx.y) {
-    case 0: ctu_corr_dir<R, 0>(p, c, r); break;
-    case 1: ctu_corr_dir<R, 1>(p, c, r); break;
-    default: ctu_corr_dir<R, 2>(p, c, r); break;
+    case 0: ctu_corr_dir<R, 0>(p, bx.b[0], flo, fhi); break;
+    case 1: ctu_corr_dir<R, 1>(p, bx.b[1], flo, fhi); break;
+    default: ctu_corr_dir<R, 2>(p, bx.b[2], flo, fhi); break;
   }
 }
 

@@ -1,18 +1,46 @@
-// mhd_kernels3.cuh -- full update, coarse-fine boundary planes and the
-// CFL reduction.  See mhd_kernels.cuh for the layout.
+// mhd_kernels3.cuh -- stage kernels, part 3: full update with the coarse-fine boundary planes
+// (PAPER.md:207), and the CFL reduction.  See mhd_kernels.cuh for the layout.
 #pragma once
 #include "mhd_kernels2.cuh"
 
 namespace mhd {
 
-// ---- S8: U^{n+1} = U^n - dt/dh sum dF2 (Eq. 10) on the N^3 interior cells, b^{n+1} by Eq. 13 on their faces -------
+// ---- S8: U^{n+1} = U^n - dt/dh sum dF2 (Eq. 10) on the N^3 interior cells, b^{n+1} by Eq. 13 on their faces;
+// epilogue: time-centred fluxes and edge EMFs on the lower / mid / upper face planes of each
+// direction, copied by the first 9 (N+1)^2 threads of the group (one per plane point (a2, a1), a1, a2 in [0, N]) -------
 template <class R>
-__global__ void __launch_bounds__(256) k_final(const KParams<R> p) {
-  Ctx<R> c(p);
-  if (!c.valid()) return;
+__device__ __forceinline__ void copy_planes(const KParams<R>& p, int grp, int t) {
+  const int N = p.N, M = N + 1, g = p.g;
+  if (t >= 9 * M * M) return;
+  const int a1 = t % M, a2 = (t / M) % M, pl = t / (M * M);
+  const int d = pl / 3, s = pl - 3 * d, t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+  const int fi = (s == 0 ? 0 : (s == 1 ? N / 2 : N)) + g, c1 = a1 + g, c2 = a2 + g;
+  // flat index with idx[d] = fi, idx[t1] = c1, idx[t2] = c2
+  const int ix = d == 0 ? fi : (t1 == 0 ? c1 : c2), iy = d == 1 ? fi : (t1 == 1 ? c1 : c2), iz = d == 2 ? fi : (t1 == 2 ? c1 : c2);
+  const int q = (iz * p.S + iy) * p.S + ix;
+  const R* w = p.ws + (size_t)grp * p.narr * p.S3;
+  if (p.fout && a1 < N && a2 < N) {
+    const R* F = w + (size_t)(A_F + 7 * d) * p.S3;
+    const R f0 = F[q], fn = F[(size_t)p.S3 + q], f1 = F[(size_t)2 * p.S3 + q], f2 = F[(size_t)3 * p.S3 + q], f4 = F[(size_t)4 * p.S3 + q];
+    R* fo = p.fout + (size_t)grp * p.nF + (size_t)pl * 5 * N * N + (size_t)a2 * N + a1;
+    const size_t NN = (size_t)N * N;
+    fo[0] = f0; fo[(size_t)(1 + d) * NN] = fn; fo[(size_t)(1 + t1) * NN] = f1; fo[(size_t)(1 + t2) * NN] = f2; fo[4 * NN] = f4;
+  }
+  if (p.eout) {
+    R* e0 = p.eout + (size_t)grp * p.nE + (size_t)pl * 2 * M * N;
+    R* e1 = e0 + (size_t)M * N;
+    if (a1 < N) e0[(size_t)a2 * N + a1] = w[(size_t)(A_E + t1) * p.S3 + q];
+    if (a2 < N) e1[(size_t)a2 * M + a1] = w[(size_t)(A_E + t2) * p.S3 + q];
+  }
+}
+
+template <class R>
+__global__ void __launch_bounds__(256) k_final(const KParams<R> p, const Box3 box) {
+  Ctx<R> c(p, box);
+  if (p.fout || p.eout) copy_planes(p, blockIdx.z, blockIdx.x * blockDim.x + threadIdx.x);
+  if (!c.ok) return;
   const int g = p.g, N = p.N;
   const int ii = c.i - g, jj = c.j - g, kk = c.k - g;
-  if (ii < 0 || ii >= N || jj < 0 || jj >= N || kk < 0 || kk >= N) return;
   const R qh = p.dt / p.dh;
   R u[5], dU[5];
   load_U_in(p, c, u);
@@ -31,37 +59,6 @@ __global__ void __launch_bounds__(256) k_final(const KParams<R> p) {
   if (ii == N - 1) Bx[((size_t)kk * N + jj) * (N + 1) + N] = ct_face<R, 0>(c, c.arr(A_B + 0), q + 1, qh);
   if (jj == N - 1) By[((size_t)kk * (N + 1) + N) * N + ii] = ct_face<R, 1>(c, c.arr(A_B + 1), q + p.S, qh);
   if (kk == N - 1) Bz[((size_t)N * N + jj) * N + ii] = ct_face<R, 2>(c, c.arr(A_B + 2), q + p.S2, qh);
-}
-
-// ---- epilogue: time-centred fluxes and edge EMFs on the lower / mid / upper face planes of each direction ----------
-// one thread per (plane, a2, a1) with a1, a2 in [0, N]
-template <class R>
-__global__ void __launch_bounds__(256) k_planes(const KParams<R> p) {
-  const int N = p.N, M = N + 1, g = p.g;
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= 9 * M * M) return;
-  const int grp = blockIdx.z;
-  const int a1 = t % M, a2 = (t / M) % M, pl = t / (M * M);
-  const int d = pl / 3, s = pl % 3, t1 = (d + 1) % 3, t2 = (d + 2) % 3;
-  int id[3];
-  id[d] = (s == 0 ? 0 : (s == 1 ? N / 2 : N)) + g; id[t1] = a1 + g; id[t2] = a2 + g;
-  const int q = (id[2] * p.S + id[1]) * p.S + id[0];
-  const R* w = p.ws + (size_t)grp * p.narr * p.S3;
-  if (p.fout && a1 < N && a2 < N) {
-    const R* F = w + (size_t)(A_F + 7 * d) * p.S3;
-    R fg[5];
-    fg[0] = F[q]; fg[1 + d] = F[(size_t)p.S3 + q]; fg[1 + t1] = F[(size_t)2 * p.S3 + q]; fg[1 + t2] = F[(size_t)3 * p.S3 + q];
-    fg[4] = F[(size_t)4 * p.S3 + q];
-    R* fo = p.fout + (size_t)grp * p.nF + (size_t)pl * 5 * N * N + (size_t)a2 * N + a1;
-#pragma unroll
-    for (int v = 0; v < 5; ++v) fo[(size_t)v * N * N] = fg[v];
-  }
-  if (p.eout) {
-    R* e0 = p.eout + (size_t)grp * p.nE + (size_t)pl * 2 * M * N;
-    R* e1 = e0 + (size_t)M * N;
-    if (a1 < N) e0[(size_t)a2 * N + a1] = w[(size_t)(A_E + t1) * p.S3 + q];
-    if (a2 < N) e1[(size_t)a2 * M + a1] = w[(size_t)(A_E + t2) * p.S3 + q];
-  }
 }
 
 // ---- S9: CFL (R13): max over interior cells and directions of |v_d| + c_f,d -------------------

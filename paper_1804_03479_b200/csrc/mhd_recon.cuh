@@ -28,11 +28,11 @@ __device__ __forceinline__ void limited_slope(const R (&w0)[7], R bn, R gam, con
     for (int v = 0; v < 7; ++v) dw[v] = lim_mc(dl[v], dr[v]);
     return;
   }
-  const R rho = w0[0], irho = R(1) / rho;
-  const R a2 = gam * w0[4] * irho, a = Num<R>::sqrt(a2), srho = Num<R>::sqrt(rho), isrho = R(1) / srho;
+  const R rho = w0[0], irho = frcp(rho);
+  const R a2 = gam * w0[4] * irho, a = Num<R>::sqrt(a2), srho = Num<R>::sqrt(rho), isrho = frcp(srho);
   const WaveSet<R> w = wave_set(a2, rho, bn, w0[5], w0[6]);
   const R Qf = w.cf * w.af * w.S, Qs = w.cs * w.as * w.S, Af = a * w.af * srho, As = a * w.as * srho;
-  const R nn = R(0.5) / a2;
+  const R nn = fdiv(R(0.5), a2);
 #pragma unroll
   for (int v = 0; v < 7; ++v) dw[v] = R(0);
 #pragma unroll
@@ -55,7 +55,7 @@ __device__ __forceinline__ void limited_slope(const R (&w0)[7], R bn, R gam, con
       Rk[0] = rho * w.as; Rk[1] = -s * w.cs * w.as; Rk[2] = -s * Qf * w.b1; Rk[3] = -s * Qf * w.b2;
       Rk[4] = rho * a2 * w.as; Rk[5] = -Af * w.b1; Rk[6] = -Af * w.b2;
     } else {
-      Lk[0] = R(1); Lk[1] = R(0); Lk[2] = R(0); Lk[3] = R(0); Lk[4] = -R(1) / a2; Lk[5] = R(0); Lk[6] = R(0);
+      Lk[0] = R(1); Lk[1] = R(0); Lk[2] = R(0); Lk[3] = R(0); Lk[4] = -R(2) * nn; Lk[5] = R(0); Lk[6] = R(0);
       Rk[0] = R(1); Rk[1] = R(0); Rk[2] = R(0); Rk[3] = R(0); Rk[4] = R(0); Rk[5] = R(0); Rk[6] = R(0);
     }
     R al = R(0), ar = R(0);
@@ -79,7 +79,7 @@ __device__ __forceinline__ void slope3(const R (&wm)[7], const R (&w0)[7], const
 template <class R>
 __device__ __forceinline__ void plm_trace(const R (&w0)[7], R bn, R gam, R sig, const R (&dw)[7], R (&wlo)[7], R (&wup)[7]) {
   R Ad[7];
-  jac_mul(w0, bn, gam, R(1) / w0[0], dw, Ad);
+  jac_mul(w0, bn, gam, frcp(w0[0]), dw, Ad);
 #pragma unroll
   for (int v = 0; v < 7; ++v) {
     wup[v] = w0[v] + R(0.5) * dw[v] - R(0.5) * sig * Ad[v];
@@ -95,8 +95,8 @@ __device__ __forceinline__ void ppm_trace(const R (&wm)[7], const R (&w0)[7], co
   R Wl[7], Wr[7], xu[7], xl[7], W6[7];
 #pragma unroll
   for (int v = 0; v < 7; ++v) {
-    R l = R(0.5) * (wm[v] + w0[v]) - (s0[v] - sm[v]) / R(6);
-    R r = R(0.5) * (w0[v] + wp[v]) - (sp[v] - s0[v]) / R(6);
+    R l = R(0.5) * (wm[v] + w0[v]) - (s0[v] - sm[v]) * R(1.0 / 6.0);
+    R r = R(0.5) * (w0[v] + wp[v]) - (sp[v] - s0[v]) * R(1.0 / 6.0);
     if ((r - w0[v]) * (w0[v] - l) <= R(0)) { l = w0[v]; r = w0[v]; }
     const R d = r - l, w6 = R(6) * (w0[v] - R(0.5) * (l + r));
     R nl = l, nr = r;
@@ -109,7 +109,7 @@ __device__ __forceinline__ void ppm_trace(const R (&wm)[7], const R (&w0)[7], co
     W6[v] = R(6) * (w0[v] - R(0.5) * (l + r));
     xu[v] = dd - W6[v]; xl[v] = dd + W6[v];
   }
-  const R irho = R(1) / w0[0];
+  const R irho = frcp(w0[0]);
   R Au[7], Al[7], A6[7], AA6[7];
   jac_mul(w0, bn, gam, irho, xu, Au);
   jac_mul(w0, bn, gam, irho, xl, Al);
@@ -117,8 +117,8 @@ __device__ __forceinline__ void ppm_trace(const R (&wm)[7], const R (&w0)[7], co
   jac_mul(w0, bn, gam, irho, A6, AA6);
 #pragma unroll
   for (int v = 0; v < 7; ++v) {
-    wup[v] = Wr[v] - R(0.5) * sig * Au[v] - sig * sig * AA6[v] / R(3);
-    wlo[v] = Wl[v] - R(0.5) * sig * Al[v] - sig * sig * AA6[v] / R(3);
+    wup[v] = Wr[v] - R(0.5) * sig * Au[v] - sig * sig * AA6[v] * R(1.0 / 3.0);
+    wlo[v] = Wl[v] - R(0.5) * sig * Al[v] - sig * sig * AA6[v] * R(1.0 / 3.0);
   }
 }
 
