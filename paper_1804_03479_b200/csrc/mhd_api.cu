@@ -298,11 +298,13 @@ int mhd_create(const mhd_config* cfg, mhd_solver** out) {
   s->nUo = 5 * N * N * N; s->nBo = 3 * N * N * (N + 1);
   s->nF = 9 * 5 * N * N; s->nE = 9 * 2 * (N + 1) * N;
   // Lanes x slice: nlanes slices are in flight at once; a slice holds as many groups as fit the per-lane share of
-  // the workspace budget (MHD_LANES / MHD_SLICE_MB / MHD_SLICE_GROUPS override for experiments)
-  int nl = 3;
+  // the workspace budget.  Measured on B200: time per group falls monotonically with the slice size even far beyond
+  // the L2 capacity, so slices only bound the workspace memory (MHD_LANES / MHD_SLICE_MB /
+  // MHD_SLICE_GROUPS override for experiments)
+  int nl = 2;
   if (const char* e = getenv("MHD_LANES")) { int v = atoi(e); if (v >= 1) nl = v; }
   s->nlanes = std::min(nl, kMaxStreams);
-  double budget_mb = 288.0;
+  double budget_mb = 6144.0;
   if (const char* e = getenv("MHD_SLICE_MB")) { double v = atof(e); if (v > 0) budget_mb = v; }
   const size_t per_group = ((size_t)s->narr * s->S3 + s->nUi + s->nBi + s->nUo + s->nBo + s->nF + s->nE) * s->esz;
   long sg = (long)(budget_mb * 1048576.0 / s->nlanes / (double)per_group);
