@@ -16,12 +16,25 @@
 namespace mhd {
 
 enum : int { kHLLE = 0, kHLLD = 1, kROE = 2 };
+
+// resident 256-thread blocks per SM requested from ptxas for the ALU-bound (Riemann / reconstruction) kernels
+#ifndef MHD_MINB32
+#define MHD_MINB32 4
+#endif
+#ifndef MHD_MINB64
+#define MHD_MINB64 2
+#endif
+#ifndef MHD_MINB64_FLUX
+#define MHD_MINB64_FLUX 3
+#endif
+template <class R> struct Occ { static constexpr int minb = sizeof(R) == 8 ? MHD_MINB64 : MHD_MINB32; };          // reconstruction
+template <class R> struct OccFlux { static constexpr int minb = sizeof(R) == 8 ? MHD_MINB64_FLUX : MHD_MINB32; }; // Riemann kernels (measured: FP64 3 > 2 > 4)
 enum : int { kPLM = 0, kPPM = 1 };
 enum : int { kLimPrim = 0, kLimChar = 1 };
 
 template <class R> struct Num;
 template <> struct Num<float> {
-  static __device__ __forceinline__ float sqrt(float x) { float r; asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+  static __device__ __forceinline__ float sqrt(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
   static __device__ __forceinline__ float abs(float x) { return fabsf(x); }
   static __device__ __forceinline__ float min(float a, float b) { return fminf(a, b); }
   static __device__ __forceinline__ float max(float a, float b) { return fmaxf(a, b); }
@@ -40,8 +53,31 @@ template <class R> __device__ __forceinline__ R sqr(R x) { return x * x; }
 // (1e-4 after 10 steps) is four orders of magnitude above their error.
 __device__ __forceinline__ double frcp(double x) { return 1.0 / x; }
 __device__ __forceinline__ double fdiv(double a, double b) { return a / b; }
-__device__ __forceinline__ float frcp(float x) { float r; asm("rcp.approx.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float frcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float fdiv(float a, float b) { return a * frcp(b); }
+__device__ __forceinline__ float frsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ double frsqrt(double x) { return rsqrt(x); }
+// sqrt(x) and 1/sqrt(x): FP64 from one rsqrt (sqrt = x * rsqrt), FP32 from the two SFU approximations
+__device__ __forceinline__ void sqrt_and_inverse(double x, double& s, double& is) { is = rsqrt(x); s = x * is; }
+__device__ __forceinline__ void sqrt_and_inverse(float x, float& s, float& is) {
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(x));
+  is = frcp(s);
+}
+// several reciprocals at once.  FP32: one SFU op each.  FP64: ONE division for the product and a few multiplications
+// (a double division is ~10 DFMA-pipe instructions plus a slow-path call); all arguments must be finite and non-zero.
+__device__ __forceinline__ void frcp2(float a, float b, float& ia, float& ib) { ia = frcp(a); ib = frcp(b); }
+__device__ __forceinline__ void frcp2(double a, double b, double& ia, double& ib) {
+  const double inv = 1.0 / (a * b);
+  ia = b * inv; ib = a * inv;
+}
+__device__ __forceinline__ void frcp4(float a, float b, float c, float d, float& ia, float& ib, float& ic, float& id) {
+  ia = frcp(a); ib = frcp(b); ic = frcp(c); id = frcp(d);
+}
+__device__ __forceinline__ void frcp4(double a, double b, double c, double d, double& ia, double& ib, double& ic, double& id) {
+  const double ab = a * b, cd = c * d, inv = 1.0 / (ab * cd);
+  const double iab = cd * inv, icd = ab * inv;
+  ia = b * iab; ib = a * iab; ic = d * icd; id = c * icd;
+}
 
 // monotonised-central limiter (R5)
 template <class R> __device__ __forceinline__ R lim_mc(R a, R b) {
@@ -105,15 +141,42 @@ __device__ __forceinline__ R fast_speed(R rho, R P, R bn2, R bt2, R gam) {
 }
 
 // ---- HLLD (Miyoshi & Kusano form; R7/R12) ------------------------------------------------
+// Evaluation notes (all algebraic identities of the reading): the scalars of both sides first, the
+// reciprocals of independent denominators batched (frcp2 / frcp4), sqrt(rho*) together with its reciprocal from one
+// rsqrt, and the flux / conserved vectors only of the side the face turns out to lie on.
 template <class R>
 __device__ __forceinline__ void riemann_hlld(const R (&wl)[7], const R (&wr)[7], R bn, R gam, R gm1inv, R (&F)[7]) {
   const R bn2 = bn * bn;
-  Side<R> L, Rr;
-  side_setup(wl, bn, bn2, gm1inv, gam, L);
-  side_setup(wr, bn, bn2, gm1inv, gam, Rr);
+  R irL, irR;
+  frcp2(wl[0], wr[0], irL, irR);
+  R pT[2], vB[2], en[2], cf[2], gg[2], root[2], xx[2];
+#pragma unroll
+  for (int a = 0; a < 2; ++a) {
+    const R (&w)[7] = a ? wr : wl;
+    const R ir = a ? irR : irL;
+    const R bt2 = w[5] * w[5] + w[6] * w[6];
+    const R pmag = R(0.5) * (bn2 + bt2);
+    pT[a] = w[4] + pmag;
+    vB[a] = bn * w[1] + w[5] * w[2] + w[6] * w[3];
+    en[a] = w[4] * gm1inv + R(0.5) * w[0] * (w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) + pmag;
+    // c_f^2 = 1/2 [ (a^2+ca^2+ct^2) + sqrt( (ca^2+ct^2-a^2)^2 + 4 a^2 ct^2 ) ]   (R1, R18)
+    const R a2 = gam * w[4] * ir, ca2 = bn2 * ir, ct2 = bt2 * ir;
+    const R sum = a2 + ca2 + ct2, dif = ca2 + ct2 - a2;
+    root[a] = Num<R>::sqrt(dif * dif + R(4) * a2 * ct2);
+    cf[a] = Num<R>::sqrt(R(0.5) * (sum + root[a]));
+    // cf^2 - ca^2 = 1/2 (x + root), x = a^2 + ct^2 - ca^2 (root^2 = x^2 + 4 ca^2 ct^2); rationalised where x < 0
+    xx[a] = a2 + ct2 - ca2;
+    gg[a] = R(2) * ca2 * ct2;                 // numerator of the rationalised form
+  }
+  {
+    R i0, i1;
+    frcp2(xx[0] < R(0) ? root[0] - xx[0] : R(1), xx[1] < R(0) ? root[1] - xx[1] : R(1), i0, i1);
+    gg[0] = xx[0] < R(0) ? gg[0] * i0 : R(0.5) * (xx[0] + root[0]);
+    gg[1] = xx[1] < R(0) ? gg[1] * i1 : R(0.5) * (xx[1] + root[1]);
+  }
   const R uL = wl[1], uR = wr[1];
-  const bool lmax = L.cf >= Rr.cf;
-  const R cmax = lmax ? L.cf : Rr.cf;
+  const bool lmax = cf[0] >= cf[1];
+  const R cmax = lmax ? cf[0] : cf[1];
   const R SL = Num<R>::min(uL, uR) - cmax, SR = Num<R>::max(uL, uR) + cmax;
   const R sL = (SL - uL) * wl[0], sR = (SR - uR) * wr[0];
   const R idn = frcp(sR - sL);
@@ -123,36 +186,39 @@ __device__ __forceinline__ void riemann_hlld(const R (&wl)[7], const R (&wr)[7],
   const R dp = (wr[4] - wl[4]) + R(0.5) * ((wr[5] - wl[5]) * (wr[5] + wl[5]) + (wr[6] - wl[6]) * (wr[6] + wl[6]));
   const R uLmSM = (sR * du + dp) * idn, uRmSM = (sL * du + dp) * idn;     // u_alpha - S_M
   const R SM = uL - uLmSM;
-  const R pTs = (sR * L.pT - sL * Rr.pT + sL * sR * (uR - uL)) * idn;
+  const R pTs = (sR * pT[0] - sL * pT[1] + sL * sR * (uR - uL)) * idn;
   const R tiny = R(1e-12) * pTs;
   // rho (S-u)^2 - Bn^2 of each side without cancellation: (S-u)^2 = (cmax + delta)^2, cmax^2 = ca_m^2 + g_m
   const R delta = Num<R>::max(du, R(0));
-  const R gm = lmax ? L.g : Rr.g, rhom = lmax ? wl[0] : wr[0];
+  const R gm = lmax ? gg[0] : gg[1], rhom = lmax ? wl[0] : wr[0], irm = lmax ? irL : irR;
   const R grow = gm + delta * (R(2) * cmax + delta);
+  const R bfac = bn2 * irm;
 
   // star states of both sides (the double-star state needs both)
-  R rs[2], v1s[2], v2s[2], b1s[2], b2s[2], es[2], vBs[2], sq[2];
+  const R dSML = (SL - uL) + uLmSM, dSMR = (SR - uR) + uRmSM;               // S_alpha - S_M
+  const R NbL = wl[0] * grow + bfac * (wl[0] - rhom), NbR = wr[0] * grow + bfac * (wr[0] - rhom);   // rho (S-u)^2 - Bn^2
+  const R DL = NbL + sL * uLmSM, DR = NbR + sR * uRmSM;                     // rho (S-u)(S-S_M) - Bn^2
+  const bool degL = Num<R>::abs(DL) < tiny, degR = Num<R>::abs(DR) < tiny;
+  R idSML, idSMR, iDL, iDR;
+  frcp4(dSML, dSMR, degL ? R(1) : DL, degR ? R(1) : DR, idSML, idSMR, iDL, iDR);
+  R rs[2], v1s[2], v2s[2], b1s[2], b2s[2], es[2], vBs[2], sq[2], isq[2];
 #pragma unroll
   for (int a = 0; a < 2; ++a) {
     const R (&w)[7] = a ? wr : wl;
-    const Side<R>& s = a ? Rr : L;
     const R Sa = a ? SR : SL, sa = a ? sR : sL, umSM = a ? uRmSM : uLmSM;
-    const R dSM = (Sa - w[1]) + umSM, idSM = frcp(dSM);      // S_alpha - S_M
+    const R idSM = a ? idSMR : idSML, iD = a ? iDR : iDL, Nb = a ? NbR : NbL;
+    const bool degen = a ? degR : degL;
     rs[a] = sa * idSM;
-    const R Nb = w[0] * grow + fdiv(bn2 * (w[0] - rhom), rhom);     // rho (S-u)^2 - Bn^2
-    const R D = Nb + sa * umSM;                                // rho (S-u)(S-S_M) - Bn^2
-    const bool degen = Num<R>::abs(D) < tiny;
-    const R iD = frcp(D);
     const R fv = degen ? R(0) : -bn * umSM * iD;
     const R fb = degen ? R(1) : Nb * iD;
     v1s[a] = w[2] - w[5] * fv; v2s[a] = w[3] - w[6] * fv;
     b1s[a] = w[5] * fb; b2s[a] = w[6] * fb;
     vBs[a] = bn * SM + b1s[a] * v1s[a] + b2s[a] * v2s[a];
-    es[a] = ((Sa - w[1]) * s.U[4] - s.pT * w[1] + pTs * SM + bn * (s.vB - vBs[a])) * idSM;
-    sq[a] = Num<R>::sqrt(rs[a]);
+    es[a] = ((Sa - w[1]) * en[a] - pT[a] * w[1] + pTs * SM + bn * (vB[a] - vBs[a])) * idSM;
+    sqrt_and_inverse(rs[a], sq[a], isq[a]);
   }
   const R abn = Num<R>::abs(bn);
-  const R SsL = SM - fdiv(abn, sq[0]), SsR = SM + fdiv(abn, sq[1]);
+  const R SsL = SM - abn * isq[0], SsR = SM + abn * isq[1];
 
   // which side of the contact the face lies on, and in which region of that side
   const bool left = (SL >= R(0)) || (SsL >= R(0)) || (SM >= R(0));
@@ -181,12 +247,20 @@ __device__ __forceinline__ void riemann_hlld(const R (&wl)[7], const R (&wr)[7],
     Uss[4] = esa + pm * sq_a * (vBa - vBss) * sg;
     Uss[5] = b1; Uss[6] = b2;
   }
+  // conserved state and physical flux (Eq. 5, 7) of the chosen side only
+  R wa[7];
+#pragma unroll
+  for (int c = 0; c < 7; ++c) wa[c] = left ? wl[c] : wr[c];
+  const R pTa = left ? pT[0] : pT[1], vBa0 = left ? vB[0] : vB[1], ena = left ? en[0] : en[1];
+  const R mn = wa[0] * wa[1];
+  const R Ua[7] = { wa[0], mn, wa[0] * wa[2], wa[0] * wa[3], ena, wa[5], wa[6] };
+  const R Fa[7] = { mn, mn * wa[1] + pTa - bn2, mn * wa[2] - bn * wa[5], mn * wa[3] - bn * wa[6],
+                    (ena + pTa) * wa[1] - bn * vBa0, wa[5] * wa[1] - bn * wa[2], wa[6] * wa[1] - bn * wa[3] };
 #pragma unroll
   for (int c = 0; c < 7; ++c) {
-    const R Fa = left ? L.F[c] : Rr.F[c], Ua = left ? L.U[c] : Rr.U[c];
-    const R f_star = Fa + Sa * (Us[c] - Ua);
-    const R f_dstar = Fa + Ssa * Uss[c] - (Ssa - Sa) * Us[c] - Sa * Ua;
-    F[c] = outer ? Fa : (star ? f_star : f_dstar);
+    const R f_star = Fa[c] + Sa * (Us[c] - Ua[c]);
+    const R f_dstar = Fa[c] + Ssa * Uss[c] - (Ssa - Sa) * Us[c] - Sa * Ua[c];
+    F[c] = outer ? Fa[c] : (star ? f_star : f_dstar);
   }
 }
 
