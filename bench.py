@@ -38,7 +38,7 @@ NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scheme", default="vl", choices=["vl", "ctu"])
@@ -68,7 +68,7 @@ def faces_per_group(g, scheme):
 class ClockSampler(threading.Thread):
     """SM clock + throttle reasons sampled through NVML while the timed region runs."""
 
-    def __init__(self, index, period=0.05):
+    def __init__(self, index, period=0.004):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.reasons, self.stop_flag, self.max_mhz = [], set(), False, None
@@ -109,6 +109,14 @@ class ClockSampler(threading.Thread):
                 "samples": len(s)}
 
 
+def hbm_peak():
+    """measured copy bandwidth of this pool's B200s (driver-written MEASURED_PEAKS.json), else the guide's fallback"""
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
 def make_batch(G, g, npdt):
     """config-2 batch: a pool of 16 distinct seeded groups tiled to G (the kernels' work does not depend on values)."""
     import numpy as np
@@ -123,7 +131,7 @@ def measure(args, prec_name, rank, world, dist):
     """Time K steps of (mhd_advance + mhd_dt_reduce) on device-resident data, then the per-stage profile, then e2e."""
     import numpy as np
     import torch
-    from paper_1804_03479_b200 import mhd
+    from paper_1804_03479_b200 import mhd, shard
     sp = scheme_params(args)
     g, G = sp["g"], args.groups
     prec = mhd.FP32 if prec_name == "f32" else mhd.FP64
@@ -164,10 +172,7 @@ def measure(args, prec_name, rank, world, dist):
     clocks = sampler.result()
     ms = e0.elapsed_time(e1)
     launches = solver.launch_count() - l0
-    if dist is not None:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = shard.max_over_ranks(ms, dist, dev)          # job time = slowest rank's device time
     cells = G * N_PS2 ** 3 * args.steps * world
     res = dict(value=cells / (ms * 1e-3), ms_per_step=ms / args.steps, launches=launches, clocks=clocks)
 
@@ -204,7 +209,9 @@ def measure(args, prec_name, rank, world, dist):
     bytes_step = (sz["n_U_in"] + sz["n_B_in"] + sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]
                   + sz["n_U_out"] + sz["n_B_out"]) * esz * G
     res.update(stages=stages, roofline=roof, profiled_ms_per_step=prof_ms / args.steps,
-               hbm={"algorithmic_GB_per_step": bytes_step / 1e9, "achieved_GBs": bytes_step / 1e9 / (res["ms_per_step"] * 1e-3)})
+               hbm={"algorithmic_GB_per_step": bytes_step / 1e9, "achieved_GBs": bytes_step / 1e9 / (res["ms_per_step"] * 1e-3),
+                    "peak_GBs": hbm_peak()[0], "peak_source": hbm_peak()[1],
+                    "frac": bytes_step / 1e9 / (res["ms_per_step"] * 1e-3) / hbm_peak()[0]})
 
     # end to end through mhd_advance_host: pinned host buffers, H2D + kernels + D2H inside the timed region
     pin = lambda a: torch.from_numpy(a).pin_memory()
@@ -219,10 +226,7 @@ def measure(args, prec_name, rank, world, dist):
         solver.advance_host(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], G, dt0, dh, chunk, 3)
     torch.cuda.synchronize()
     te = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([te], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        te = float(t.item())
+    te = shard.max_over_ranks(te, dist, dev)
     h2d = (sz["n_U_in"] + sz["n_B_in"]) * esz * G
     d2h = (sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]) * esz * G
     res["e2e"] = {"value": cells / te, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
