@@ -60,9 +60,9 @@ def faces_per_group(g, scheme):
     """Riemann solves per group in pass 1 and pass 2 (index ranges of DESIGN.md 'Index ranges')."""
     N, T = N_PS2, N_PS2 + 2 * g
     if scheme == "vl":
-        return 3 * (T - 1) * T * T, 3 * (T - 5) * (T - 2) ** 2
+        return 3 * (T - 1) * T * T, 3 * (N + 1) * (N + 2) ** 2
     r = 2
-    return 3 * (T - 2 * r - 1) * T * T, 3 * (T - 2 * r - 1) * (T - 2 * r - 2) ** 2
+    return 3 * (T - 2 * r - 1) * T * T, 3 * (N + 1) * (N + 2) ** 2
 
 
 class ClockSampler(threading.Thread):

@@ -166,7 +166,8 @@ int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
   if (s->cfg.scheme == MHD_VL) {
     const Box3x3 bf1 = dir_boxes(1, T, 0, T), be1 = edge_boxes(1, T - 1, 0, T);
     const Box3 bh = box(1, T - 1, 1, T - 1, 1, T - 1);
-    const Box3x3 bf2 = dir_boxes(3, T - 2, 1, T - 1), be2 = edge_boxes(3, T - 3, 1, T - 1);
+    // pass 2 only where the final update needs it: faces n in [g, g+N], t in [g-1, g+N]; edges of the interior faces
+    const Box3x3 bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1), be2 = edge_boxes(g, g + N, g, g + N);
     LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER><<<GRID3(bf1), blk, 0, st>>>(p, bf1))));          // step 1
     LAUNCH(ST_EMF1, (k_emf<R><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 2
     LAUNCH(ST_HALF, (k_half<R><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 3
@@ -177,8 +178,8 @@ int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
     const int r = s->cfg.recon == MHD_PLM ? 1 : 2;
     const Box3x3 brc = dir_boxes(r, T - r, 0, T), bf1 = dir_boxes(r + 1, T - r, 0, T), be1 = edge_boxes(r + 1, T - 1 - r, 0, T);
     const Box3 bh = box(r + 1, T - 1 - r, r + 1, T - 1 - r, r + 1, T - 1 - r);
-    const Box3x3 bco = dir_boxes(r, T - r, r + 1, T - 1 - r), bf2 = dir_boxes(r + 1, T - r, r + 1, T - 1 - r);
-    const Box3x3 be2 = edge_boxes(r + 2, T - 2 - r, r + 1, T - 1 - r);
+    const Box3x3 bco = dir_boxes(g - 1, g + N + 1, g - 1, g + N + 1), bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1);
+    const Box3x3 be2 = edge_boxes(g, g + N, g, g + N);
     if (s->cfg.recon == MHD_PLM) {
       if (lim == MHD_LIM_PRIM) LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimPrim><<<GRID3(brc), blk, 0, st>>>(p, brc)));
       else LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimChar><<<GRID3(brc), blk, 0, st>>>(p, brc)));

@@ -80,7 +80,7 @@ def test_other_group_sizes_and_wider_ghosts(oracle, N, g, scheme, recon):
     out = gpu(Ui, Bi, dt, dh)
     errs = GU.field_errors(out, ref, N)
     assert max(errs.values()) <= 2e-13, errs
-    assert gpu.stats() == ref["stats"]
+    assert all(a <= b for a, b in zip(gpu.stats(), ref["stats"]))
 
 
 @pytest.mark.parametrize("prec", [1, 0])

@@ -48,8 +48,9 @@ def test_one_step_every_variant(oracle, name, scheme, recon, g, riemann, limvar,
     out = gpu(U_in, B_in, dt, dh)
     assert_fields(GU.field_errors(out, ref, N), TOL_ONE_STEP[prec], f"{name} riemann={riemann} limvar={limvar}")
     if prec == 1:
-        # same floors / fallbacks fire (same index ranges on both sides)
-        assert gpu.stats() == ref["stats"]
+        # the kernels evaluate pass 2 only where the final update needs it, the oracle on its maximal index ranges:
+        # every floor / fallback event of the device is one of the oracle's
+        assert all(a <= b for a, b in zip(gpu.stats(), ref["stats"]))
 
 
 # ---------------------------------------------------------------------------------------------------------------
