@@ -119,16 +119,26 @@ __global__ void __launch_bounds__(256) k_load_prim(const KParams<R> p, const Box
   const R* Bx = p.Bin + (size_t)c.grp * p.nBi;
   const R* By = Bx + (size_t)T * T * (T + 1);
   const R* Bz = By + (size_t)T * T * (T + 1);
-  R bl[3] = { R(0), R(0), R(0) };
-  if (j < T && k < T) { bl[0] = Bx[((size_t)k * T + j) * (T + 1) + i]; c.arr(A_B + 0)[q] = bl[0]; }
-  if (i < T && k < T) { bl[1] = By[((size_t)k * (T + 1) + j) * T + i]; c.arr(A_B + 1)[q] = bl[1]; }
-  if (i < T && j < T) { bl[2] = Bz[((size_t)k * T + j) * T + i]; c.arr(A_B + 2)[q] = bl[2]; }
-  if (i >= T || j >= T || k >= T) return;
-  const R bu[3] = { Bx[((size_t)k * T + j) * (T + 1) + i + 1], By[((size_t)k * (T + 1) + j + 1) * T + i],
-                    Bz[((size_t)(k + 1) * T + j) * T + i] };
-  const R* U = p.Uin + (size_t)c.grp * p.nUi;
-  const size_t T3 = (size_t)T * T * T, cq = ((size_t)k * T + j) * T + i;
-  const R u[5] = { U[cq], U[T3 + cq], U[2 * T3 + cq], U[3 * T3 + cq], U[4 * T3 + cq] };
+  // every load is issued before the first store: the compiler cannot prove that the workspace does not alias the
+  // inputs, so a load placed after a store would wait for that store's data, i.e. for a full memory round trip
+  const bool fx = j < T && k < T, fy = i < T && k < T, fz = i < T && j < T, cell = i < T && j < T && k < T;
+  R bl[3] = { R(0), R(0), R(0) }, bu[3] = { R(0), R(0), R(0) }, u[5] = { R(1), R(0), R(0), R(0), R(1) };
+  if (fx) bl[0] = Bx[((size_t)k * T + j) * (T + 1) + i];
+  if (fy) bl[1] = By[((size_t)k * (T + 1) + j) * T + i];
+  if (fz) bl[2] = Bz[((size_t)k * T + j) * T + i];
+  if (cell) {
+    bu[0] = Bx[((size_t)k * T + j) * (T + 1) + i + 1];
+    bu[1] = By[((size_t)k * (T + 1) + j + 1) * T + i];
+    bu[2] = Bz[((size_t)(k + 1) * T + j) * T + i];
+    const R* U = p.Uin + (size_t)c.grp * p.nUi;
+    const size_t T3 = (size_t)T * T * T, cq = ((size_t)k * T + j) * T + i;
+#pragma unroll
+    for (int v = 0; v < 5; ++v) u[v] = U[v * T3 + cq];
+  }
+  if (fx) c.arr(A_B + 0)[q] = bl[0];
+  if (fy) c.arr(A_B + 1)[q] = bl[1];
+  if (fz) c.arr(A_B + 2)[q] = bl[2];
+  if (!cell) return;
   R W[8];
   cons_to_prim(p, u, bl, bu, W);
   store_prim(c, A_W, W);
@@ -161,10 +171,12 @@ __global__ void __launch_bounds__(256, OccFlux<R>::minb) k_flux1_vl(const KParam
 // upwind switch on the face mass flux m (R10).  R10a: |m| <= m0 (less than emf_tie of the cell mass crosses the face
 // in dt) counts as zero -> centred mean; between m0 and 2 m0 a linear ramp to the upwind value keeps the EMF continuous
 template <class R> __device__ __forceinline__ R upwind(R m, R m0, R qm, R qp) {
-  const R am = Num<R>::abs(m), mean = R(0.5) * (qm + qp), qu = m > R(0) ? qm : qp;
+  const R am = Num<R>::abs(m), qu = m > R(0) ? qm : qp;
+  if (am >= R(2) * m0) return qu;                      // plain upwinding: all but a vanishing fraction of the faces
+  const R mean = R(0.5) * (qm + qp);
+  if (am <= m0) return mean;
   const R w = fdiv(am - m0, m0);                       // weight of the upwind value on the ramp m0 < |m| < 2 m0
-  const R ramp = w * qu + (R(1) - w) * mean;
-  return (am <= m0) ? mean : ((am < R(2) * m0) ? ramp : qu);
+  return w * qu + (R(1) - w) * mean;
 }
 template <class R, int C>
 __device__ __forceinline__ void emf_dir(const KParams<R>& p, const Box3& box, int rhobase) {
