@@ -158,7 +158,7 @@ __device__ __forceinline__ void flux1_dir(const KParams<R>& p, const Box3& box) 
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[c.q] = F[v];
 }
 template <class R, int SOLVER>
-__global__ void __launch_bounds__(256, OccFlux<R>::minb) k_flux1_vl(const KParams<R> p, const Box3x3 bx) {
+__global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux1_vl(const KParams<R> p, const Box3x3 bx) {
   switch (blockIdx.y) {
     case 0: flux1_dir<R, SOLVER, 0>(p, bx.b[0]); break;
     case 1: flux1_dir<R, SOLVER, 1>(p, bx.b[1]); break;

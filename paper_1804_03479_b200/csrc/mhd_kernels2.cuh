@@ -28,7 +28,7 @@ __device__ __forceinline__ void flux2_vl_dir(const KParams<R>& p, const Box3& bo
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[q] = F[v];
 }
 template <class R, int SOLVER, int LIMVAR>
-__global__ void __launch_bounds__(256, OccFlux<R>::minb) k_flux2_vl(const KParams<R> p, const Box3x3 bx) {
+__global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux2_vl(const KParams<R> p, const Box3x3 bx) {
   switch (blockIdx.y) {
     case 0: flux2_vl_dir<R, SOLVER, LIMVAR, 0>(p, bx.b[0]); break;
     case 1: flux2_vl_dir<R, SOLVER, LIMVAR, 1>(p, bx.b[1]); break;
@@ -123,7 +123,7 @@ __device__ __forceinline__ void flux_lr_dir(const KParams<R>& p, const Box3& box
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[q] = F[v];
 }
 template <class R, int SOLVER>
-__global__ void __launch_bounds__(256, OccFlux<R>::minb) k_flux_lr(const KParams<R> p, const Box3x3 bx, int bbase) {
+__global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux_lr(const KParams<R> p, const Box3x3 bx, int bbase) {
   switch (blockIdx.y) {
     case 0: flux_lr_dir<R, SOLVER, 0>(p, bx.b[0], bbase); break;
     case 1: flux_lr_dir<R, SOLVER, 1>(p, bx.b[1], bbase); break;

@@ -28,7 +28,10 @@ enum : int { kHLLE = 0, kHLLD = 1, kROE = 2 };
 #define MHD_MINB64_FLUX 3
 #endif
 template <class R> struct Occ { static constexpr int minb = sizeof(R) == 8 ? MHD_MINB64 : MHD_MINB32; };          // reconstruction
-template <class R> struct OccFlux { static constexpr int minb = sizeof(R) == 8 ? MHD_MINB64_FLUX : MHD_MINB32; }; // Riemann kernels (measured: FP64 3 > 2 > 4)
+// Riemann kernels (measured: HLLD FP64 3 > 2 > 4 blocks; Roe needs ~220 FP64 / ~120 FP32 registers and must not be capped)
+template <class R, int SOLVER> struct OccFlux {
+  static constexpr int minb = SOLVER == 2 ? (sizeof(R) == 8 ? 1 : 2) : (sizeof(R) == 8 ? MHD_MINB64_FLUX : MHD_MINB32);
+};
 enum : int { kPLM = 0, kPPM = 1 };
 enum : int { kLimPrim = 0, kLimChar = 1 };
 
