@@ -321,7 +321,9 @@ int mhd_create(const mhd_config* cfg, mhd_solver** out) {
     e = cudaStreamCreateWithFlags(&s->dev[l].stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->dev[l].done, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaMalloc(&s->dev[l].ws, ws_bytes);
-    if (e == cudaSuccess) e = cudaMemset(s->dev[l].ws, 0, ws_bytes);
+    // MHD_POISON=1 fills the workspace with NaN bit patterns: a stage that read a value no earlier stage wrote would
+    // poison the output (tests/test_gpu_api.py compares a poisoned run bitwise with a normal one)
+    if (e == cudaSuccess) e = cudaMemset(s->dev[l].ws, getenv("MHD_POISON") ? 0xFF : 0, ws_bytes);
   }
   if (e != cudaSuccess) { int r = cuda_fail(e, "mhd_create allocation"); mhd_destroy(s); return r; }
   s->d_red = s->d_stats + 3;

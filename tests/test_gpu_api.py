@@ -177,3 +177,22 @@ def test_full_size_batch_on_sampled_groups(oracle, prec, scheme, recon, g):
     # invariants that hold at any size: div B of every group's output at round-off
     bx, by, bz = inputs.split_B(out["B"].astype(np.float64), N)
     assert H.rel_divb(bx, by, bz, dh) < (1e-13 if prec == 1 else 2e-5)
+
+
+@pytest.mark.parametrize("scheme,recon,g", [(0, 0, 3), (1, 0, 3), (1, 1, 4)])
+@pytest.mark.parametrize("prec", [1, 0])
+def test_no_stage_reads_an_unwritten_workspace_value(scheme, recon, g, prec, monkeypatch):
+    """NaN-poisoned workspace (MHD_POISON): outputs must be finite and bitwise equal to the normal run, for every
+    Riemann solver and both limiter variables (the oracle's NaN-initialised temporaries, on the device)."""
+    dtp = GU.np_dtype(prec)
+    U, B, dh = small_batch(3, g=g, dtype=dtp)
+    for riemann in (0, 1, 2):
+        for limvar in (0, 1):
+            kw = dict(N=16, g=g, scheme=scheme, recon=recon, riemann=riemann, limvar=limvar, prec=prec, max_groups=3)
+            ref = GU.GpuRunner(**kw)(U, B, 2e-3, dh)
+            monkeypatch.setenv("MHD_POISON", "1")
+            out = GU.GpuRunner(**kw)(U, B, 2e-3, dh)
+            monkeypatch.delenv("MHD_POISON")
+            for k in ("U", "B", "flux", "emf"):
+                assert np.isfinite(out[k]).all(), (riemann, limvar, k)
+                assert np.array_equal(out[k], ref[k]), (riemann, limvar, k)
