@@ -241,7 +241,7 @@ __device__ __forceinline__ void load_U_in(const KParams<R>& p, const Ctx<R>& c, 
 
 // ---- S4: half-step state: U^{n+1/2}, b^{n+1/2} on the faces of the cells, W^{n+1/2} -------
 template <class R>
-__global__ void __launch_bounds__(256) k_half(const KParams<R> p, const Box3 box) {
+__global__ void __launch_bounds__(256, OccMem<R>::minb) k_half(const KParams<R> p, const Box3 box) {
   Ctx<R> c(p, box);
   if (!c.ok) return;
   const R qh = (R(0.5) * p.dt) / p.dh;

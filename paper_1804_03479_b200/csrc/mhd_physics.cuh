@@ -27,6 +27,8 @@ enum : int { kHLLE = 0, kHLLD = 1, kROE = 2 };
 #ifndef MHD_MINB64_FLUX
 #define MHD_MINB64_FLUX 3
 #endif
+// latency-bound update kernels (half step, final update): measured FP32 6 blocks (40 registers) > uncapped > 8
+template <class R> struct OccMem { static constexpr int minb = sizeof(R) == 8 ? 1 : 6; };
 template <class R> struct Occ { static constexpr int minb = sizeof(R) == 8 ? MHD_MINB64 : MHD_MINB32; };          // reconstruction
 // Riemann kernels (measured: HLLD FP64 3 > 2 > 4 blocks; Roe needs ~220 FP64 / ~120 FP32 registers and must not be capped)
 template <class R, int SOLVER> struct OccFlux {
