@@ -196,3 +196,43 @@ def test_no_stage_reads_an_unwritten_workspace_value(scheme, recon, g, prec, mon
             for k in ("U", "B", "flux", "emf"):
                 assert np.isfinite(out[k]).all(), (riemann, limvar, k)
                 assert np.array_equal(out[k], ref[k]), (riemann, limvar, k)
+
+
+@pytest.mark.parametrize("which,prec", [("abc", 1), ("abc", 0), ("blast", 1)])
+def test_configs_3_4_full_size_256_cubed_on_sampled_groups(oracle, which, prec):
+    """BASELINE.json configs 3 / 4 at full size: 256^3 -> 4096 groups of 16^3 (g = 4), CTU+PPM+HLLD+CT, one step through
+    ONE mhd_advance call (several workspace slices on concurrent lanes); 24 sampled groups against the oracle (groups
+    are independent given their ghost zones), plus the invariants that hold at any size: shared faces bitwise equal,
+    div B at round-off, exact conservation on the periodic grid."""
+    n, N, g = 256, 16, 4
+    dtp = GU.np_dtype(prec)
+    if which == "abc":
+        U, bx, by, bz, dh = inputs.abc_grid(n, seed=1805, p0=0.15, vamp=1e-2)
+    else:
+        U, bx, by, bz, dh = inputs.blast_grid(n)
+    U, bx, by, bz = (a.astype(dtp) for a in (U, bx, by, bz))
+    Ui, Bi = inputs.pack_groups(U, bx, by, bz, N, g, dtp)
+    G = Ui.shape[0]
+    assert G == 4096
+    sample = list(range(7, G, 173))
+    # include groups that cut the blast sphere (centre of the grid)
+    sample += [G // 2 + 8 * 16 + 8, G // 2 - 8 * 16 - 8 - 1]
+    cfg = oracle.make_config(N=N, g=g, scheme=1, recon=1, emf_tie=(1e-12 if prec == 1 else 1e-5))
+    dt, _ = oracle.dt_reduce(cfg, Ui.astype(np.float64), Bi.astype(np.float64), g, dh, 0.3)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=1, recon=1, prec=prec, max_groups=G, planes=True)
+    dt_gpu, _ = gpu.dt(Ui, Bi, g, dh, 0.3)
+    assert abs(dt_gpu - dt) <= (1e-14 if prec == 1 else 1e-6) * dt
+    out = gpu(Ui, Bi, dt, dh)
+    ref = oracle.advance(cfg, Ui[sample].astype(np.float64), Bi[sample].astype(np.float64), dt, dh)
+    errs = GU.field_errors({k: out[k][sample] for k in out}, ref, N)
+    if prec == 0:
+        # |M|, the mass flux and the EMF (~ v B) are 1e-2 of the momentum-flux scale on this config (DESIGN.md section 9)
+        for k in ("Mx", "My", "Mz", "flux_rho", "emf"):
+            assert errs.pop(k) <= 1e-3
+    assert max(errs.values()) <= (1e-12 if prec == 1 else 1e-4), errs
+    Un, bxn, byn, bzn, mism = inputs.unpack_groups(out["U"], out["B"], n, N)
+    assert mism == 0.0
+    assert H.rel_divb(bxn.astype(np.float64), byn.astype(np.float64), bzn.astype(np.float64), dh) < (1e-13 if prec == 1 else 2e-5)
+    t0, t1 = H.totals(U), H.totals(Un)
+    tol = 1e-13 if prec == 1 else 2e-6
+    assert abs(t1[0] - t0[0]) / t0[0] < tol and abs(t1[4] - t0[4]) / t0[4] < tol
