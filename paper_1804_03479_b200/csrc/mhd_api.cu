@@ -175,16 +175,20 @@ int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
     else LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, kLimChar><<<GRID3(bf2), blk, 0, st>>>(p, bf2))));   // steps 4+5
     LAUNCH(ST_EMF2, (k_emf<R><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 6
   } else {
-    const int r = s->cfg.recon == MHD_PLM ? 1 : 2;
-    const Box3x3 brc = dir_boxes(r, T - r, 0, T), bf1 = dir_boxes(r + 1, T - r, 0, T), be1 = edge_boxes(r + 1, T - 1 - r, 0, T);
-    const Box3 bh = box(r + 1, T - 1 - r, r + 1, T - 1 - r, r + 1, T - 1 - r);
+    // everything is derived from the cells whose half-step state the second pass needs, [lo, hi)^3 = interior + 1:
+    // pass-1 fluxes on their faces and on the faces their edge EMFs touch, face states one cell further, PPM slopes
+    // one more (the oracle evaluates these stages on the whole tile; what it computes outside is never used)
+    const int lo = g - 1, hi = g + N + 1;
+    const Box3x3 brc = dir_boxes(lo - 1, hi + 1, lo - 1, hi + 1), bf1 = dir_boxes(lo, hi + 1, lo - 1, hi + 1);
+    const Box3x3 be1 = edge_boxes(lo, hi, lo, hi);
+    const Box3 bh = box(lo, hi, lo, hi, lo, hi);
     const Box3x3 bco = dir_boxes(g - 1, g + N + 1, g - 1, g + N + 1), bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1);
     const Box3x3 be2 = edge_boxes(g, g + N, g, g + N);
     if (s->cfg.recon == MHD_PLM) {
       if (lim == MHD_LIM_PRIM) LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimPrim><<<GRID3(brc), blk, 0, st>>>(p, brc)));
       else LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimChar><<<GRID3(brc), blk, 0, st>>>(p, brc)));
     } else {
-      const Box3x3 bsl = dir_boxes(1, T - 1, 0, T);
+      const Box3x3 bsl = dir_boxes(lo - 2, hi + 2, lo - 1, hi + 1);
       if (lim == MHD_LIM_PRIM) {
         LAUNCH(ST_RECON, (k_slope_ctu<R, kLimPrim><<<GRID3(bsl), blk, 0, st>>>(p, bsl)));
         LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, kLimPrim><<<GRID3(brc), blk, 0, st>>>(p, brc)));
@@ -196,7 +200,7 @@ int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
     LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<GRID3(bf1), blk, 0, st>>>(p, bf1, A_B))));      // step 2
     LAUNCH(ST_EMF1, (k_emf<R><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 3
     LAUNCH(ST_HALF, (k_half<R><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 4
-    LAUNCH(ST_CORR, (k_ctu_corr<R><<<GRID3(bco), blk, 0, st>>>(p, bco, r + 1, T - 1 - r)));                    // step 5
+    LAUNCH(ST_CORR, (k_ctu_corr<R><<<GRID3(bco), blk, 0, st>>>(p, bco, lo, hi)));                    // step 5
     LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<GRID3(bf2), blk, 0, st>>>(p, bf2, A_BH))));     // step 6
     LAUNCH(ST_EMF2, (k_emf<R><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 7
   }
