@@ -28,43 +28,43 @@ __device__ __forceinline__ void limited_slope(const R (&w0)[7], R bn, R gam, con
     for (int v = 0; v < 7; ++v) dw[v] = lim_mc(dl[v], dr[v]);
     return;
   }
+  // The eigenvectors of SURVEY A1 are sparse and come in +/- pairs: the projections are written through the
+  // components of the differences along and across beta = B_t/|B_t| (tv, tb / pv, pb), the pair sums and differences.
   const R rho = w0[0], irho = frcp(rho);
   const R a2 = gam * w0[4] * irho, a = Num<R>::sqrt(a2), srho = Num<R>::sqrt(rho), isrho = frcp(srho);
   const WaveSet<R> w = wave_set(a2, rho, bn, w0[5], w0[6]);
   const R Qf = w.cf * w.af * w.S, Qs = w.cs * w.as * w.S, Af = a * w.af * srho, As = a * w.as * srho;
   const R nn = fdiv(R(0.5), a2);
+  R am[7];   // limited amplitudes in the wave order -f, -A, -s, entropy, +s, +A, +f
+  {
+    R amp[2][7];
 #pragma unroll
-  for (int v = 0; v < 7; ++v) dw[v] = R(0);
-#pragma unroll
-  for (int k = 0; k < 7; ++k) {
-    const R s = (k < 3) ? R(1) : R(-1);
-    R Lk[7], Rk[7];
-    if (k == 0 || k == 6) {
-      Lk[0] = R(0); Lk[1] = -s * nn * w.cf * w.af; Lk[2] = s * nn * Qs * w.b1; Lk[3] = s * nn * Qs * w.b2;
-      Lk[4] = nn * w.af * irho; Lk[5] = nn * As * w.b1 * irho; Lk[6] = nn * As * w.b2 * irho;
-      Rk[0] = rho * w.af; Rk[1] = -s * w.cf * w.af; Rk[2] = s * Qs * w.b1; Rk[3] = s * Qs * w.b2;
-      Rk[4] = rho * a2 * w.af; Rk[5] = As * w.b1; Rk[6] = As * w.b2;
-    } else if (k == 1 || k == 5) {
-      Lk[0] = R(0); Lk[1] = R(0); Lk[2] = -s * R(0.5) * w.b2; Lk[3] = s * R(0.5) * w.b1; Lk[4] = R(0);
-      Lk[5] = -R(0.5) * w.b2 * w.S * isrho; Lk[6] = R(0.5) * w.b1 * w.S * isrho;
-      Rk[0] = R(0); Rk[1] = R(0); Rk[2] = -s * w.b2; Rk[3] = s * w.b1; Rk[4] = R(0);
-      Rk[5] = -w.b2 * w.S * srho; Rk[6] = w.b1 * w.S * srho;
-    } else if (k == 2 || k == 4) {
-      Lk[0] = R(0); Lk[1] = -s * nn * w.cs * w.as; Lk[2] = -s * nn * Qf * w.b1; Lk[3] = -s * nn * Qf * w.b2;
-      Lk[4] = nn * w.as * irho; Lk[5] = -nn * Af * w.b1 * irho; Lk[6] = -nn * Af * w.b2 * irho;
-      Rk[0] = rho * w.as; Rk[1] = -s * w.cs * w.as; Rk[2] = -s * Qf * w.b1; Rk[3] = -s * Qf * w.b2;
-      Rk[4] = rho * a2 * w.as; Rk[5] = -Af * w.b1; Rk[6] = -Af * w.b2;
-    } else {
-      Lk[0] = R(1); Lk[1] = R(0); Lk[2] = R(0); Lk[3] = R(0); Lk[4] = -R(2) * nn; Lk[5] = R(0); Lk[6] = R(0);
-      Rk[0] = R(1); Rk[1] = R(0); Rk[2] = R(0); Rk[3] = R(0); Rk[4] = R(0); Rk[5] = R(0); Rk[6] = R(0);
+    for (int side = 0; side < 2; ++side) {
+      const R (&d)[7] = side ? dr : dl;
+      const R tv = w.b1 * d[2] + w.b2 * d[3], pv = w.b1 * d[3] - w.b2 * d[2];
+      const R tb = w.b1 * d[5] + w.b2 * d[6], pb = w.b1 * d[6] - w.b2 * d[5];
+      const R Pf = nn * irho * (w.af * d[4] + As * tb), Vf = nn * (w.cf * w.af * d[1] - Qs * tv);
+      const R Ps = nn * irho * (w.as * d[4] - Af * tb), Vs = nn * (w.cs * w.as * d[1] + Qf * tv);
+      const R Pa = R(0.5) * w.S * isrho * pb, Va = R(0.5) * pv;
+      amp[side][0] = Pf - Vf; amp[side][6] = Pf + Vf;
+      amp[side][2] = Ps - Vs; amp[side][4] = Ps + Vs;
+      amp[side][1] = Pa + Va; amp[side][5] = Pa - Va;
+      amp[side][3] = d[0] - R(2) * nn * d[4];
     }
-    R al = R(0), ar = R(0);
 #pragma unroll
-    for (int v = 0; v < 7; ++v) { al += Lk[v] * dl[v]; ar += Lk[v] * dr[v]; }
-    const R am = lim_mc(al, ar);
-#pragma unroll
-    for (int v = 0; v < 7; ++v) dw[v] += am * Rk[v];
+    for (int k = 0; k < 7; ++k) am[k] = lim_mc(amp[0][k], amp[1][k]);
   }
+  const R Fs = am[0] + am[6], Fd = am[0] - am[6], Ss = am[2] + am[4], Sd = am[2] - am[4];
+  const R Asum = am[1] + am[5], Adif = am[1] - am[5];
+  const R comp = w.af * Fs + w.as * Ss;                  // compressive part: density and pressure
+  const R tv = Qs * Fd - Qf * Sd, tb = As * Fs - Af * Ss, pb = w.S * srho * Asum;
+  dw[0] = rho * comp + am[3];
+  dw[1] = -(w.cf * w.af * Fd + w.cs * w.as * Sd);
+  dw[2] = w.b1 * tv - w.b2 * Adif;
+  dw[3] = w.b2 * tv + w.b1 * Adif;
+  dw[4] = rho * a2 * comp;
+  dw[5] = w.b1 * tb - w.b2 * pb;
+  dw[6] = w.b2 * tb + w.b1 * pb;
 }
 
 template <class R, int LIMVAR>
