@@ -102,6 +102,23 @@ int mhd_get_stats(mhd_solver* s, unsigned long long* n_floor_dens, unsigned long
 /* Number of kernel launches issued by this solver since creation (bench.py's gpu_launches). */
 unsigned long long mhd_launch_count(const mhd_solver* s);
 
+/* ---- device-side preparation and closing steps for a uniform PERIODIC grid ----
+ * Grid arrays (DEVICE pointers, solver precision, x fastest): U[5][nz][ny][nx], bx[nz][ny][nx+1], by[nz][ny+1][nx],
+ * bz[nz+1][ny][nx]; the last face of each direction duplicates the first.  nx, ny, nz are multiples of ps2 and >= nghost;
+ * the grid is cut into (nx/ps2)(ny/ps2)(nz/ps2) <= max_groups patch groups, group index (gz*my + gy)*mx + gx.
+ * mhd_grid_pack fills U_in / B_in (layouts of mhd_advance) with periodic ghost zones; mhd_grid_unpack stores U_out / B_out
+ * back (every cell owns its three lower faces; the duplicate last faces are rewritten).  mhd_grid_advance = pack ->
+ * mhd_advance -> unpack in place on the grid through solver-owned staging buffers (allocated on first use; asynchronous
+ * on cuda_stream afterwards).  mhd_grid_dt is mhd_dt_reduce on the grid layout (synchronises cuda_stream). */
+int mhd_grid_pack(mhd_solver* s, const void* U, const void* bx, const void* by, const void* bz, int nx, int ny, int nz,
+                  void* U_in, void* B_in, void* cuda_stream);
+int mhd_grid_unpack(mhd_solver* s, const void* U_out, const void* B_out, int nx, int ny, int nz, void* U, void* bx, void* by,
+                    void* bz, void* cuda_stream);
+int mhd_grid_advance(mhd_solver* s, void* U, void* bx, void* by, void* bz, int nx, int ny, int nz, double dt, double dh,
+                     void* cuda_stream);
+int mhd_grid_dt(mhd_solver* s, const void* U, const void* bx, const void* by, const void* bz, int nx, int ny, int nz, double dh,
+                double cfl, double* dt_out, double* maxspeed_out, void* cuda_stream);
+
 /* Per-stage device timing for the roofline report: when on, every stage launch is bracketed by CUDA events on its
  * stream (up to 16384 launches since the last mhd_set_profiling call; later ones are not recorded).
  * mhd_get_profile synchronises the device, fills the summed milliseconds and launch counts of each stage

@@ -11,6 +11,7 @@
 
 #include "../../include/mhd.h"
 #include "mhd_kernels3.cuh"
+#include "mhd_grid.cuh"
 
 using namespace mhd;
 
@@ -64,6 +65,9 @@ struct mhd_solver {
   std::vector<cudaEvent_t> prof_ev;         // 2 per recorded launch
   std::vector<int> prof_stage;              // stage id per recorded launch
   size_t prof_used = 0;
+  // staging buffers of mhd_grid_advance (ghost-zoned groups of the whole grid), allocated on first use
+  void *gUi = nullptr, *gBi = nullptr, *gUo = nullptr, *gBo = nullptr;
+  int grid_groups = 0;
 };
 
 namespace {
@@ -347,6 +351,7 @@ int mhd_destroy(mhd_solver* s) {
     cudaFree(s->dev[l].ws);
   }
   if (s->fork) cudaEventDestroy(s->fork);
+  cudaFree(s->gUi); cudaFree(s->gBi); cudaFree(s->gUo); cudaFree(s->gBo);
   cudaFree(s->d_stats);
   delete s;
   return MHD_OK;
@@ -374,3 +379,4 @@ int mhd_advance(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, 
 }  // extern "C"
 
 #include "mhd_api_host.inl"
+#include "mhd_api_grid.inl"

@@ -20,7 +20,7 @@ LIM_PRIM, LIM_CHAR = 0, 1
 OK, EINVAL, ECUDA, ENOMEM = 0, -1, -2, -3
 
 EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance_host", "mhd_dt_reduce",
-           "mhd_get_stats", "mhd_launch_count", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
+           "mhd_get_stats", "mhd_launch_count", "mhd_grid_pack", "mhd_grid_unpack", "mhd_grid_advance", "mhd_grid_dt", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
            "mhd_measure_fma_peak", "mhd_strerror"]
 
 
@@ -59,6 +59,11 @@ def lib():
         L.mhd_get_stats.argtypes = [vp, ull, ull, ull]
         L.mhd_launch_count.argtypes = [vp]
         L.mhd_launch_count.restype = C.c_ulonglong
+        L.mhd_grid_pack.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, vp, vp, vp]
+        L.mhd_grid_unpack.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, vp, vp]
+        L.mhd_grid_advance.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, vp]
+        L.mhd_grid_dt.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
+                                  C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
         L.mhd_set_profiling.argtypes = [vp, C.c_int]
         L.mhd_get_profile.argtypes = [vp, C.POINTER(C.c_double), ull, C.c_int]
         L.mhd_profile_stage_name.argtypes = [C.c_int]
@@ -160,6 +165,29 @@ class Solver:
         dt, sm = C.c_double(), C.c_double()
         _check(lib().mhd_dt_reduce(self._h, _ptr(U), _ptr(B), int(ngroups), int(nghost_of_arrays), float(dh),
                                    float(cfl), C.byref(dt), C.byref(sm), _stream_ptr(stream)))
+        return dt.value, sm.value
+
+    # ---- uniform periodic grid resident on the device (NEXT-1): grid = (U, bx, by, bz) device tensors, shape = (nz, ny, nx)
+    def grid_pack(self, U, bx, by, bz, shape, U_in, B_in, stream=None):
+        nz, ny, nx = shape
+        _check(lib().mhd_grid_pack(self._h, _ptr(U), _ptr(bx), _ptr(by), _ptr(bz), nx, ny, nz, _ptr(U_in), _ptr(B_in),
+                                   _stream_ptr(stream)))
+
+    def grid_unpack(self, U_out, B_out, shape, U, bx, by, bz, stream=None):
+        nz, ny, nx = shape
+        _check(lib().mhd_grid_unpack(self._h, _ptr(U_out), _ptr(B_out), nx, ny, nz, _ptr(U), _ptr(bx), _ptr(by), _ptr(bz),
+                                     _stream_ptr(stream)))
+
+    def grid_advance(self, U, bx, by, bz, shape, dt, dh, stream=None):
+        nz, ny, nx = shape
+        _check(lib().mhd_grid_advance(self._h, _ptr(U), _ptr(bx), _ptr(by), _ptr(bz), nx, ny, nz, float(dt), float(dh),
+                                      _stream_ptr(stream)))
+
+    def grid_dt(self, U, bx, by, bz, shape, dh, cfl, stream=None):
+        nz, ny, nx = shape
+        dt, sm = C.c_double(), C.c_double()
+        _check(lib().mhd_grid_dt(self._h, _ptr(U), _ptr(bx), _ptr(by), _ptr(bz), nx, ny, nz, float(dh), float(cfl),
+                                 C.byref(dt), C.byref(sm), _stream_ptr(stream)))
         return dt.value, sm.value
 
     def get_stats(self):
