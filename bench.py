@@ -46,6 +46,8 @@ def parse():
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"], help="precision of the headline value")
     ap.add_argument("--groups", type=int, default=NGROUPS)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--grid", type=int, default=0, help="instead of the batch: a periodic n^3 ABC grid (BASELINE config 3 "
+                    "state) kept on the device; step = mhd_grid_dt + mhd_grid_advance (pack + scheme + unpack)")
     return ap.parse_args()
 
 
@@ -237,6 +239,46 @@ def measure(args, prec_name, rank, world, dist):
     return res
 
 
+def measure_grid(args, prec_name):
+    """Uniform periodic grid resident on the device (NEXT-1): K steps of mhd_grid_dt + mhd_grid_advance."""
+    import numpy as np
+    import torch
+    from paper_1804_03479_b200 import inputs, mhd
+    sp = scheme_params(args)
+    n, g = args.grid, sp["g"]
+    prec = mhd.FP32 if prec_name == "f32" else mhd.FP64
+    npdt = np.float32 if prec_name == "f32" else np.float64
+    riem = {"hlle": mhd.HLLE, "hlld": mhd.HLLD, "roe": mhd.ROE}[args.riemann]
+    G = (n // N_PS2) ** 3
+    solver = mhd.Solver(mhd.make_config(N=N_PS2, g=g, scheme=sp["scheme"], recon=sp["recon"], riemann=riem, prec=prec, max_groups=G))
+    U, bx, by, bz, dh = inputs.abc_grid(n, seed=1805, p0=0.15, vamp=1e-2)
+    grid = [torch.from_numpy(np.ascontiguousarray(a, dtype=npdt)).cuda() for a in (U, bx, by, bz)]
+    shape = (n, n, n)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        dt, _ = solver.grid_dt(*grid, shape, dh, 0.3, stream)
+        solver.grid_advance(*grid, shape, dt, dh, stream)
+
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(torch.cuda.current_device())
+    l0 = solver.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    sampler.start()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    res = dict(value=n ** 3 * args.steps / (ms * 1e-3), ms_per_step=ms / args.steps, launches=solver.launch_count() - l0,
+               clocks=sampler.result(), stats=solver.get_stats(), dtype=prec_name)
+    solver.destroy()
+    return res
+
+
 def cpu_baseline(args, groups, reps=None, target_seconds=12.0):
     """The oracle, as it stands, on the host cores: `reps` passes (default: as many as fill ~target_seconds of CPU
     work) over `groups` groups of the workload, one pass = advance + dt; value from the mean pass time."""
@@ -313,6 +355,17 @@ def main():
         import torch.distributed as dist_mod
         dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
         dist = dist_mod
+    if args.grid:
+        a, b = measure_grid(args, args.prec), measure_grid(args, "f64" if args.prec == "f32" else "f32")
+        config.update(workload="BASELINE.json config 3 state: periodic %d^3 ABC grid (beta 0.1) resident on the device, cut "
+                               "into %d patch groups of 16^3 every step, %s+%s+CT" % (args.grid, (args.grid // N_PS2) ** 3, sp_name, args.riemann.upper()),
+                      step="mhd_grid_dt + mhd_grid_advance (device-side pack, S0-S8, unpack)", groups_per_rank=(args.grid // N_PS2) ** 3)
+        print(json.dumps({"metric": "cell-updates/sec", "value": a["value"], "unit": "cell-updates/s", "n_gpus": 1,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": a["ms_per_step"], "higher_is_better": True,
+                          "scaling": "weak", "vs_baseline": None, "dtype": a["dtype"], "data": "synthetic", "config": config,
+                          "clocks": a["clocks"], "gpu_launches": a["launches"], "stats": a["stats"],
+                          ("fp64" if b["dtype"] == "f64" else "fp32"): b}))
+        return 0
     main_prec = args.prec
     other = "f64" if main_prec == "f32" else "f32"
     r_main = measure(args, main_prec, rank, world, dist)
