@@ -32,6 +32,12 @@ PAPER_P100 = {"f32": 1.2e8, "f64": 5.5e7}       # PAPER.md:12, :465-467 (Tesla P
 # algorithmic work per Riemann solve and per group, DESIGN.md "Roofline arithmetic"
 FLOP_PER_SOLVE = {"hlld": 371, "roe": 915, "hlle": 297}   # add/mul/div/sqrt = 1 each, as the oracle states the solver
 FLOP_PLM_PER_FACE = 140     # two MC-limited primitive slopes + the two face states (VL pass 2)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage kernel at 512 groups, VL+PLM+HLLD, from the
+# ncu --set full captures summarised in profiles/r01_full_top_kernels.md / r01_full_top_kernels_f64.md (MB)
+NCU_TRAFFIC_MB = {"f32": {"load_prim": 569.4, "flux_pass1": 862.9, "emf_pass1": 380.8, "half_step": 888.4, "flux_pass2": 644.2,
+                          "emf_pass2": 242.5, "final_update": 431.0, "dt_reduce": 69.2},
+                  "f64": {"load_prim": 1063.3, "flux_pass1": 1598.1, "emf_pass1": 737.8, "half_step": 1666.0, "flux_pass2": 1078.6,
+                          "emf_pass2": 451.5, "final_update": 848.8, "dt_reduce": 140.8}}
 NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
 
 
@@ -203,13 +209,20 @@ def measure(args, prec_name, rank, world, dist):
         peak = NOMINAL_TFLOPS[prec_name]
         roof = {"bound": "alu", "kernel": top, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
                 "peak_source": "nominal: 148 SMs x %d FMA lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if prec_name == "f32" else 64),
-                "peak_fma_measured": mhd.measure_fma_peak(dev.index, prec), "traffic": None,
+                "peak_fma_measured": mhd.measure_fma_peak(dev.index, prec),
+                "traffic": (NCU_TRAFFIC_MB[prec_name].get(top) * 1e6 if (args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS) else None),
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_*)",
                 "avg_launch_ms": dur * 1e3, "launches_per_step": n_launch,
                 "share_of_step": stages[top]["ms_per_step"] / (prof_ms / args.steps)}
     # HBM view of the whole step: algorithmic bytes = read the ghost-zoned tile once, write the results once (+ dt read)
     sz = solver.sizes()
     bytes_step = (sz["n_U_in"] + sz["n_B_in"] + sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]
                   + sz["n_U_out"] + sz["n_B_out"]) * esz * G
+    if args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS:
+        tot = sum(NCU_TRAFFIC_MB[prec_name].values()) * 1e6
+        res["dram_traffic"] = {"bytes_per_step_ncu": tot, "GBs": tot / 1e9 / (res["ms_per_step"] * 1e-3),
+                               "frac_of_hbm_peak": tot / 1e9 / (res["ms_per_step"] * 1e-3) / hbm_peak()[0],
+                               "note": "all stage kernels of one step; the intermediates between stages go through HBM"}
     res.update(stages=stages, roofline=roof, profiled_ms_per_step=prof_ms / args.steps,
                hbm={"algorithmic_GB_per_step": bytes_step / 1e9, "achieved_GBs": bytes_step / 1e9 / (res["ms_per_step"] * 1e-3),
                     "peak_GBs": hbm_peak()[0], "peak_source": hbm_peak()[1],
@@ -386,7 +399,7 @@ def main():
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": r_main["ms_per_step"], "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": main_prec, "data": "synthetic", "config": config,
                 "clocks": r_main["clocks"], "e2e": r_main["e2e"], "gpu_launches": r_main["launches"],
-                "roofline": r_main["roofline"], "cpu_baseline": cb,
+                "roofline": r_main["roofline"], "cpu_baseline": cb, "dram_traffic": r_main.get("dram_traffic"),
                 "hbm": r_main["hbm"], "stages_ms_per_step": {k: round(v["ms_per_step"], 4) for k, v in r_main["stages"].items()},
                 "profiled_ms_per_step": r_main["profiled_ms_per_step"],
                 "paper_p100_context": {"value": PAPER_P100[main_prec], "note": "Tesla P100, VL+PLM+Roe, PAPER.md:12,:465 -- context, not a target"},

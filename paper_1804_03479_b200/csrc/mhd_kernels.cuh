@@ -196,7 +196,7 @@ __device__ __forceinline__ void emf_dir(const KParams<R>& p, const Box3& box, in
   c.arr(A_E + C)[q] = e;
 }
 template <class R>
-__global__ void __launch_bounds__(256) k_emf(const KParams<R> p, const Box3x3 bx, int rhobase) {
+__global__ void __launch_bounds__(256, OccEmf<R>::minb) k_emf(const KParams<R> p, const Box3x3 bx, int rhobase) {
   switch (blockIdx.y) {
     case 0: emf_dir<R, 0>(p, bx.b[0], rhobase); break;
     case 1: emf_dir<R, 1>(p, bx.b[1], rhobase); break;
@@ -241,7 +241,7 @@ __device__ __forceinline__ void load_U_in(const KParams<R>& p, const Ctx<R>& c, 
 
 // ---- S4: half-step state: U^{n+1/2}, b^{n+1/2} on the faces of the cells, W^{n+1/2} -------
 template <class R>
-__global__ void __launch_bounds__(256, OccMem<R>::minb) k_half(const KParams<R> p, const Box3 box) {
+__global__ void __launch_bounds__(256, OccHalf<R>::minb) k_half(const KParams<R> p, const Box3 box) {
   Ctx<R> c(p, box);
   if (!c.ok) return;
   const R qh = (R(0.5) * p.dt) / p.dh;

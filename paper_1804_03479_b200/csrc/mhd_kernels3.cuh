@@ -35,7 +35,7 @@ __device__ __forceinline__ void copy_planes(const KParams<R>& p, int grp, int t)
 }
 
 template <class R>
-__global__ void __launch_bounds__(256, OccMem<R>::minb) k_final(const KParams<R> p, const Box3 box) {
+__global__ void __launch_bounds__(256, OccFinal<R>::minb) k_final(const KParams<R> p, const Box3 box) {
   Ctx<R> c(p, box);
   if (p.fout || p.eout) copy_planes(p, blockIdx.z, blockIdx.x * blockDim.x + threadIdx.x);
   if (!c.ok) return;

@@ -27,8 +27,11 @@ enum : int { kHLLE = 0, kHLLD = 1, kROE = 2 };
 #ifndef MHD_MINB64_FLUX
 #define MHD_MINB64_FLUX 3
 #endif
-// latency-bound update kernels (half step, final update): measured FP32 6 blocks (40 registers) > uncapped > 8
-template <class R> struct OccMem { static constexpr int minb = sizeof(R) == 8 ? 1 : 6; };
+// latency-bound update kernels: resident 256-thread blocks per SM requested from ptxas, from sweeps on B200
+// (uncapped, ptxas hoists every load of the FP64 half-step kernel into 158 registers: 11 % of the warps resident)
+template <class R> struct OccHalf  { static constexpr int minb = sizeof(R) == 8 ? 2 : 6; };
+template <class R> struct OccFinal { static constexpr int minb = sizeof(R) == 8 ? 4 : 6; };
+template <class R> struct OccEmf   { static constexpr int minb = sizeof(R) == 8 ? 5 : 1; };
 template <class R> struct Occ { static constexpr int minb = sizeof(R) == 8 ? MHD_MINB64 : MHD_MINB32; };          // reconstruction
 // Riemann kernels (measured: HLLD FP64 3 > 2 > 4 blocks; Roe needs ~220 FP64 / ~120 FP32 registers and must not be capped)
 template <class R, int SOLVER> struct OccFlux {
