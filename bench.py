@@ -30,7 +30,9 @@ sys.path.insert(0, ROOT)
 N_PS2, NGROUPS = 16, 512
 PAPER_P100 = {"f32": 1.2e8, "f64": 5.5e7}       # PAPER.md:12, :465-467 (Tesla P100, VL+PLM+Roe) -- context only
 # algorithmic work per Riemann solve and per group, DESIGN.md "Roofline arithmetic"
-FLOP_PER_SOLVE = {"hlld": 371, "roe": 915, "hlle": 297}   # add/mul/div/sqrt = 1 each, as the oracle states the solver
+# exact operation counts of the oracle instantiated with a counting scalar (oracle/count_ops.cpp; add/sub/mul/div/sqrt = 1)
+FLOP_PER_SOLVE = {"hlld": 381, "roe": 1107, "hlle": 361}
+FLOP_PER_CELL_UPDATE = {("vl", "hlld"): 6263.5, ("vl", "roe"): 15289.0, ("ctu", "hlld"): 26067.6, ("ctu", "roe"): 35160.4}   # whole step
 FLOP_PLM_PER_FACE = 140     # two MC-limited primitive slopes + the two face states (VL pass 2)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage kernel at 512 groups, VL+PLM+HLLD, from the
 # ncu --set full captures summarised in profiles/r01_full_top_kernels.md / r01_full_top_kernels_f64.md (MB)
@@ -223,6 +225,11 @@ def measure(args, prec_name, rank, world, dist):
         res["dram_traffic"] = {"bytes_per_step_ncu": tot, "GBs": tot / 1e9 / (res["ms_per_step"] * 1e-3),
                                "frac_of_hbm_peak": tot / 1e9 / (res["ms_per_step"] * 1e-3) / hbm_peak()[0],
                                "note": "all stage kernels of one step; the intermediates between stages go through HBM"}
+    fpc = FLOP_PER_CELL_UPDATE.get((args.scheme, args.riemann))
+    if fpc:
+        tf = fpc * res["value"] / world / 1e12
+        res["alu_whole_step"] = {"flops_per_cell_update": fpc, "achieved_TFLOPs": tf, "frac_of_nominal_peak": tf / NOMINAL_TFLOPS[prec_name],
+                                 "note": "oracle's exact operation count on its maximal index ranges (oracle/count_ops.cpp) x measured cell-updates/s"}
     res.update(stages=stages, roofline=roof, profiled_ms_per_step=prof_ms / args.steps,
                hbm={"algorithmic_GB_per_step": bytes_step / 1e9, "achieved_GBs": bytes_step / 1e9 / (res["ms_per_step"] * 1e-3),
                     "peak_GBs": hbm_peak()[0], "peak_source": hbm_peak()[1],
@@ -399,7 +406,7 @@ def main():
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": r_main["ms_per_step"], "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": main_prec, "data": "synthetic", "config": config,
                 "clocks": r_main["clocks"], "e2e": r_main["e2e"], "gpu_launches": r_main["launches"],
-                "roofline": r_main["roofline"], "cpu_baseline": cb, "dram_traffic": r_main.get("dram_traffic"),
+                "roofline": r_main["roofline"], "cpu_baseline": cb, "dram_traffic": r_main.get("dram_traffic"), "alu_whole_step": r_main.get("alu_whole_step"),
                 "hbm": r_main["hbm"], "stages_ms_per_step": {k: round(v["ms_per_step"], 4) for k, v in r_main["stages"].items()},
                 "profiled_ms_per_step": r_main["profiled_ms_per_step"],
                 "paper_p100_context": {"value": PAPER_P100[main_prec], "note": "Tesla P100, VL+PLM+Roe, PAPER.md:12,:465 -- context, not a target"},
