@@ -119,6 +119,25 @@ int mhd_grid_advance(mhd_solver* s, void* U, void* bx, void* by, void* bz, int n
 int mhd_grid_dt(mhd_solver* s, const void* U, const void* bx, const void* by, const void* bz, int nx, int ny, int nz, double dh,
                 double cfl, double* dt_out, double* maxspeed_out, void* cuda_stream);
 
+/* ---- the AMR correction operation on a static two-level mesh ----
+ * Coarse level: a periodic grid in the layout of mhd_grid_* (DEVICE pointers) cut into patch groups in grid order; fine
+ * level: the patch groups (cell size dh_c / 2) covering ONE refined box of coarse cells lo[d] .. hi[d]-1, ordered z
+ * outermost, x fastest.  lo, hi: HOST int[3], multiples of ps2/2, ps2/2 <= lo < hi <= n - ps2/2.
+ * mhd_amr_restrict: coarse cells of the box <- volume average of 8 fine cells (U_out of the fine groups), coarse faces of
+ * the box including its surface <- area average of 4 fine faces (B_out).
+ * mhd_amr_fixup: every leaf coarse cell sharing a face with the box gets  U += -/+ (dt/dh_c) (w_f <F_fine> - w_c F_coarse)
+ * (upper / lower face of the cell), <F_fine> the mean of the 4 fine fluxes of that face; every leaf coarse face touching an
+ * edge of the box surface gets the Eq. 13 update of the jump  w_f <E_fine> - w_c E_coarse  of that edge.  flux_c / emf_c:
+ * flux_out / emf_out of ALL coarse groups of the step being corrected; flux_f / emf_f: those of the fine groups.  With
+ * both levels advanced by the same dt, w_c = w_f = 1; with sub-cycling call once per fine step with w_f = 1/nsub and
+ * w_c = 1 on the first call, 0 afterwards.  Call the fix-up BEFORE the restriction is irrelevant: they touch disjoint data.
+ * Asynchronous on cuda_stream.  MHD_EINVAL for a misaligned box. */
+int mhd_amr_restrict(mhd_solver* s, const void* U_f, const void* B_f, const int* lo, const int* hi, void* Uc, void* bxc,
+                     void* byc, void* bzc, int nx, int ny, int nz, void* cuda_stream);
+int mhd_amr_fixup(mhd_solver* s, const void* flux_c, const void* emf_c, const void* flux_f, const void* emf_f, const int* lo,
+                  const int* hi, double dt, double dh_c, double w_c, double w_f, void* Uc, void* bxc, void* byc, void* bzc,
+                  int nx, int ny, int nz, void* cuda_stream);
+
 /* Per-stage device timing for the roofline report: when on, every stage launch is bracketed by CUDA events on its
  * stream (up to 16384 launches since the last mhd_set_profiling call; later ones are not recorded).
  * mhd_get_profile synchronises the device, fills the summed milliseconds and launch counts of each stage

@@ -12,6 +12,7 @@
 #include "../../include/mhd.h"
 #include "mhd_kernels3.cuh"
 #include "mhd_grid.cuh"
+#include "mhd_amr.cuh"
 
 using namespace mhd;
 
@@ -380,3 +381,4 @@ int mhd_advance(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, 
 
 #include "mhd_api_host.inl"
 #include "mhd_api_grid.inl"
+#include "mhd_api_amr.inl"

@@ -20,7 +20,7 @@ LIM_PRIM, LIM_CHAR = 0, 1
 OK, EINVAL, ECUDA, ENOMEM = 0, -1, -2, -3
 
 EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance_host", "mhd_dt_reduce",
-           "mhd_get_stats", "mhd_launch_count", "mhd_grid_pack", "mhd_grid_unpack", "mhd_grid_advance", "mhd_grid_dt", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
+           "mhd_get_stats", "mhd_launch_count", "mhd_grid_pack", "mhd_grid_unpack", "mhd_grid_advance", "mhd_grid_dt", "mhd_amr_restrict", "mhd_amr_fixup", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
            "mhd_measure_fma_peak", "mhd_strerror"]
 
 
@@ -64,6 +64,10 @@ def lib():
         L.mhd_grid_advance.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, vp]
         L.mhd_grid_dt.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
                                   C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
+        ip = C.POINTER(C.c_int)
+        L.mhd_amr_restrict.argtypes = [vp, vp, vp, ip, ip, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, vp]
+        L.mhd_amr_fixup.argtypes = [vp, vp, vp, vp, vp, ip, ip, C.c_double, C.c_double, C.c_double, C.c_double, vp, vp, vp, vp,
+                                    C.c_int, C.c_int, C.c_int, vp]
         L.mhd_set_profiling.argtypes = [vp, C.c_int]
         L.mhd_get_profile.argtypes = [vp, C.POINTER(C.c_double), ull, C.c_int]
         L.mhd_profile_stage_name.argtypes = [C.c_int]
@@ -189,6 +193,18 @@ class Solver:
         _check(lib().mhd_grid_dt(self._h, _ptr(U), _ptr(bx), _ptr(by), _ptr(bz), nx, ny, nz, float(dh), float(cfl),
                                  C.byref(dt), C.byref(sm), _stream_ptr(stream)))
         return dt.value, sm.value
+
+    # ---- AMR correction operation on a static two-level mesh (NEXT-2); lo, hi: (x, y, z) coarse cell indices of the box
+    def amr_restrict(self, U_f, B_f, lo, hi, U, bx, by, bz, shape, stream=None):
+        nz, ny, nx = shape
+        _check(lib().mhd_amr_restrict(self._h, _ptr(U_f), _ptr(B_f), (C.c_int * 3)(*lo), (C.c_int * 3)(*hi), _ptr(U), _ptr(bx),
+                                      _ptr(by), _ptr(bz), nx, ny, nz, _stream_ptr(stream)))
+
+    def amr_fixup(self, flux_c, emf_c, flux_f, emf_f, lo, hi, dt, dh_c, U, bx, by, bz, shape, w_c=1.0, w_f=1.0, stream=None):
+        nz, ny, nx = shape
+        _check(lib().mhd_amr_fixup(self._h, _ptr(flux_c), _ptr(emf_c), _ptr(flux_f), _ptr(emf_f), (C.c_int * 3)(*lo),
+                                   (C.c_int * 3)(*hi), float(dt), float(dh_c), float(w_c), float(w_f), _ptr(U), _ptr(bx), _ptr(by),
+                                   _ptr(bz), nx, ny, nz, _stream_ptr(stream)))
 
     def get_stats(self):
         a, b, c = C.c_ulonglong(), C.c_ulonglong(), C.c_ulonglong()
