@@ -202,3 +202,173 @@ def inject(Uc, bxc, byc, bzc):
         sl[axis] = slice(1, None, 2); out[tuple(sl)] = 0.5 * (f[tuple(lo_)] + f[tuple(hi_)])
         return out
     return U, up(bxc, 2), up(byc, 1), up(bzc, 0)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# NEXT-3: creating new fine grids: conservative interpolation of the conserved variables and the
+# divergence-free interpolation of Balsara (2001) for the face field, written as the paper words it and generalised
+# from its 2-D example (Eq. 17, 10 coefficients) to 3-D (21 coefficients).  Readings: MC-limited
+# slopes (the limiter of the solver); periodic coarse neighbours; the refined box is surrounded by coarse
+# cells (no copy from pre-existing fine neighbours).
+#
+# Step by step for every coarse cell (unit cube, centre at the origin, x, y, z in units of the coarse cell size):
+#   first set  -- the 24 fine faces lying on the six coarse faces: piecewise-linear interpolation of the coarse face
+#                 value within the face, slopes from the neighbouring coarse faces of the same orientation;
+#   second set -- the 12 interior fine faces: the polynomial
+#                     Bx = a0 + ax x + ay y + az z + axx x^2 + axy xy + axz xz          (and cyclic for By, Bz)
+#                 whose 21 coefficients are fixed by (i) matching the linear profile on each of the six coarse faces
+#                 (18 equations, 17 independent when the coarse field is divergence-free) and (ii) div B = 0
+#                 identically (4 equations); the linear system is SOLVED NUMERICALLY here (no closed form), and the
+#                 interior fine-face values are the area averages of the polynomial (2-point Gauss, exact for degree 2).
+# ------------------------------------------------------------------------------------------------------------------
+def mc(a, b):
+    """MC limiter: 0 if ab <= 0, else sign(a+b) min(|a+b|/2, 2|a|, 2|b|)"""
+    if a * b <= 0.0:
+        return 0.0
+    return np.sign(a + b) * min(0.5 * abs(a + b), 2.0 * abs(a), 2.0 * abs(b))
+
+
+# monomials of the three components: exponents (px, py, pz) in the order of the comment above
+_MONO = (
+    ((0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), (2, 0, 0), (1, 1, 0), (1, 0, 1)),      # Bx
+    ((0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), (0, 2, 0), (1, 1, 0), (0, 1, 1)),      # By
+    ((0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), (0, 0, 2), (1, 0, 1), (0, 1, 1)),      # Bz
+)
+
+
+def _poly(coef, comp, x, y, z):
+    return sum(c * x ** p[0] * y ** p[1] * z ** p[2] for c, p in zip(coef[7 * comp:7 * comp + 7], _MONO[comp]))
+
+
+def _dmono(p, axis):
+    """d/d(axis) of the monomial with exponents p: (factor, exponents)"""
+    if p[axis] == 0:
+        return 0.0, p
+    q = list(p); q[axis] -= 1
+    return float(p[axis]), tuple(q)
+
+
+def balsara_coefficients(face_val, face_slope):
+    """face_val[d][s]: coarse face value of component d on side s (0 lower, 1 upper); face_slope[d][s][t]: its slope
+    along axis t (t != d) per coarse cell.  Returns the 21 coefficients solving the matching + divergence-free system."""
+    rows, rhs = [], []
+    for d in range(3):
+        for s in (0, 1):
+            pos = [0.0, 0.0, 0.0]; pos[d] = -0.5 if s == 0 else 0.5
+            # value at the face centre
+            r = np.zeros(21)
+            for m, p in enumerate(_MONO[d]):
+                r[7 * d + m] = pos[0] ** p[0] * pos[1] ** p[1] * pos[2] ** p[2]
+            rows.append(r); rhs.append(face_val[d][s])
+            # in-face slopes at the face centre (the profile on the face is linear in the in-face coordinates)
+            for t in range(3):
+                if t == d:
+                    continue
+                r = np.zeros(21)
+                for m, p in enumerate(_MONO[d]):
+                    f, q = _dmono(p, t)
+                    r[7 * d + m] = f * pos[0] ** q[0] * pos[1] ** q[1] * pos[2] ** q[2]
+                rows.append(r); rhs.append(face_slope[d][s][t])
+    # div B = 0 identically: the coefficient of every monomial of d(Bx)/dx + d(By)/dy + d(Bz)/dz vanishes
+    div = {}
+    for d in range(3):
+        for m, p in enumerate(_MONO[d]):
+            f, q = _dmono(p, d)
+            if f != 0.0:
+                div.setdefault(q, np.zeros(21))[7 * d + m] += f
+    for q, r in sorted(div.items()):
+        rows.append(r); rhs.append(0.0)
+    A, b = np.array(rows), np.array(rhs)
+    coef, res, rank, _ = np.linalg.lstsq(A, b, rcond=None)
+    assert rank == 21
+    return coef, float(np.abs(A @ coef - b).max())
+
+
+_GAUSS = (-0.5 / np.sqrt(3.0), 0.5 / np.sqrt(3.0))      # 2-point Gauss nodes on [-1/2, 1/2] (scaled by the interval length)
+
+
+def _face_average(coef, comp, centre, size):
+    """area average of component comp over the square fine face centred at `centre` (normal = comp), edge `size`"""
+    t1, t2 = (comp + 1) % 3, (comp + 2) % 3
+    acc = 0.0
+    for g1 in _GAUSS:
+        for g2 in _GAUSS:
+            p = list(centre); p[t1] += g1 * size; p[t2] += g2 * size
+            acc += 0.25 * _poly(coef, comp, *p)
+    return acc
+
+
+def prolong(Uc, bxc, byc, bzc, lo, hi):
+    """new fine grids covering coarse cells lo..hi-1 of a periodic coarse grid.  Returns U_f[5][2nbz][2nby][2nbx],
+    bx_f[2nbz][2nby][2nbx+1], by_f[2nbz][2nby+1][2nbx], bz_f[2nbz+1][2nby][2nbx] and the largest residual of the linear
+    systems (round-off when the coarse field is divergence-free)."""
+    nz, ny, nx = Uc.shape[1:]
+    n = (nx, ny, nz)
+    nb = [hi[d] - lo[d] for d in range(3)]
+    b = (bxc, byc, bzc)
+
+    def face(d, pos):
+        """coarse face value of component d at lattice position pos (periodic)"""
+        q = [pos[a] % n[a] for a in range(3)]
+        return b[d][q[2], q[1], q[0]]
+
+    def slope(d, pos, t):
+        up = list(pos); up[t] += 1
+        dn = list(pos); dn[t] -= 1
+        c = face(d, pos)
+        return mc(face(d, up) - c, c - face(d, dn))
+
+    U_f = np.empty((5, 2 * nb[2], 2 * nb[1], 2 * nb[0]))
+    out = [np.full((2 * nb[2], 2 * nb[1], 2 * nb[0] + 1), np.nan), np.full((2 * nb[2], 2 * nb[1] + 1, 2 * nb[0]), np.nan),
+           np.full((2 * nb[2] + 1, 2 * nb[1], 2 * nb[0]), np.nan)]
+    worst = 0.0
+    for k in range(nb[2]):
+        for j in range(nb[1]):
+            for i in range(nb[0]):
+                cell = (lo[0] + i, lo[1] + j, lo[2] + k)
+                rel = (i, j, k)
+                # ---- conserved variables: conservative piecewise-linear interpolation ----
+                for v in range(5):
+                    c = Uc[v, cell[2], cell[1], cell[0]]
+                    s = []
+                    for t in range(3):
+                        up = list(cell); up[t] = (up[t] + 1) % n[t]
+                        dn = list(cell); dn[t] = (dn[t] - 1) % n[t]
+                        s.append(mc(Uc[v, up[2], up[1], up[0]] - c, c - Uc[v, dn[2], dn[1], dn[0]]))
+                    for dz in (0, 1):
+                        for dy in (0, 1):
+                            for dx in (0, 1):
+                                U_f[v, 2 * k + dz, 2 * j + dy, 2 * i + dx] = c + (dx - 0.5) * 0.5 * s[0] + (dy - 0.5) * 0.5 * s[1] + (dz - 0.5) * 0.5 * s[2]
+                # ---- face field ----
+                fv = [[0.0, 0.0] for _ in range(3)]
+                fs = [[[0.0] * 3, [0.0] * 3] for _ in range(3)]
+                for d in range(3):
+                    t1, t2 = (d + 1) % 3, (d + 2) % 3
+                    for s_ in (0, 1):
+                        pos = list(cell); pos[d] += s_
+                        fv[d][s_] = face(d, pos)
+                        fs[d][s_][t1] = slope(d, pos, t1)
+                        fs[d][s_][t2] = slope(d, pos, t2)
+                        # first set: the four fine faces on this coarse face
+                        for o2 in (0, 1):
+                            for o1 in (0, 1):
+                                val = fv[d][s_] + (o1 - 0.5) * 0.5 * fs[d][s_][t1] + (o2 - 0.5) * 0.5 * fs[d][s_][t2]
+                                idx = [0, 0, 0]
+                                idx[d] = 2 * rel[d] + 2 * s_
+                                idx[t1] = 2 * rel[t1] + o1
+                                idx[t2] = 2 * rel[t2] + o2
+                                out[d][idx[2], idx[1], idx[0]] = val
+                coef, res = balsara_coefficients(fv, fs)
+                worst = max(worst, res)
+                # second set: the four interior fine faces per direction (normal coordinate 0)
+                for d in range(3):
+                    t1, t2 = (d + 1) % 3, (d + 2) % 3
+                    for o2 in (0, 1):
+                        for o1 in (0, 1):
+                            centre = [0.0, 0.0, 0.0]; centre[t1] = (o1 - 0.5) * 0.5; centre[t2] = (o2 - 0.5) * 0.5
+                            idx = [0, 0, 0]
+                            idx[d] = 2 * rel[d] + 1
+                            idx[t1] = 2 * rel[t1] + o1
+                            idx[t2] = 2 * rel[t2] + o2
+                            out[d][idx[2], idx[1], idx[0]] = _face_average(coef, d, centre, 0.5)
+    return U_f, out[0], out[1], out[2], worst
