@@ -138,6 +138,19 @@ int mhd_amr_fixup(mhd_solver* s, const void* flux_c, const void* emf_c, const vo
                   const int* hi, double dt, double dh_c, double w_c, double w_f, void* Uc, void* bxc, void* byc, void* bzc,
                   int nx, int ny, int nz, void* cuda_stream);
 
+/* ---- creating new fine grids ----
+ * Coarse level: a periodic grid in the layout of mhd_grid_* (DEVICE pointers, solver precision).  The box of coarse cells
+ * lo[d] .. hi[d]-1 (HOST int[3], 0 <= lo < hi <= n) is refined by 2: U_f[5][2nbz][2nby][2nbx] <- conservative
+ * piecewise-linear interpolation with MC-limited slopes (the mean of the 8 fine cells is the coarse cell); bx_f[2nbz][2nby]
+ * [2nbx+1], by_f[2nbz][2nby+1][2nbx], bz_f[2nbz+1][2nby][2nbx] <- Balsara (2001) divergence-free interpolation: fine faces
+ * on a coarse face from the MC-limited linear profile of that face (their mean is the coarse value), interior fine faces
+ * from the polynomial of Eq. 17 carried to 3-D (21 coefficients fixed by the interface and divergence conditions,
+ * PAPER.md:213-219), so that the fine field is divergence-free to round-off when the coarse one is.  Coarse neighbours
+ * are periodic; every coarse face of the box is interpolated (no copy from pre-existing fine neighbours: the box is
+ * taken to be surrounded by coarse cells).  nb[d] = hi[d] - lo[d].  Asynchronous on cuda_stream.  MHD_EINVAL for a bad box. */
+int mhd_amr_prolong(mhd_solver* s, const void* Uc, const void* bxc, const void* byc, const void* bzc, int nx, int ny, int nz,
+                    const int* lo, const int* hi, void* U_f, void* bx_f, void* by_f, void* bz_f, void* cuda_stream);
+
 /* Per-stage device timing for the roofline report: when on, every stage launch is bracketed by CUDA events on its
  * stream (up to 16384 launches since the last mhd_set_profiling call; later ones are not recorded).
  * mhd_get_profile synchronises the device, fills the summed milliseconds and launch counts of each stage

@@ -13,6 +13,7 @@
 #include "mhd_kernels3.cuh"
 #include "mhd_grid.cuh"
 #include "mhd_amr.cuh"
+#include "mhd_prolong.cuh"
 
 using namespace mhd;
 

@@ -74,4 +74,31 @@ int mhd_amr_fixup(mhd_solver* s, const void* flux_c, const void* emf_c, const vo
   return MHD_OK;
 }
 
+int mhd_amr_prolong(mhd_solver* s, const void* Uc, const void* bxc, const void* byc, const void* bzc, int nx, int ny, int nz,
+                    const int* lo, const int* hi, void* U_f, void* bx_f, void* by_f, void* bz_f, void* cuda_stream) {
+  if (!s || !Uc || !bxc || !byc || !bzc || !U_f || !bx_f || !by_f || !bz_f || !lo || !hi) return MHD_EINVAL;
+  const int n[3] = { nx, ny, nz };
+  ProlongGeom g;
+  long long npts = 1;
+  for (int d = 0; d < 3; ++d) {
+    if (n[d] < 2 || lo[d] < 0 || lo[d] >= hi[d] || hi[d] > n[d]) return MHD_EINVAL;
+    g.n.set(d, n[d]); g.lo.set(d, lo[d]); g.hi.set(d, hi[d]);
+    npts *= hi[d] - lo[d] + 1;
+  }
+  CU(cudaSetDevice(s->cfg.device));
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const dim3 grid((unsigned)((npts + 127) / 128)), blk(128);
+  if (s->cfg.prec == MHD_FP32)
+    k_amr_prolong<float><<<grid, blk, 0, st>>>(static_cast<const float*>(Uc), static_cast<const float*>(bxc), static_cast<const float*>(byc),
+                                               static_cast<const float*>(bzc), g, static_cast<float*>(U_f), static_cast<float*>(bx_f),
+                                               static_cast<float*>(by_f), static_cast<float*>(bz_f));
+  else
+    k_amr_prolong<double><<<grid, blk, 0, st>>>(static_cast<const double*>(Uc), static_cast<const double*>(bxc), static_cast<const double*>(byc),
+                                                static_cast<const double*>(bzc), g, static_cast<double*>(U_f), static_cast<double*>(bx_f),
+                                                static_cast<double*>(by_f), static_cast<double*>(bz_f));
+  s->launches++;
+  CU(cudaGetLastError());
+  return MHD_OK;
+}
+
 }  // extern "C"

@@ -20,7 +20,7 @@ LIM_PRIM, LIM_CHAR = 0, 1
 OK, EINVAL, ECUDA, ENOMEM = 0, -1, -2, -3
 
 EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance_host", "mhd_dt_reduce",
-           "mhd_get_stats", "mhd_launch_count", "mhd_grid_pack", "mhd_grid_unpack", "mhd_grid_advance", "mhd_grid_dt", "mhd_amr_restrict", "mhd_amr_fixup", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
+           "mhd_get_stats", "mhd_launch_count", "mhd_grid_pack", "mhd_grid_unpack", "mhd_grid_advance", "mhd_grid_dt", "mhd_amr_restrict", "mhd_amr_fixup", "mhd_amr_prolong", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
            "mhd_measure_fma_peak", "mhd_strerror"]
 
 
@@ -68,6 +68,7 @@ def lib():
         L.mhd_amr_restrict.argtypes = [vp, vp, vp, ip, ip, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, vp]
         L.mhd_amr_fixup.argtypes = [vp, vp, vp, vp, vp, ip, ip, C.c_double, C.c_double, C.c_double, C.c_double, vp, vp, vp, vp,
                                     C.c_int, C.c_int, C.c_int, vp]
+        L.mhd_amr_prolong.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, ip, ip, vp, vp, vp, vp, vp]
         L.mhd_set_profiling.argtypes = [vp, C.c_int]
         L.mhd_get_profile.argtypes = [vp, C.POINTER(C.c_double), ull, C.c_int]
         L.mhd_profile_stage_name.argtypes = [C.c_int]
@@ -205,6 +206,11 @@ class Solver:
         _check(lib().mhd_amr_fixup(self._h, _ptr(flux_c), _ptr(emf_c), _ptr(flux_f), _ptr(emf_f), (C.c_int * 3)(*lo),
                                    (C.c_int * 3)(*hi), float(dt), float(dh_c), float(w_c), float(w_f), _ptr(U), _ptr(bx), _ptr(by),
                                    _ptr(bz), nx, ny, nz, _stream_ptr(stream)))
+
+    def amr_prolong(self, U, bx, by, bz, shape, lo, hi, U_f, bx_f, by_f, bz_f, stream=None):
+        nz, ny, nx = shape
+        _check(lib().mhd_amr_prolong(self._h, _ptr(U), _ptr(bx), _ptr(by), _ptr(bz), nx, ny, nz, (C.c_int * 3)(*lo),
+                                     (C.c_int * 3)(*hi), _ptr(U_f), _ptr(bx_f), _ptr(by_f), _ptr(bz_f), _stream_ptr(stream)))
 
     def get_stats(self):
         a, b, c = C.c_ulonglong(), C.c_ulonglong(), C.c_ulonglong()

@@ -90,3 +90,64 @@ def test_two_level_step_on_the_device_conserves_and_stays_divergence_free(scheme
     tot1 = A.composite_totals(grid[0], out_f["U"], lo, hi, N, dh)
     assert np.all(np.abs(tot1 - tot0) / scale < 1e-13), (tot1 - tot0) / scale
     assert H.rel_divb(grid[1], grid[2], grid[3], dh) < 1e-13
+
+
+@pytest.mark.parametrize("prec", [1, 0])
+@pytest.mark.parametrize("lo,hi", [((2, 3, 4), (8, 7, 10)), ((0, 0, 0), (16, 16, 16)), ((13, 0, 5), (16, 2, 6))])
+def test_device_prolongation_matches_the_oracle(prec, lo, hi):
+    """NEXT-3: new fine grids on the device (closed-form coefficients) against oracle/amr_ref.prolong
+    (numerical solve of the interface + divergence conditions), element by element; the box may touch the periodic rim"""
+    n = 16
+    dtp = GU.np_dtype(prec)
+    U, bx, by, bz, dh = inputs.random_group_grid(n, 4)
+    coarse = [np.ascontiguousarray(a, dtype=dtp) for a in (U, bx, by, bz)]
+    ref = amr_ref.prolong(*[a.astype(np.float64) for a in coarse], lo, hi)
+    assert ref[4] < 1e-12 if prec == 1 else True        # FP32-rounded coarse faces are divergence-free to 1e-7 only
+    gpu = GU.GpuRunner(N=16, g=3, prec=prec, max_groups=1)
+    t = gpu.torch
+    out = [t.full(a.shape, float("nan"), dtype=t.float64 if prec == 1 else t.float32, device="cuda") for a in ref[:4]]
+    gpu.solver.amr_prolong(*[t.from_numpy(a).cuda() for a in coarse], (n, n, n), lo, hi, *out)
+    t.cuda.synchronize()
+    out = [o.cpu().numpy().astype(np.float64) for o in out]
+    tol = 1e-13 if prec == 1 else 2e-6
+    for a, b in zip(out, ref[:4]):
+        assert not np.isnan(a).any()
+        assert np.abs(a - b).max() <= tol * np.abs(b).max()
+    div = (out[1][:, :, 1:] - out[1][:, :, :-1]) + (out[2][:, 1:, :] - out[2][:, :-1, :]) + (out[3][1:] - out[3][:-1])
+    assert np.abs(div).max() < (1e-13 if prec == 1 else 2e-5) * np.abs(bx).max() * n
+    with pytest.raises(gpu.mhd.MHDError):
+        gpu.solver.amr_prolong(*[t.from_numpy(a).cuda() for a in coarse], (n, n, n), (0, 0, 0), (17, 4, 4), *out)
+
+
+def test_prolongation_then_restriction_returns_the_coarse_data():
+    """the two AMR operators are consistent: restricting freshly prolonged data gives back the coarse cells and faces"""
+    n, N = 32, 16
+    lo, hi = (8, 8, 8), (24, 16, 24)
+    U, bx, by, bz, dh = inputs.random_group_grid(n, 9)
+    gpu = GU.GpuRunner(N=N, g=3, prec=1, max_groups=8)
+    t = gpu.torch
+    nb = [hi[d] - lo[d] for d in range(3)]
+    shapes = [(5, 2 * nb[2], 2 * nb[1], 2 * nb[0]), (2 * nb[2], 2 * nb[1], 2 * nb[0] + 1), (2 * nb[2], 2 * nb[1] + 1, 2 * nb[0]),
+              (2 * nb[2] + 1, 2 * nb[1], 2 * nb[0])]
+    fine = [t.empty(s, dtype=t.float64, device="cuda") for s in shapes]
+    dev = [t.from_numpy(a).cuda() for a in (U, bx, by, bz)]
+    gpu.solver.amr_prolong(*dev, (n, n, n), lo, hi, *fine)
+    t.cuda.synchronize()
+    Uf, bxf, byf, bzf = [f.cpu().numpy() for f in fine]
+    # cut the fine box into patch groups (z outermost, x fastest) in the U_out / B_out layout
+    mf = [2 * nb[d] // N for d in range(3)]
+    U_f, B_f = [], []
+    for gz in range(mf[2]):
+        for gy in range(mf[1]):
+            for gx in range(mf[0]):
+                sz, sy, sx = slice(gz * N, gz * N + N), slice(gy * N, gy * N + N), slice(gx * N, gx * N + N)
+                U_f.append(Uf[:, sz, sy, sx].ravel())
+                B_f.append(np.concatenate([bxf[sz, sy, gx * N:gx * N + N + 1].ravel(), byf[sz, gy * N:gy * N + N + 1, sx].ravel(),
+                                           bzf[gz * N:gz * N + N + 1, sy, sx].ravel()]))
+    scr = [t.from_numpy(np.full_like(a, 7.0)).cuda() for a in (U, bx, by, bz)]
+    gpu.solver.amr_restrict(t.from_numpy(np.array(U_f)).cuda(), t.from_numpy(np.array(B_f)).cuda(), lo, hi, *scr, (n, n, n))
+    t.cuda.synchronize()
+    box = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+    assert np.abs(scr[0].cpu().numpy()[(slice(None),) + box] - U[(slice(None),) + box]).max() < 1e-14 * np.abs(U).max()
+    assert np.abs(scr[1].cpu().numpy()[lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0] + 1] - bx[lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0] + 1]).max() < 1e-14
+    assert np.abs(scr[3].cpu().numpy()[lo[2]:hi[2] + 1, lo[1]:hi[1], lo[0]:hi[0]] - bz[lo[2]:hi[2] + 1, lo[1]:hi[1], lo[0]:hi[0]]).max() < 1e-14
