@@ -40,6 +40,7 @@ typedef struct {
   int limvar;   // 0 primitive, 1 characteristic
   double min_dens, min_pres;
   double emf_tie;  // reading R10a: width of the linear blend of the CT upwind switch, in units of (mean cell density) * dh/dt
+  int limiter;     // NEXT-4 variants: 0 MC (reading R5, the default), 1 minmod, 2 van Leer
 } mhdref_config;
 }
 
@@ -59,7 +60,13 @@ inline double mc(double a, double b) {
   double m = std::min(0.5 * std::fabs(s), std::min(2.0 * std::fabs(a), 2.0 * std::fabs(b)));
   return s > 0.0 ? m : -m;
 }
-// minmod used by the CTU MHD source terms, reading R6
+// NEXT-4 slope-limiter variants (PAPER.md:176 names none): the two other classical symmetric TVD limiters
+// van Leer (harmonic mean): 2ab/(a+b) if ab > 0, else 0
+inline double vanleer(double a, double b) {
+  if (a * b <= 0.0) return 0.0;
+  return 2.0 * a * b / (a + b);
+}
+// minmod used by the CTU MHD source terms, reading R6 (and as the minmod slope limiter, limiter = 1)
 inline double mm(double a, double b) {
   if (a * b <= 0.0) return 0.0;
   double m = std::min(std::fabs(a), std::fabs(b));
@@ -491,19 +498,45 @@ struct Group {
     for (int v = 0; v < 7; ++v) F[d][v][q] = f[v];
   }
 
+  // the slope limiter selected by the configuration (R5: MC; NEXT-4 variants: minmod, van Leer)
+  double lim(double a, double b) const { return c.limiter == 1 ? mm(a, b) : (c.limiter == 2 ? vanleer(a, b) : mc(a, b)); }
+
+  // PPM parabola of cell q in direction d (reading C4): interface values from the limited slopes of the cell and its
+  // two neighbours, monotonised (i)-(iii); returns W_l, W_r, dW = W_r - W_l, W6
+  void ppm_parabola(const Arr Wc[8], size_t q, int d, double Wl[7], double Wr[7], double dW[7], double W6[7]) const {
+    int od = off(d);
+    double sm[7], s0[7], sp[7], wm[7], w0[7], wp[7];
+    slope(Wc, q - od, d, sm); slope(Wc, q, d, s0); slope(Wc, q + od, d, sp);
+    gen(Wc, q - od, d, wm); gen(Wc, q, d, w0); gen(Wc, q + od, d, wp);
+    for (int v = 0; v < 7; ++v) {
+      Wl[v] = 0.5 * (wm[v] + w0[v]) - (s0[v] - sm[v]) / 6.0;
+      Wr[v] = 0.5 * (w0[v] + wp[v]) - (sp[v] - s0[v]) / 6.0;
+      // monotonise (C4 i-iii)
+      if ((Wr[v] - w0[v]) * (w0[v] - Wl[v]) <= 0.0) { Wl[v] = w0[v]; Wr[v] = w0[v]; }
+      double dw = Wr[v] - Wl[v], w6 = 6.0 * (w0[v] - 0.5 * (Wl[v] + Wr[v]));
+      double nl = Wl[v], nr = Wr[v];
+      if (dw * w6 > dw * dw) nl = 3.0 * w0[v] - 2.0 * Wr[v];
+      if (dw * w6 < -dw * dw) nr = 3.0 * w0[v] - 2.0 * Wl[v];
+      Wl[v] = nl; Wr[v] = nr;
+      Wl[v] = std::max(std::min(w0[v], wm[v]), std::min(std::max(w0[v], wm[v]), Wl[v]));
+      Wr[v] = std::max(std::min(w0[v], wp[v]), std::min(std::max(w0[v], wp[v]), Wr[v]));
+      dW[v] = Wr[v] - Wl[v]; W6[v] = 6.0 * (w0[v] - 0.5 * (Wl[v] + Wr[v]));
+    }
+  }
+
   // limited slope of the generic state of cell q in direction d (R4/R5): primitive or characteristic
   void slope(const Arr Wc[8], size_t q, int d, double dWm[7]) const {
     double wm[7], w0[7], wp[7], dl[7], dr[7];
     gen(Wc, q - off(d), d, wm); gen(Wc, q, d, w0); gen(Wc, q + off(d), d, wp);
     for (int v = 0; v < 7; ++v) { dl[v] = w0[v] - wm[v]; dr[v] = wp[v] - w0[v]; }
-    if (c.limvar == 0) { for (int v = 0; v < 7; ++v) dWm[v] = mc(dl[v], dr[v]); return; }
+    if (c.limvar == 0) { for (int v = 0; v < 7; ++v) dWm[v] = lim(dl[v], dr[v]); return; }
     double lam[7], R[7][7], L[7][7];
     eig_prim(w0, Wc[5 + d][q], gam, lam, R, L);
     for (int v = 0; v < 7; ++v) dWm[v] = 0.0;
     for (int k = 0; k < 7; ++k) {
       double al = 0.0, ar = 0.0;
       for (int v = 0; v < 7; ++v) { al += L[k][v] * dl[v]; ar += L[k][v] * dr[v]; }
-      double am = mc(al, ar);
+      double am = lim(al, ar);
       for (int v = 0; v < 7; ++v) dWm[v] += am * R[k][v];
     }
   }
@@ -529,21 +562,31 @@ struct Group {
     ct_update(b, bh, 0.5 * dt, 1, T - 1);
     con2prim(Uh, bh, Wh, 1, T - 1);
     for (auto& fd : F) for (auto& a : fd) a.assign(t.n3, NaN);           // pass-1 fluxes are dead from here on
-    // step 4+5: PLM in primitive/characteristic variables at the half step, no tracing; Bn = bh(face)
+    // step 4+5: PLM (or, NEXT-4 variant, the PPM parabola of C4) in primitive/characteristic variables at the half step,
+    // no tracing (the half step supplies the time centring); Bn = bh(face).  Faces whose stencil lies inside the cells
+    // that carry a half-step state: PLM cells i-2..i+1 -> faces 3..T-3; PPM cells i-3..i+2 -> faces 4..T-4
+    const int r = c.recon == 0 ? 3 : 4;
     for (int d = 0; d < 3; ++d) {
       int t1, t2; cyc(d, t1, t2);
       int idx[3];
-      for (idx[t2] = 1; idx[t2] < T - 1; ++idx[t2]) for (idx[t1] = 1; idx[t1] < T - 1; ++idx[t1]) for (idx[d] = 3; idx[d] <= T - 3; ++idx[d]) {
+      for (idx[t2] = 1; idx[t2] < T - 1; ++idx[t2]) for (idx[t1] = 1; idx[t1] < T - 1; ++idx[t1]) for (idx[d] = r; idx[d] <= T - r; ++idx[d]) {
         size_t q = t.id(idx[0], idx[1], idx[2]), ql = q - off(d);
-        double wl[7], wr[7], sl[7], sr[7];
-        gen(Wh, ql, d, wl); gen(Wh, q, d, wr);
-        slope(Wh, ql, d, sl); slope(Wh, q, d, sr);
-        for (int v = 0; v < 7; ++v) { wl[v] += 0.5 * sl[v]; wr[v] -= 0.5 * sr[v]; }
+        double wl[7], wr[7];
+        if (c.recon == 0) {
+          double sl[7], sr[7];
+          gen(Wh, ql, d, wl); gen(Wh, q, d, wr);
+          slope(Wh, ql, d, sl); slope(Wh, q, d, sr);
+          for (int v = 0; v < 7; ++v) { wl[v] += 0.5 * sl[v]; wr[v] -= 0.5 * sr[v]; }
+        } else {
+          double lo_[7], dW[7], W6[7], up_[7];
+          ppm_parabola(Wh, ql, d, lo_, wl, dW, W6);      // L state = W_r of the cell below the face
+          ppm_parabola(Wh, q, d, wr, up_, dW, W6);       // R state = W_l of the cell above it
+        }
         floors(wl); floors(wr);
         solve_face(d, q, wl, wr, bh[d][q]);
       }
     }
-    edge_emf(Wh, 3, T - 3, 1, T - 1);                                  // step 6
+    edge_emf(Wh, r, T - r, 1, T - 1);                                  // step 6
   }
 
   // ------------------------------------------------------------------------------
@@ -570,23 +613,8 @@ struct Group {
           slope(W, q, d, dWm); Ax(dWm, AdW);
           for (int v = 0; v < 7; ++v) { wup[v] = w0[v] + 0.5 * dWm[v] - 0.5 * sig * AdW[v]; wlo[v] = w0[v] - 0.5 * dWm[v] - 0.5 * sig * AdW[v]; }
         } else {
-          double sm[7], s0[7], sp[7], wm[7], wp[7], Wl[7], Wr[7], dW[7], W6[7];
-          slope(W, q - od, d, sm); slope(W, q, d, s0); slope(W, q + od, d, sp);
-          gen(W, q - od, d, wm); gen(W, q + od, d, wp);
-          for (int v = 0; v < 7; ++v) {
-            Wl[v] = 0.5 * (wm[v] + w0[v]) - (s0[v] - sm[v]) / 6.0;
-            Wr[v] = 0.5 * (w0[v] + wp[v]) - (sp[v] - s0[v]) / 6.0;
-            // monotonise (C4 i-iii)
-            if ((Wr[v] - w0[v]) * (w0[v] - Wl[v]) <= 0.0) { Wl[v] = w0[v]; Wr[v] = w0[v]; }
-            double dw = Wr[v] - Wl[v], w6 = 6.0 * (w0[v] - 0.5 * (Wl[v] + Wr[v]));
-            double nl = Wl[v], nr = Wr[v];
-            if (dw * w6 > dw * dw) nl = 3.0 * w0[v] - 2.0 * Wr[v];
-            if (dw * w6 < -dw * dw) nr = 3.0 * w0[v] - 2.0 * Wl[v];
-            Wl[v] = nl; Wr[v] = nr;
-            Wl[v] = std::max(std::min(w0[v], wm[v]), std::min(std::max(w0[v], wm[v]), Wl[v]));
-            Wr[v] = std::max(std::min(w0[v], wp[v]), std::min(std::max(w0[v], wp[v]), Wr[v]));
-            dW[v] = Wr[v] - Wl[v]; W6[v] = 6.0 * (w0[v] - 0.5 * (Wl[v] + Wr[v]));
-          }
+          double Wl[7], Wr[7], dW[7], W6[7];
+          ppm_parabola(W, q, d, Wl, Wr, dW, W6);
           double xu[7], xl[7], Au[7], Al[7], A6[7], AA6[7];
           for (int v = 0; v < 7; ++v) { xu[v] = dW[v] - W6[v]; xl[v] = dW[v] + W6[v]; }
           Ax(xu, Au); Ax(xl, Al); Ax(W6, A6); Ax(A6, AA6);
@@ -735,8 +763,7 @@ struct Group {
 
 int check_cfg(const mhdref_config* c) {
   if (!c) return -1;
-  if (c->ps2 < 2 || c->scheme < 0 || c->scheme > 1 || c->recon < 0 || c->recon > 1 || c->riemann < 0 || c->riemann > 2 || c->limvar < 0 || c->limvar > 1) return -1;
-  if (c->scheme == 0 && c->recon == 1) return -1;          // VL+PPM is a NEXT variant
+  if (c->ps2 < 2 || c->scheme < 0 || c->scheme > 1 || c->recon < 0 || c->recon > 1 || c->riemann < 0 || c->riemann > 2 || c->limvar < 0 || c->limvar > 1 || c->limiter < 0 || c->limiter > 2) return -1;
   int need = c->recon == 1 ? 4 : 3;                        // reading R8
   if (c->nghost < need) return -1;
   if (!(c->gamma > 1.0)) return -1;
@@ -822,4 +849,6 @@ int mhdref_eig_roe(const double* WL, const double* WR, double Bn, double gamma, 
   return 0;
 }
 double mhdref_mc(double a, double b) { return mc(a, b); }
+// slope limiter by index (0 MC, 1 minmod, 2 van Leer), for the limiter pins
+double mhdref_limiter(int which, double a, double b) { return which == 1 ? mm(a, b) : (which == 2 ? vanleer(a, b) : mc(a, b)); }
 }

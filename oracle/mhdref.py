@@ -19,12 +19,13 @@ VL, CTU = 0, 1
 PLM, PPM = 0, 1
 HLLE, HLLD, ROE = 0, 1, 2
 LIM_PRIM, LIM_CHAR = 0, 1
+MC, MINMOD, VANLEER = 0, 1, 2
 
 
 class Config(C.Structure):
     _fields_ = [("ps2", C.c_int), ("nghost", C.c_int), ("gamma", C.c_double), ("scheme", C.c_int),
                 ("recon", C.c_int), ("riemann", C.c_int), ("limvar", C.c_int),
-                ("min_dens", C.c_double), ("min_pres", C.c_double), ("emf_tie", C.c_double)]
+                ("min_dens", C.c_double), ("min_pres", C.c_double), ("emf_tie", C.c_double), ("limiter", C.c_int)]
 
 
 def build(force: bool = False) -> str:
@@ -55,6 +56,8 @@ def lib():
         _lib.mhdref_eig_roe.argtypes = [dp, dp, C.c_double, C.c_double, dp, dp, dp, dp]
         _lib.mhdref_mc.argtypes = [C.c_double, C.c_double]
         _lib.mhdref_mc.restype = C.c_double
+        _lib.mhdref_limiter.argtypes = [C.c_int, C.c_double, C.c_double]
+        _lib.mhdref_limiter.restype = C.c_double
     return _lib
 
 
@@ -68,11 +71,11 @@ def _c(a):
 
 
 def make_config(N=16, g=3, gamma=5.0 / 3.0, scheme=VL, recon=PLM, riemann=HLLD, limvar=None,
-                min_dens=1e-10, min_pres=1e-10, emf_tie=1e-12) -> Config:
+                min_dens=1e-10, min_pres=1e-10, emf_tie=1e-12, limiter=MC) -> Config:
     """emf_tie: reading R10a; 1e-12 is the FP64 value, the FP32 path is checked against the oracle run with 1e-5."""
     if limvar is None:
         limvar = LIM_PRIM if scheme == VL else LIM_CHAR
-    return Config(N, g, gamma, scheme, recon, riemann, limvar, min_dens, min_pres, emf_tie)
+    return Config(N, g, gamma, scheme, recon, riemann, limvar, min_dens, min_pres, emf_tie, limiter)
 
 
 def advance(cfg: Config, U_in, B_in, dt, dh, want_planes=True, force_ghost_ok=False):
@@ -139,3 +142,8 @@ def eig_roe(WL, WR, Bn, gamma=5.0 / 3.0):
 
 def mc(a, b):
     return lib().mhdref_mc(float(a), float(b))
+
+
+def limiter(which, a, b):
+    """slope limiter by index: MC, MINMOD, VANLEER"""
+    return lib().mhdref_limiter(int(which), float(a), float(b))
