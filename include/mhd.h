@@ -41,12 +41,14 @@ typedef enum { MHD_VL = 0, MHD_CTU = 1 } mhd_scheme;            /* PAPER.md:191-
 typedef enum { MHD_PLM = 0, MHD_PPM = 1 } mhd_recon;            /* PAPER.md:176, :194 */
 typedef enum { MHD_HLLE = 0, MHD_HLLD = 1, MHD_ROE = 2 } mhd_riemann; /* PAPER.md:177 */
 typedef enum { MHD_LIM_PRIM = 0, MHD_LIM_CHAR = 1 } mhd_limvar; /* limiter in primitive / characteristic variables */
+typedef enum { MHD_LIMITER_MC = 0, MHD_LIMITER_MINMOD = 1, MHD_LIMITER_VANLEER = 2 } mhd_limiter; /* slope limiter; the paper
+                                              names none (PAPER.md:176): MC is the default reading (DESIGN.md R5), the others NEXT-4 variants */
 
 typedef struct {
   int ps2;          /* N: interior cells per side of a patch group; 16 = 2 patches of 8 (PAPER.md:234, :330); even, 8..64 */
   int nghost;       /* g: >= 3 for PLM, >= 4 for PPM (DESIGN.md R8); exactly the ghost width of the arrays passed in */
   double gamma;     /* ratio of specific heats, > 1 (5/3 in every paper test, PAPER.md:250) */
-  int scheme;       /* mhd_scheme; VL+PPM is rejected */
+  int scheme;       /* mhd_scheme */
   int recon;        /* mhd_recon */
   int riemann;      /* mhd_riemann */
   int limvar;       /* mhd_limvar */
@@ -57,6 +59,7 @@ typedef struct {
                        two cells) counts as zero and takes the centred average; <= 0 selects 1e-12 (FP64) / 1e-5 (FP32) */
   int max_groups;   /* largest ngroups of one mhd_advance call (bounds nothing but argument checking) */
   int device;       /* CUDA device ordinal */
+  int limiter;      /* mhd_limiter (0 = MC) */
 } mhd_config;
 
 enum { MHD_OK = 0, MHD_EINVAL = -1, MHD_ECUDA = -2, MHD_ENOMEM = -3 };

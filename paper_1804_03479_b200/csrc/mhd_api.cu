@@ -102,6 +102,16 @@ KParams<R> make_params(const mhd_solver* s, const void* Ui, const void* Bi, void
     default:       { constexpr int SOLVER = kROE;  CALL; } break; \
   }
 
+#define LIM_SWITCH(lim, CALL)             \
+  switch (lim) {                           \
+    case 0: { constexpr int LIM = 0; CALL; } break; \
+    case 1: { constexpr int LIM = 1; CALL; } break; \
+    case 2: { constexpr int LIM = 2; CALL; } break; \
+    case 3: { constexpr int LIM = 3; CALL; } break; \
+    case 4: { constexpr int LIM = 4; CALL; } break; \
+    default: { constexpr int LIM = 5; CALL; } break; \
+  }
+
 enum Stage : int { ST_LOAD = 0, ST_RECON, ST_FLUX1, ST_EMF1, ST_HALF, ST_CORR, ST_FLUX2, ST_EMF2, ST_FINAL, ST_DT, ST_COUNT };
 const char* const kStageNames[ST_COUNT] = { "load_prim", "recon_ctu", "flux_pass1", "emf_pass1", "half_step", "ctu_corr",
                                             "flux_pass2", "emf_pass2", "final_update", "dt_reduce" };
@@ -164,7 +174,8 @@ template <class R>
 int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
   const int TPB = 256;
   const dim3 blk(TPB);
-  const int T = s->T, S = s->S, N = s->N, g = s->g, sol = s->cfg.riemann, lim = s->cfg.limvar;
+  const int T = s->T, S = s->S, N = s->N, g = s->g, sol = s->cfg.riemann;
+  const int lim = s->cfg.limvar + 2 * s->cfg.limiter;     // template parameter LIM of the slope kernels
 #define GRID1(b) dim3(blocks_for(b, TPB), 1, ng)
 #define GRID3(b) dim3(blocks_for(b, TPB), 3, ng)
   const Box3 ball = box(0, S, 0, S, 0, S);
@@ -177,8 +188,16 @@ int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
     LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER><<<GRID3(bf1), blk, 0, st>>>(p, bf1))));          // step 1
     LAUNCH(ST_EMF1, (k_emf<R><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 2
     LAUNCH(ST_HALF, (k_half<R><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 3
-    if (lim == MHD_LIM_PRIM) LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, kLimPrim><<<GRID3(bf2), blk, 0, st>>>(p, bf2))));
-    else LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, kLimChar><<<GRID3(bf2), blk, 0, st>>>(p, bf2))));   // steps 4+5
+    if (s->cfg.recon == MHD_PLM) {
+      LIM_SWITCH(lim, LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, LIM><<<GRID3(bf2), blk, 0, st>>>(p, bf2)))));   // steps 4+5
+    } else {
+      // VL + PPM (NEXT-4): limited slopes of the half-step primitives (parked in the dead pass-1 flux arrays), the
+      // monotonised parabola's interface values as L/R states, then the plain L/R Riemann kernel of CTU
+      const Box3x3 bsl = dir_boxes(g - 2, g + N + 2, g - 1, g + N + 1), brc = dir_boxes(g - 1, g + N + 1, g - 1, g + N + 1);
+      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_slope_ctu<R, LIM><<<GRID3(bsl), blk, 0, st>>>(p, bsl, A_WH))));
+      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPPMNoTrace, LIM><<<GRID3(brc), blk, 0, st>>>(p, brc, A_WH))));
+      LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<GRID3(bf2), blk, 0, st>>>(p, bf2, A_BH))));
+    }
     LAUNCH(ST_EMF2, (k_emf<R><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 6
   } else {
     // everything is derived from the cells whose half-step state the second pass needs, [lo, hi)^3 = interior + 1:
@@ -191,17 +210,11 @@ int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
     const Box3x3 bco = dir_boxes(g - 1, g + N + 1, g - 1, g + N + 1), bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1);
     const Box3x3 be2 = edge_boxes(g, g + N, g, g + N);
     if (s->cfg.recon == MHD_PLM) {
-      if (lim == MHD_LIM_PRIM) LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimPrim><<<GRID3(brc), blk, 0, st>>>(p, brc)));
-      else LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, kLimChar><<<GRID3(brc), blk, 0, st>>>(p, brc)));
+      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, LIM><<<GRID3(brc), blk, 0, st>>>(p, brc, A_W))));
     } else {
       const Box3x3 bsl = dir_boxes(lo - 2, hi + 2, lo - 1, hi + 1);
-      if (lim == MHD_LIM_PRIM) {
-        LAUNCH(ST_RECON, (k_slope_ctu<R, kLimPrim><<<GRID3(bsl), blk, 0, st>>>(p, bsl)));
-        LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, kLimPrim><<<GRID3(brc), blk, 0, st>>>(p, brc)));
-      } else {
-        LAUNCH(ST_RECON, (k_slope_ctu<R, kLimChar><<<GRID3(bsl), blk, 0, st>>>(p, bsl)));
-        LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, kLimChar><<<GRID3(brc), blk, 0, st>>>(p, brc)));
-      }
+      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_slope_ctu<R, LIM><<<GRID3(bsl), blk, 0, st>>>(p, bsl, A_W))));
+      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, LIM><<<GRID3(brc), blk, 0, st>>>(p, brc, A_W))));
     }                                                                                                          // step 1
     LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<GRID3(bf1), blk, 0, st>>>(p, bf1, A_B))));      // step 2
     LAUNCH(ST_EMF1, (k_emf<R><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 3
@@ -264,7 +277,7 @@ int check_config(const mhd_config* c) {
   if (c->riemann < MHD_HLLE || c->riemann > MHD_ROE) return MHD_EINVAL;
   if (c->limvar != MHD_LIM_PRIM && c->limvar != MHD_LIM_CHAR) return MHD_EINVAL;
   if (c->prec != MHD_FP32 && c->prec != MHD_FP64) return MHD_EINVAL;
-  if (c->scheme == MHD_VL && c->recon == MHD_PPM) return MHD_EINVAL;
+  if (c->limiter < MHD_LIMITER_MC || c->limiter > MHD_LIMITER_VANLEER) return MHD_EINVAL;
   const int need = c->recon == MHD_PPM ? 4 : 3;     // DESIGN.md R8
   if (c->nghost < need || c->nghost > 8) return MHD_EINVAL;
   if (!(c->gamma > 1.0) || !std::isfinite(c->gamma)) return MHD_EINVAL;
@@ -302,7 +315,7 @@ int mhd_create(const mhd_config* cfg, mhd_solver** out) {
   if (!(s->cfg.emf_tie > 0.0)) s->cfg.emf_tie = cfg->prec == MHD_FP32 ? 1e-5 : 1e-12;
   s->N = cfg->ps2; s->g = cfg->nghost; s->T = s->N + 2 * s->g; s->S = s->T + 1;
   s->S3 = (size_t)s->S * s->S * s->S;
-  s->narr = cfg->scheme == MHD_VL ? A_VL_END : A_CTU_END;
+  s->narr = (cfg->scheme == MHD_VL && cfg->recon == MHD_PLM) ? A_VL_END : A_CTU_END;   // face-state arrays: CTU, VL + PPM
   s->esz = cfg->prec == MHD_FP32 ? 4 : 8;
   const size_t N = s->N, T = s->T;
   s->nUi = 5 * T * T * T; s->nBi = 3 * T * T * (T + 1);

@@ -40,11 +40,11 @@ __global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux2_vl(cons
 // PPM needs the limited slope of three cells per cell: the slopes are computed once per cell and direction by
 // k_slope_ctu (parked in the flux arrays, which are free until step 2) and read back here.
 template <class R, int LIMVAR, int D>
-__device__ __forceinline__ void slope_ctu_dir(const KParams<R>& p, const Box3& box) {
+__device__ __forceinline__ void slope_ctu_dir(const KParams<R>& p, const Box3& box, int wbase) {
   Ctx<R> c(p, box);
   if (!c.ok) return;
   const int o = c.off(D), q = c.q, S3 = p.S3;
-  const R* W = c.arr(A_W);
+  const R* W = c.arr(wbase);
   R wm[7], w0[7], wp[7], dw[7];
   load_gen<R, D>(W, S3, q - o, wm);
   load_gen<R, D>(W, S3, q, w0);
@@ -54,21 +54,21 @@ __device__ __forceinline__ void slope_ctu_dir(const KParams<R>& p, const Box3& b
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[q] = dw[v];
 }
 template <class R, int LIMVAR>
-__global__ void __launch_bounds__(256, Occ<R>::minb) k_slope_ctu(const KParams<R> p, const Box3x3 bx) {
+__global__ void __launch_bounds__(256, Occ<R>::minb) k_slope_ctu(const KParams<R> p, const Box3x3 bx, int wbase) {
   switch (blockIdx.y) {
-    case 0: slope_ctu_dir<R, LIMVAR, 0>(p, bx.b[0]); break;
-    case 1: slope_ctu_dir<R, LIMVAR, 1>(p, bx.b[1]); break;
-    default: slope_ctu_dir<R, LIMVAR, 2>(p, bx.b[2]); break;
+    case 0: slope_ctu_dir<R, LIMVAR, 0>(p, bx.b[0], wbase); break;
+    case 1: slope_ctu_dir<R, LIMVAR, 1>(p, bx.b[1], wbase); break;
+    default: slope_ctu_dir<R, LIMVAR, 2>(p, bx.b[2], wbase); break;
   }
 }
 
 template <class R, int RECON, int LIMVAR, int D>
-__device__ __forceinline__ void recon_ctu_dir(const KParams<R>& p, const Box3& box) {
+__device__ __forceinline__ void recon_ctu_dir(const KParams<R>& p, const Box3& box, int wbase) {
   constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
   Ctx<R> c(p, box);
   if (!c.ok) return;
   const int o = c.off(D), q = c.q, S3 = p.S3;
-  const R* W = c.arr(A_W);
+  const R* W = c.arr(wbase);
   const R* Bn = W + (size_t)(5 + D) * S3;
   const R sig = p.dt / p.dh, hdt = R(0.5) * p.dt;
   R wm[7], w0[7], wp[7], wlo[7], wup[7];
@@ -86,6 +86,15 @@ __device__ __forceinline__ void recon_ctu_dir(const KParams<R>& p, const Box3& b
       const R* sl = c.arr(A_F + 7 * D + v);
       sm[v] = sl[q - o]; s0[v] = sl[q]; sp[v] = sl[q + o];
     }
+    if (RECON == kPPMNoTrace) {
+      // VL + PPM (NEXT-4): the parabola's interface values at the half step, no tracing, no source terms
+      R W6[7];
+      ppm_parabola(wm, w0, wp, sm, s0, sp, wlo, wup, W6);
+      apply_floors(p, wlo); apply_floors(p, wup);
+#pragma unroll
+      for (int v = 0; v < 7; ++v) { c.arr(A_LO + 7 * D + v)[q] = wlo[v]; c.arr(A_UP + 7 * D + v)[q] = wup[v]; }
+      return;
+    }
     ppm_trace(wm, w0, wp, sm, s0, sp, Bn[q], p.gam, sig, wlo, wup);
   }
   const R* bn_ = c.arr(A_B + D); const R* b1_ = c.arr(A_B + T1); const R* b2_ = c.arr(A_B + T2);
@@ -100,11 +109,11 @@ __device__ __forceinline__ void recon_ctu_dir(const KParams<R>& p, const Box3& b
   for (int v = 0; v < 7; ++v) { c.arr(A_LO + 7 * D + v)[q] = wlo[v]; c.arr(A_UP + 7 * D + v)[q] = wup[v]; }
 }
 template <class R, int RECON, int LIMVAR>
-__global__ void __launch_bounds__(256, Occ<R>::minb) k_recon_ctu(const KParams<R> p, const Box3x3 bx) {
+__global__ void __launch_bounds__(256, Occ<R>::minb) k_recon_ctu(const KParams<R> p, const Box3x3 bx, int wbase) {
   switch (blockIdx.y) {
-    case 0: recon_ctu_dir<R, RECON, LIMVAR, 0>(p, bx.b[0]); break;
-    case 1: recon_ctu_dir<R, RECON, LIMVAR, 1>(p, bx.b[1]); break;
-    default: recon_ctu_dir<R, RECON, LIMVAR, 2>(p, bx.b[2]); break;
+    case 0: recon_ctu_dir<R, RECON, LIMVAR, 0>(p, bx.b[0], wbase); break;
+    case 1: recon_ctu_dir<R, RECON, LIMVAR, 1>(p, bx.b[1], wbase); break;
+    default: recon_ctu_dir<R, RECON, LIMVAR, 2>(p, bx.b[2], wbase); break;
   }
 }
 

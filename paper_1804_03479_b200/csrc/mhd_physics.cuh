@@ -37,8 +37,8 @@ template <class R> struct Occ { static constexpr int minb = sizeof(R) == 8 ? MHD
 template <class R, int SOLVER> struct OccFlux {
   static constexpr int minb = SOLVER == 2 ? (sizeof(R) == 8 ? 1 : 2) : (sizeof(R) == 8 ? MHD_MINB64_FLUX : MHD_MINB32);
 };
-enum : int { kPLM = 0, kPPM = 1 };
-enum : int { kLimPrim = 0, kLimChar = 1 };
+enum : int { kPLM = 0, kPPM = 1, kPPMNoTrace = 2 };   // kPPMNoTrace: the PPM parabola at the half step of VL (NEXT-4)
+enum : int { kLimPrim = 0, kLimChar = 1 };   // kernels take LIM = limvar + 2 * limiter (limiter: 0 MC, 1 minmod, 2 van Leer)
 
 template <class R> struct Num;
 template <> struct Num<float> {
@@ -99,6 +99,15 @@ template <class R> __device__ __forceinline__ R lim_minmod(R a, R b) {
   R m = Num<R>::min(Num<R>::abs(a), Num<R>::abs(b));
   m = (a > R(0)) ? m : -m;
   return (a * b <= R(0)) ? R(0) : m;
+}
+// van Leer (harmonic-mean) limiter, NEXT-4 variant
+template <class R> __device__ __forceinline__ R lim_vanleer(R a, R b) {
+  const R ab = a * b;
+  return (ab <= R(0)) ? R(0) : fdiv(R(2) * ab, a + b);
+}
+// slope limiter selected at compile time: 0 MC (R5), 1 minmod, 2 van Leer
+template <class R, int LIMITER> __device__ __forceinline__ R lim_sel(R a, R b) {
+  return LIMITER == 1 ? lim_minmod(a, b) : (LIMITER == 2 ? lim_vanleer(a, b) : lim_mc(a, b));
 }
 
 // ---- one side of a face: everything the solvers need from a primitive state -------------------------------

@@ -18,14 +18,15 @@ __device__ __forceinline__ void jac_mul(const R (&w0)[7], R bn, R gam, R irho, c
   y[6] = vn * x[6] + w0[6] * x[1] - bn * x[3];
 }
 
-// MC-limited slope of cell w0 from its two one-sided differences.
+// Limited slope of cell w0 from its two one-sided differences; LIMVAR = limvar + 2 * limiter.
 // LIM_PRIM: componentwise.  LIM_CHAR: project on the left eigenvectors of (w0, bn), limit each characteristic
 // amplitude, project back (wave order -f, -A, -s, entropy, +s, +A, +f).
 template <class R, int LIMVAR>
 __device__ __forceinline__ void limited_slope(const R (&w0)[7], R bn, R gam, const R (&dl)[7], const R (&dr)[7], R (&dw)[7]) {
-  if (LIMVAR == kLimPrim) {
+  constexpr int LM = LIMVAR >> 1;
+  if ((LIMVAR & 1) == kLimPrim) {
 #pragma unroll
-    for (int v = 0; v < 7; ++v) dw[v] = lim_mc(dl[v], dr[v]);
+    for (int v = 0; v < 7; ++v) dw[v] = lim_sel<R, LM>(dl[v], dr[v]);
     return;
   }
   // The eigenvectors of SURVEY A1 are sparse and come in +/- pairs: the projections are written through the
@@ -52,7 +53,7 @@ __device__ __forceinline__ void limited_slope(const R (&w0)[7], R bn, R gam, con
       amp[side][3] = d[0] - R(2) * nn * d[4];
     }
 #pragma unroll
-    for (int k = 0; k < 7; ++k) am[k] = lim_mc(amp[0][k], amp[1][k]);
+    for (int k = 0; k < 7; ++k) am[k] = lim_sel<R, LM>(amp[0][k], amp[1][k]);
   }
   const R Fs = am[0] + am[6], Fd = am[0] - am[6], Ss = am[2] + am[4], Sd = am[2] - am[4];
   const R Asum = am[1] + am[5], Adif = am[1] - am[5];
@@ -87,12 +88,11 @@ __device__ __forceinline__ void plm_trace(const R (&w0)[7], R bn, R gam, R sig, 
   }
 }
 
-// CTU step 1, PPM: parabola from the limited slopes of the cell and its two neighbours, monotonised
-// (R4 i-iii), then traced with the parabola's first and second moments.
+// PPM parabola of a cell from the limited slopes of the cell and its two neighbours, monotonised (R4 i-iii):
+// interface values Wl, Wr and W6
 template <class R>
-__device__ __forceinline__ void ppm_trace(const R (&wm)[7], const R (&w0)[7], const R (&wp)[7], const R (&sm)[7],
-                                          const R (&s0)[7], const R (&sp)[7], R bn, R gam, R sig, R (&wlo)[7], R (&wup)[7]) {
-  R Wl[7], Wr[7], xu[7], xl[7], W6[7];
+__device__ __forceinline__ void ppm_parabola(const R (&wm)[7], const R (&w0)[7], const R (&wp)[7], const R (&sm)[7],
+                                             const R (&s0)[7], const R (&sp)[7], R (&Wl)[7], R (&Wr)[7], R (&W6)[7]) {
 #pragma unroll
   for (int v = 0; v < 7; ++v) {
     R l = R(0.5) * (wm[v] + w0[v]) - (s0[v] - sm[v]) * R(1.0 / 6.0);
@@ -105,8 +105,19 @@ __device__ __forceinline__ void ppm_trace(const R (&wm)[7], const R (&w0)[7], co
     l = Num<R>::max(Num<R>::min(w0[v], wm[v]), Num<R>::min(Num<R>::max(w0[v], wm[v]), nl));
     r = Num<R>::max(Num<R>::min(w0[v], wp[v]), Num<R>::min(Num<R>::max(w0[v], wp[v]), nr));
     Wl[v] = l; Wr[v] = r;
-    const R dd = r - l;
     W6[v] = R(6) * (w0[v] - R(0.5) * (l + r));
+  }
+}
+
+// CTU step 1, PPM: the parabola traced with its first and second moments (matrix form, all waves).
+template <class R>
+__device__ __forceinline__ void ppm_trace(const R (&wm)[7], const R (&w0)[7], const R (&wp)[7], const R (&sm)[7],
+                                          const R (&s0)[7], const R (&sp)[7], R bn, R gam, R sig, R (&wlo)[7], R (&wup)[7]) {
+  R Wl[7], Wr[7], xu[7], xl[7], W6[7];
+  ppm_parabola(wm, w0, wp, sm, s0, sp, Wl, Wr, W6);
+#pragma unroll
+  for (int v = 0; v < 7; ++v) {
+    const R dd = Wr[v] - Wl[v];
     xu[v] = dd - W6[v]; xl[v] = dd + W6[v];
   }
   const R irho = frcp(w0[0]);

@@ -61,7 +61,9 @@ def test_strerror_and_null_argument_checks_need_no_device(libpath):
     h = C.c_void_p()
     bad = mhd.make_config(g=2)                       # ghost width below the minimum of DESIGN.md R8
     assert L.mhd_create(C.byref(bad), C.byref(h)) == mhd.EINVAL and not h
-    bad = mhd.make_config(scheme=mhd.VL, recon=mhd.PPM, g=4)
+    bad = mhd.make_config(scheme=mhd.VL, recon=mhd.PPM, g=3)      # VL + PPM needs 4 ghost cells like CTU + PPM
+    assert L.mhd_create(C.byref(bad), C.byref(h)) == mhd.EINVAL
+    bad = mhd.make_config(limiter=3)
     assert L.mhd_create(C.byref(bad), C.byref(h)) == mhd.EINVAL
     bad = mhd.make_config(scheme=mhd.CTU, recon=mhd.PPM, g=3)
     assert L.mhd_create(C.byref(bad), C.byref(h)) == mhd.EINVAL

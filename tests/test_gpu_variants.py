@@ -1,0 +1,71 @@
+"""-m gpu parity tests of the NEXT-4 variants: minmod / van Leer slope limiters and VL + PPM, the CUDA
+path through the C ABI against the oracle on the same seeded inputs.  Tolerances as tests/test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+from paper_1804_03479_b200 import inputs
+import harness as H
+import gpu_util as GU
+
+pytestmark = pytest.mark.gpu
+
+TOL = {1: 1e-11, 0: 1e-4}
+TOL_ONE_STEP = {1: 2e-13, 0: 1e-4}
+EMF_TIE = {1: 1e-12, 0: 1e-5}
+
+# name, scheme, recon, g, limiter
+VARIANTS = [("vl_ppm", 0, 1, 4, 0), ("vl_ppm_minmod", 0, 1, 4, 1), ("vl_ppm_vanleer", 0, 1, 4, 2), ("vl_plm_minmod", 0, 0, 3, 1),
+            ("vl_plm_vanleer", 0, 0, 3, 2), ("ctu_plm_minmod", 1, 0, 3, 1), ("ctu_plm_vanleer", 1, 0, 3, 2), ("ctu_ppm_minmod", 1, 1, 4, 1),
+            ("ctu_ppm_vanleer", 1, 1, 4, 2)]
+
+
+def bad_fields(errs, tol):
+    return {k: v for k, v in errs.items() if not (v <= tol)}
+
+
+@pytest.mark.parametrize("name,scheme,recon,g,limiter", VARIANTS)
+@pytest.mark.parametrize("limvar", [0, 1])
+@pytest.mark.parametrize("prec", [1, 0])
+def test_one_step_every_variant(oracle, name, scheme, recon, g, limiter, limvar, prec):
+    N, G = 16, 5
+    dtp = GU.np_dtype(prec)
+    U_in, B_in, dh = inputs.config2_batch(G, N=N, g=g, dtype=dtp)
+    U64, B64 = U_in.astype(np.float64), B_in.astype(np.float64)
+    for riemann in (1, 2):
+        cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon, riemann=riemann, limvar=limvar, limiter=limiter, emf_tie=EMF_TIE[prec])
+        dt, _ = oracle.dt_reduce(cfg, U64, B64, g, dh, 0.3)
+        ref = oracle.advance(cfg, U64, B64, dt, dh)
+        gpu = GU.GpuRunner(N=N, g=g, scheme=scheme, recon=recon, riemann=riemann, limvar=limvar, prec=prec, max_groups=G, limiter=limiter)
+        out = gpu(U_in, B_in, dt, dh)
+        errs = GU.field_errors(out, ref, N)
+        assert not bad_fields(errs, TOL_ONE_STEP[prec]), (name, riemann, limvar, errs)
+
+
+@pytest.mark.parametrize("prec", [1, 0])
+def test_vl_ppm_ten_steps_on_a_periodic_grid(oracle, prec):
+    """config-1 type run (32^3 periodic ABC grid cut into 8 groups, 10 steps at CFL 0.3) with VL + PPM, g = 4: per-field
+    parity at step 10, div B and shared faces on the device side"""
+    n, N, g = 32, 16, 4
+    dtp = GU.np_dtype(prec)
+    U, bx, by, bz, dh = inputs.abc_grid(n, seed=1804, p0=1.0, vamp=1e-3)
+    cfg = oracle.make_config(N=N, g=g, scheme=0, recon=1, emf_tie=EMF_TIE[prec])
+    adv = lambda Ui, Bi, dt, dh_: oracle.advance(cfg, Ui, Bi, dt, dh_)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=0, recon=1, prec=prec, max_groups=8)
+    ref = [a.astype(dtp).astype(np.float64) for a in (U, bx, by, bz)]
+    dev = [a.astype(dtp) for a in (U, bx, by, bz)]
+    for _ in range(10):
+        Ui, Bi = inputs.pack_groups(*ref, n, 0)
+        dt, _ = oracle.dt_reduce(oracle.make_config(N=n, g=3), Ui, Bi, 0, dh, 0.3)
+        ref = list(H.step_grid(adv, *ref, dt, dh, N, g)[:4])
+        r = H.step_grid(gpu, *dev, dt, dh, N, g, dtype=dtp)
+        dev = list(r[:4])
+        assert r[5] == 0.0                                       # faces shared by two groups: bitwise equal
+    assert H.rel_divb(*[a.astype(np.float64) for a in dev[1:]], dh) < (1e-13 if prec == 1 else 2e-5)
+    names = ["rho", "Mx", "My", "Mz", "e"]
+    errs = {names[v]: H.field_err(dev[0][v], ref[0][v]) for v in (0, 4)}
+    mom = max(np.abs(ref[0][v]).max() for v in (1, 2, 3))        # the three momentum components share one scale
+    for v in (1, 2, 3):
+        errs[names[v]] = float(np.abs(dev[0][v] - ref[0][v]).max() / mom)
+    for k, a, b in (("Bx", dev[1], ref[1]), ("By", dev[2], ref[2]), ("Bz", dev[3], ref[3])):
+        errs[k] = H.field_err(a, b)
+    assert not bad_fields(errs, TOL[prec]), errs
