@@ -259,3 +259,40 @@ def config2_batch(G, N=16, g=3, seed=3479, first=0, dtype=np.float64, gamma=GAMM
         u, b = pack_groups(U, bx, by, bz, N, g, dtype)
         U_in[q], B_in[q] = u[0], b[0]
     return U_in, B_in, 1.0 / N
+
+
+# ----------------------------------------------------------------------------------------
+# SURVEY 8(f) NEXT-4 second workload: the paper's 1-D Riemann problems (Table 1)
+# ----------------------------------------------------------------------------------------
+# (rho, vn, vt1, vt2, P, Bt1, Bt2) left / right and the longitudinal field Bn, as printed in Table 1 and PAPER.md:270
+RIEMANN_PROBLEMS = {
+    "rj2a": dict(L=(1.08, 1.2, 0.01, 0.5, 0.95, 3.6 / np.sqrt(4 * np.pi), 2.0 / np.sqrt(4 * np.pi)),
+                 R=(1.0, 0.0, 0.0, 0.0, 1.0, 4.0 / np.sqrt(4 * np.pi), 2.0 / np.sqrt(4 * np.pi)), Bn=2.0 / np.sqrt(4 * np.pi), t_end=0.2),
+    "torrilhon": dict(L=(1.0, 0.0, 0.0, 0.0, 1.0, 1.0, 0.0), R=(0.2, 0.0, 0.0, 0.0, 0.2, np.cos(3.0), np.sin(3.0)), Bn=1.0, t_end=0.08),
+}
+
+
+def shock_tube(name, n, axis=0, nt=8, gamma=GAMMA):
+    """Two copies of the tube back to back on a PERIODIC domain of length 2 along `axis` (2n cells, nt cells across):
+    left state on [0, 0.5) and [1.5, 2), right state on [0.5, 1.5), so that the paper's Dirichlet tube of length 1
+     is the part [0, 1) until the waves of the second interface arrive.  Returns U, bx, by, bz, dh."""
+    pr = RIEMANN_PROBLEMS[name]
+    nn = 2 * n
+    dh = 1.0 / n
+    xc = (np.arange(nn) + 0.5) * dh
+    left = (xc < 0.5) | (xc >= 1.5)
+    n_, t1, t2 = axis, (axis + 1) % 3, (axis + 2) % 3
+    shape = [nt, nt, nt]; shape[2 - axis] = nn
+    nz, ny, nx = shape
+    bshape = [1, 1, 1]; bshape[2 - axis] = nn
+    prof = [np.where(left, pr["L"][v], pr["R"][v]).reshape(bshape) for v in range(7)]
+    fs = [(nz, ny, nx + 1), (nz, ny + 1, nx), (nz + 1, ny, nx)]
+    b = [None, None, None]
+    b[n_] = np.full(fs[n_], pr["Bn"])
+    b[t1] = prof[5] + np.zeros(fs[t1])
+    b[t2] = prof[6] + np.zeros(fs[t2])
+    o = np.zeros((nz, ny, nx))
+    v = [None, None, None]
+    v[n_], v[t1], v[t2] = prof[1] + o, prof[2] + o, prof[3] + o
+    U = conserved(prof[0] + o, v[0], v[1], v[2], prof[4] + o, b[0], b[1], b[2], gamma)
+    return U, b[0], b[1], b[2], dh

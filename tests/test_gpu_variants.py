@@ -69,3 +69,37 @@ def test_vl_ppm_ten_steps_on_a_periodic_grid(oracle, prec):
     for k, a, b in (("Bx", dev[1], ref[1]), ("By", dev[2], ref[2]), ("Bz", dev[3], ref[3])):
         errs[k] = H.field_err(a, b)
     assert not bad_fields(errs, TOL[prec]), errs
+
+
+@pytest.mark.parametrize("name", ["rj2a", "torrilhon"])
+@pytest.mark.parametrize("prec", [1, 0])
+def test_shock_tubes_ctu_ppm_roe(oracle, name, prec):
+    """the paper's 1-D Riemann problems (Table 1) with its own combination CTU + PPM + Roe, patch
+    groups of 8^3 along the tube: 20 steps on the device against the oracle with the oracle's dt sequence"""
+    import tubes
+    n, g = 64, 4
+    dtp = GU.np_dtype(prec)
+    cfg = oracle.make_config(N=tubes.NT, g=g, scheme=1, recon=1, riemann=2, emf_tie=EMF_TIE[prec])
+    adv = lambda Ui, Bi, dt, dh: oracle.advance(cfg, Ui, Bi, dt, dh)
+    c0 = oracle.make_config(N=tubes.NT, g=3)
+
+    def dt_fn(U, bx, by, bz, dh):
+        Ui, Bi = inputs.pack_groups(U, bx, by, bz, tubes.NT, 0)
+        return oracle.dt_reduce(c0, Ui.astype(np.float64), Bi.astype(np.float64), 0, dh, 0.3)[0]
+    ref, dh, dts = tubes.run_tube(adv, dt_fn, name, n, max_steps=20, g=g)
+    if prec == 0:       # the FP64 oracle started from the FP32-rounded state (the tube states are not FP32 numbers)
+        U, bx, by, bz, _ = inputs.shock_tube(name, n, 0, tubes.NT)
+        ref = [a.astype(dtp).astype(np.float64) for a in (U, bx, by, bz)]
+        for dt in dts:
+            ref = list(H.step_grid(adv, *ref, dt, dh, tubes.NT, g)[:4])
+    gpu = GU.GpuRunner(N=tubes.NT, g=g, scheme=1, recon=1, riemann=2, prec=prec, max_groups=2 * n // tubes.NT)
+    it = iter(dts)
+    dev, _, _ = tubes.run_tube(gpu, lambda *a: next(it), name, n, t_end=sum(dts), dtype=dtp, g=g)
+    Pd, Pr = tubes.profile(dev, 2 * n), tubes.profile(ref, 2 * n)
+    mom = np.abs(Pr[1:4]).max()
+    errs = {}
+    for v, nm in enumerate(["rho", "Mn", "Mt1", "Mt2", "e", "Bt1", "Bt2"]):
+        den = mom if v in (1, 2, 3) else np.abs(Pr[v]).max()
+        errs[nm] = float(np.abs(Pd[v] - Pr[v]).max() / den)
+    assert not bad_fields(errs, TOL[prec]), errs
+    assert np.array_equal(dev[1], np.full_like(dev[1], dtp(inputs.RIEMANN_PROBLEMS[name]["Bn"])))      # B_n untouched
