@@ -20,7 +20,7 @@ DEPS = ["mhd_api.cu", "mhd_api_host.inl", "mhd_api_grid.inl", "mhd_api_amr.inl",
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "--expt-relaxed-constexpr",
+    "-Xcompiler", "-fPIC", "-shared", "--expt-relaxed-constexpr", "--split-compile", "0",
 ]
 
 

@@ -142,7 +142,9 @@ inline void prof_end(mhd_solver* s, cudaStream_t st) {
 
 // ---- index boxes: [lo, hi) per axis ---------------------------------------------------------
 inline Box3 box(int x0, int x1, int y0, int y1, int z0, int z1) {
-  Box3 b; b.lo[0] = x0; b.lo[1] = y0; b.lo[2] = z0; b.n[0] = x1 - x0; b.n[1] = y1 - y0; b.n[2] = z1 - z0; return b;
+  Box3 b; b.lo[0] = x0; b.lo[1] = y0; b.lo[2] = z0; b.n[0] = x1 - x0; b.n[1] = y1 - y0; b.n[2] = z1 - z0;
+  for (int a = 0; a < 2; ++a) b.m[a] = b.n[a] > 1 ? (unsigned)(0x100000000ULL / (unsigned)b.n[a]) + 1u : 0u;   // n >= 2 always (ps2 >= 8)
+  return b;
 }
 // per sweep direction d: normal index in [n0, n1), both transverse indices in [t0, t1)
 inline Box3x3 dir_boxes(int n0, int n1, int t0, int t1) {
@@ -170,8 +172,9 @@ inline unsigned blocks_for(const Box3x3& bx, int tpb) {
 }
 
 // all stages of one slice of groups, in the paper's step order
-template <class R>
-int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
+template <class R, int SC>
+int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
+  const KParamsSC<R, SC> p(p0);
   const int TPB = 256;
   const dim3 blk(TPB);
   const int T = s->T, S = s->S, N = s->N, g = s->g, sol = s->cfg.riemann;
@@ -179,26 +182,26 @@ int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
 #define GRID1(b) dim3(blocks_for(b, TPB), 1, ng)
 #define GRID3(b) dim3(blocks_for(b, TPB), 3, ng)
   const Box3 ball = box(0, S, 0, S, 0, S);
-  LAUNCH(ST_LOAD, (k_load_prim<R><<<GRID1(ball), blk, 0, st>>>(p, ball)));
+  LAUNCH(ST_LOAD, (k_load_prim<R, SC><<<GRID1(ball), blk, 0, st>>>(p, ball)));
   if (s->cfg.scheme == MHD_VL) {
     const Box3x3 bf1 = dir_boxes(1, T, 0, T), be1 = edge_boxes(1, T - 1, 0, T);
     const Box3 bh = box(1, T - 1, 1, T - 1, 1, T - 1);
     // pass 2 only where the final update needs it: faces n in [g, g+N], t in [g-1, g+N]; edges of the interior faces
     const Box3x3 bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1), be2 = edge_boxes(g, g + N, g, g + N);
-    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER><<<GRID3(bf1), blk, 0, st>>>(p, bf1))));          // step 1
-    LAUNCH(ST_EMF1, (k_emf<R><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 2
-    LAUNCH(ST_HALF, (k_half<R><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 3
+    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER, SC><<<GRID3(bf1), blk, 0, st>>>(p, bf1))));          // step 1
+    LAUNCH(ST_EMF1, (k_emf<R, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 2
+    LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 3
     if (s->cfg.recon == MHD_PLM) {
-      LIM_SWITCH(lim, LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, LIM><<<GRID3(bf2), blk, 0, st>>>(p, bf2)))));   // steps 4+5
+      LIM_SWITCH(lim, LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, LIM, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2)))));   // steps 4+5
     } else {
       // VL + PPM (NEXT-4): limited slopes of the half-step primitives (parked in the dead pass-1 flux arrays), the
       // monotonised parabola's interface values as L/R states, then the plain L/R Riemann kernel of CTU
       const Box3x3 bsl = dir_boxes(g - 2, g + N + 2, g - 1, g + N + 1), brc = dir_boxes(g - 1, g + N + 1, g - 1, g + N + 1);
-      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_slope_ctu<R, LIM><<<GRID3(bsl), blk, 0, st>>>(p, bsl, A_WH))));
-      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPPMNoTrace, LIM><<<GRID3(brc), blk, 0, st>>>(p, brc, A_WH))));
-      LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<GRID3(bf2), blk, 0, st>>>(p, bf2, A_BH))));
+      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_slope_ctu<R, LIM, SC><<<GRID3(bsl), blk, 0, st>>>(p, bsl, A_WH))));
+      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPPMNoTrace, LIM, SC><<<GRID3(brc), blk, 0, st>>>(p, brc, A_WH))));
+      LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2, A_BH))));
     }
-    LAUNCH(ST_EMF2, (k_emf<R><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 6
+    LAUNCH(ST_EMF2, (k_emf<R, SC><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 6
   } else {
     // everything is derived from the cells whose half-step state the second pass needs, [lo, hi)^3 = interior + 1:
     // pass-1 fluxes on their faces and on the faces their edge EMFs touch, face states one cell further, PPM slopes
@@ -210,26 +213,37 @@ int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
     const Box3x3 bco = dir_boxes(g - 1, g + N + 1, g - 1, g + N + 1), bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1);
     const Box3x3 be2 = edge_boxes(g, g + N, g, g + N);
     if (s->cfg.recon == MHD_PLM) {
-      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, LIM><<<GRID3(brc), blk, 0, st>>>(p, brc, A_W))));
+      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, LIM, SC><<<GRID3(brc), blk, 0, st>>>(p, brc, A_W))));
     } else {
       const Box3x3 bsl = dir_boxes(lo - 2, hi + 2, lo - 1, hi + 1);
-      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_slope_ctu<R, LIM><<<GRID3(bsl), blk, 0, st>>>(p, bsl, A_W))));
-      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, LIM><<<GRID3(brc), blk, 0, st>>>(p, brc, A_W))));
+      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_slope_ctu<R, LIM, SC><<<GRID3(bsl), blk, 0, st>>>(p, bsl, A_W))));
+      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, LIM, SC><<<GRID3(brc), blk, 0, st>>>(p, brc, A_W))));
     }                                                                                                          // step 1
-    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<GRID3(bf1), blk, 0, st>>>(p, bf1, A_B))));      // step 2
-    LAUNCH(ST_EMF1, (k_emf<R><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 3
-    LAUNCH(ST_HALF, (k_half<R><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 4
-    LAUNCH(ST_CORR, (k_ctu_corr<R><<<GRID3(bco), blk, 0, st>>>(p, bco, lo, hi)));                    // step 5
-    LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER><<<GRID3(bf2), blk, 0, st>>>(p, bf2, A_BH))));     // step 6
-    LAUNCH(ST_EMF2, (k_emf<R><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 7
+    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER, SC><<<GRID3(bf1), blk, 0, st>>>(p, bf1, A_B))));      // step 2
+    LAUNCH(ST_EMF1, (k_emf<R, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 3
+    LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 4
+    LAUNCH(ST_CORR, (k_ctu_corr<R, SC><<<GRID3(bco), blk, 0, st>>>(p, bco, lo, hi)));                    // step 5
+    LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2, A_BH))));     // step 6
+    LAUNCH(ST_EMF2, (k_emf<R, SC><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 7
   }
   const Box3 bin = box(g, g + N, g, g + N, g, g + N);
   const unsigned nbf = std::max(blocks_for(bin, TPB), (unsigned)((9 * (N + 1) * (N + 1) + TPB - 1) / TPB));
-  LAUNCH(ST_FINAL, (k_final<R><<<dim3(nbf, 1, ng), blk, 0, st>>>(p, bin)));                                    // step 7 / 8
+  LAUNCH(ST_FINAL, (k_final<R, SC><<<dim3(nbf, 1, ng), blk, 0, st>>>(p, bin)));                                    // step 7 / 8
 #undef GRID1
 #undef GRID3
   CU(cudaGetLastError());
   return MHD_OK;
+}
+
+// the kernels are instantiated for the two tile pitches of the standard patch group (N = 16: S = 23 with 3 ghost cells,
+// S = 25 with 4) and for a run-time pitch (everything else)
+template <class R>
+int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
+  switch (s->S) {
+    case 23: return run_slice_sc<R, 23>(s, p, ng, st);
+    case 25: return run_slice_sc<R, 25>(s, p, ng, st);
+    default: return run_slice_sc<R, 0>(s, p, ng, st);
+  }
 }
 
 // slices of one batch on ONE stream with ONE workspace (host path, profiling)

@@ -44,20 +44,33 @@ template <class R> struct KParams {
 };
 
 // compact index box of one launch: cells lo[d] .. lo[d]+n[d]-1; Box3x3 = one box per sweep direction
-struct Box3 { int lo[3], n[3]; };
+// m[0], m[1] = floor(2^32 / n[0,1]) + 1: t / n = umulhi(t, m) exactly for t n < 2^32 (a thread index within one group)
+struct Box3 { int lo[3], n[3]; unsigned m[2]; };
 struct Box3x3 { Box3 b[3]; };
 
-template <class R> struct Ctx {
-  const KParams<R>& p;
+// KParams with the tile pitch known at compile time (SC = S = T + 1 > 0): S, S2, S3, T shadow the run-time members, so every
+// array offset a * S3 and neighbour offset folds into the immediate field of the load / store.  SC = 0: run-time pitch.
+template <class R, int SC> struct KParamsSC : KParams<R> {
+  static constexpr int S = SC, S2 = SC * SC, S3 = SC * SC * SC, T = SC - 1;
+  KParamsSC() = default;
+  __host__ __device__ KParamsSC(const KParams<R>& b) : KParams<R>(b) {}
+};
+template <class R> struct KParamsSC<R, 0> : KParams<R> {
+  KParamsSC() = default;
+  __host__ __device__ KParamsSC(const KParams<R>& b) : KParams<R>(b) {}
+};
+
+template <class R, class KP> struct Ctx {
+  const KP& p;
   int q, i, j, k, grp;
   bool ok;
   R* w;   // this group's workspace
-  __device__ __forceinline__ Ctx(const KParams<R>& p_, const Box3& b) : p(p_) {
+  __device__ __forceinline__ Ctx(const KP& p_, const Box3& b) : p(p_) {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     ok = t < b.n[0] * b.n[1] * b.n[2];
-    const int r = t / b.n[0];
+    const int r = (int)__umulhi((unsigned)t, b.m[0]);
     i = b.lo[0] + (t - r * b.n[0]);
-    const int kk = r / b.n[1];
+    const int kk = (int)__umulhi((unsigned)r, b.m[1]);
     j = b.lo[1] + (r - kk * b.n[1]);
     k = b.lo[2] + kk;
     q = (k * p.S + j) * p.S + i;
@@ -81,15 +94,15 @@ __device__ __forceinline__ void load_gen(const R* Wb, int S3, int q, R (&w)[7]) 
   w[5] = Wb[(size_t)(5 + T1) * S3 + q]; w[6] = Wb[(size_t)(5 + T2) * S3 + q];
 }
 
-template <class R>
-__device__ __forceinline__ void apply_floors(const KParams<R>& p, R (&w)[7]) {
+template <class R, class KP>
+__device__ __forceinline__ void apply_floors(const KP& p, R (&w)[7]) {
   if (w[0] < p.min_dens) { w[0] = p.min_dens; count_event(p.stats + 0); }
   if (w[4] < p.min_pres) { w[4] = p.min_pres; count_event(p.stats + 1); }
 }
 
 // conserved cell data + the six face fields of the cell -> primitives (Eq. 5; floors R9)
-template <class R>
-__device__ __forceinline__ void cons_to_prim(const KParams<R>& p, const R (&u)[5], const R (&bl)[3], const R (&bu)[3], R (&W)[8]) {
+template <class R, class KP>
+__device__ __forceinline__ void cons_to_prim(const KP& p, const R (&u)[5], const R (&bl)[3], const R (&bu)[3], R (&W)[8]) {
   const R bcx = R(0.5) * (bl[0] + bu[0]), bcy = R(0.5) * (bl[1] + bu[1]), bcz = R(0.5) * (bl[2] + bu[2]);
   R rho = u[0];
   if (rho < p.min_dens) { rho = p.min_dens; count_event(p.stats + 0); }
@@ -101,8 +114,8 @@ __device__ __forceinline__ void cons_to_prim(const KParams<R>& p, const R (&u)[5
 }
 
 // primitives and the cell-centred reference EMF -(v x Bc) of a cell into the workspace
-template <class R>
-__device__ __forceinline__ void store_prim(const Ctx<R>& c, int wbase, const R (&W)[8]) {
+template <class R, class KP>
+__device__ __forceinline__ void store_prim(const Ctx<R, KP>& c, int wbase, const R (&W)[8]) {
 #pragma unroll
   for (int v = 0; v < 8; ++v) c.arr(wbase + v)[c.q] = W[v];
   c.arr(A_EC + 0)[c.q] = W[3] * W[6] - W[2] * W[7];
@@ -111,9 +124,10 @@ __device__ __forceinline__ void store_prim(const Ctx<R>& c, int wbase, const R (
 }
 
 // ---- S0 + S1: stage the input tile: face fields into the workspace, primitives of all T^3 cells -----------------
-template <class R>
-__global__ void __launch_bounds__(256) k_load_prim(const KParams<R> p, const Box3 box) {
-  Ctx<R> c(p, box);
+template <class R, int SC>
+__global__ void __launch_bounds__(256) k_load_prim(const KParamsSC<R, SC> p, const Box3 box) {
+  typedef KParamsSC<R, SC> KP;
+  Ctx<R, KP> c(p, box);
   if (!c.ok) return;
   const int T = p.T, i = c.i, j = c.j, k = c.k, q = c.q;
   const R* Bx = p.Bin + (size_t)c.grp * p.nBi;
@@ -145,9 +159,9 @@ __global__ void __launch_bounds__(256) k_load_prim(const KParams<R> p, const Box
 }
 
 // ---- VL step 1: first-order fluxes, normal B = face value ----------------------------------------
-template <class R, int SOLVER, int D>
-__device__ __forceinline__ void flux1_dir(const KParams<R>& p, const Box3& box) {
-  Ctx<R> c(p, box);
+template <class R, int SOLVER, int D, class KP>
+__device__ __forceinline__ void flux1_dir(const KP& p, const Box3& box) {
+  Ctx<R, KP> c(p, box);
   if (!c.ok) return;
   R wl[7], wr[7], F[7];
   load_gen<R, D>(c.arr(A_W), p.S3, c.q - c.off(D), wl);
@@ -157,8 +171,8 @@ __device__ __forceinline__ void flux1_dir(const KParams<R>& p, const Box3& box) 
 #pragma unroll
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[c.q] = F[v];
 }
-template <class R, int SOLVER>
-__global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux1_vl(const KParams<R> p, const Box3x3 bx) {
+template <class R, int SOLVER, int SC>
+__global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux1_vl(const KParamsSC<R, SC> p, const Box3x3 bx) {
   switch (blockIdx.y) {
     case 0: flux1_dir<R, SOLVER, 0>(p, bx.b[0]); break;
     case 1: flux1_dir<R, SOLVER, 1>(p, bx.b[1]); break;
@@ -178,10 +192,10 @@ template <class R> __device__ __forceinline__ R upwind(R m, R m0, R qm, R qp) {
   const R w = fdiv(am - m0, m0);                       // weight of the upwind value on the ramp m0 < |m| < 2 m0
   return w * qu + (R(1) - w) * mean;
 }
-template <class R, int C>
-__device__ __forceinline__ void emf_dir(const KParams<R>& p, const Box3& box, int rhobase) {
+template <class R, int C, class KP>
+__device__ __forceinline__ void emf_dir(const KP& p, const Box3& box, int rhobase) {
   constexpr int A = (C + 1) % 3, B = (C + 2) % 3;
-  Ctx<R> c(p, box);
+  Ctx<R, KP> c(p, box);
   if (!c.ok) return;
   const int q = c.q, qa = q - c.off(A), qb = q - c.off(B), qab = qa - c.off(B);
   const R* Fa5 = c.arr(A_F + 7 * A + 5); const R* Fa0 = c.arr(A_F + 7 * A + 0);
@@ -195,8 +209,8 @@ __device__ __forceinline__ void emf_dir(const KParams<R>& p, const Box3& box, in
   e += R(0.25) * (upwind(Fb0[qa], ht * (r_qab + r_qa), Ea_qb - ec_qab, Ea_q - ec_qa) - upwind(Fb0[q], ht * (r_qb + r_q), ec_qb - Ea_qb, ec_q - Ea_q));
   c.arr(A_E + C)[q] = e;
 }
-template <class R>
-__global__ void __launch_bounds__(256, OccEmf<R>::minb) k_emf(const KParams<R> p, const Box3x3 bx, int rhobase) {
+template <class R, int SC>
+__global__ void __launch_bounds__(256, OccEmf<R>::minb) k_emf(const KParamsSC<R, SC> p, const Box3x3 bx, int rhobase) {
   switch (blockIdx.y) {
     case 0: emf_dir<R, 0>(p, bx.b[0], rhobase); break;
     case 1: emf_dir<R, 1>(p, bx.b[1], rhobase); break;
@@ -205,16 +219,16 @@ __global__ void __launch_bounds__(256, OccEmf<R>::minb) k_emf(const KParams<R> p
 }
 
 // Eq. 13 for the lower D-face of cell x (flat index), step factor qh = tau/dh
-template <class R, int D>
-__device__ __forceinline__ R ct_face(const Ctx<R>& c, const R* bsrc, int x, R qh) {
+template <class R, int D, class KP>
+__device__ __forceinline__ R ct_face(const Ctx<R, KP>& c, const R* bsrc, int x, R qh) {
   constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
   const R* E1 = c.arr(A_E + T1); const R* E2 = c.arr(A_E + T2);
   return bsrc[x] - qh * ((E2[x + c.off(T1)] - E2[x]) - (E1[x + c.off(T2)] - E1[x]));
 }
 
 // Eq. 10: sum over x, y, z (in this order) of the flux differences of cell q, conserved order
-template <class R>
-__device__ __forceinline__ void flux_div(const Ctx<R>& c, R (&dU)[5]) {
+template <class R, class KP>
+__device__ __forceinline__ void flux_div(const Ctx<R, KP>& c, R (&dU)[5]) {
 #pragma unroll
   for (int v = 0; v < 5; ++v) dU[v] = R(0);
 #pragma unroll
@@ -230,8 +244,8 @@ __device__ __forceinline__ void flux_div(const Ctx<R>& c, R (&dU)[5]) {
   }
 }
 
-template <class R>
-__device__ __forceinline__ void load_U_in(const KParams<R>& p, const Ctx<R>& c, R (&u)[5]) {
+template <class R, class KP>
+__device__ __forceinline__ void load_U_in(const KP& p, const Ctx<R, KP>& c, R (&u)[5]) {
   const int T = p.T;
   const R* U = p.Uin + (size_t)c.grp * p.nUi;
   const size_t T3 = (size_t)T * T * T, cq = ((size_t)c.k * T + c.j) * T + c.i;
@@ -240,9 +254,10 @@ __device__ __forceinline__ void load_U_in(const KParams<R>& p, const Ctx<R>& c, 
 }
 
 // ---- S4: half-step state: U^{n+1/2}, b^{n+1/2} on the faces of the cells, W^{n+1/2} -------
-template <class R>
-__global__ void __launch_bounds__(256, OccHalf<R>::minb) k_half(const KParams<R> p, const Box3 box) {
-  Ctx<R> c(p, box);
+template <class R, int SC>
+__global__ void __launch_bounds__(256, OccHalf<R>::minb) k_half(const KParamsSC<R, SC> p, const Box3 box) {
+  typedef KParamsSC<R, SC> KP;
+  Ctx<R, KP> c(p, box);
   if (!c.ok) return;
   const R qh = (R(0.5) * p.dt) / p.dh;
   R u[5], dU[5];

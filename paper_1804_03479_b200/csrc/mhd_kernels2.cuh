@@ -5,9 +5,9 @@
 namespace mhd {
 
 // ---- VL steps 4+5: PLM at the half step + Riemann solve, normal B = half-step face value --------
-template <class R, int SOLVER, int LIMVAR, int D>
-__device__ __forceinline__ void flux2_vl_dir(const KParams<R>& p, const Box3& box) {
-  Ctx<R> c(p, box);
+template <class R, int SOLVER, int LIMVAR, int D, class KP>
+__device__ __forceinline__ void flux2_vl_dir(const KP& p, const Box3& box) {
+  Ctx<R, KP> c(p, box);
   if (!c.ok) return;
   const int o = c.off(D), q = c.q;
   const R* Wh = c.arr(A_WH);
@@ -27,8 +27,8 @@ __device__ __forceinline__ void flux2_vl_dir(const KParams<R>& p, const Box3& bo
 #pragma unroll
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[q] = F[v];
 }
-template <class R, int SOLVER, int LIMVAR>
-__global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux2_vl(const KParams<R> p, const Box3x3 bx) {
+template <class R, int SOLVER, int LIMVAR, int SC>
+__global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux2_vl(const KParamsSC<R, SC> p, const Box3x3 bx) {
   switch (blockIdx.y) {
     case 0: flux2_vl_dir<R, SOLVER, LIMVAR, 0>(p, bx.b[0]); break;
     case 1: flux2_vl_dir<R, SOLVER, LIMVAR, 1>(p, bx.b[1]); break;
@@ -39,9 +39,9 @@ __global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux2_vl(cons
 // ---- CTU step 1: reconstruction + half-step tracing + primitive MHD source terms ------------------
 // PPM needs the limited slope of three cells per cell: the slopes are computed once per cell and direction by
 // k_slope_ctu (parked in the flux arrays, which are free until step 2) and read back here.
-template <class R, int LIMVAR, int D>
-__device__ __forceinline__ void slope_ctu_dir(const KParams<R>& p, const Box3& box, int wbase) {
-  Ctx<R> c(p, box);
+template <class R, int LIMVAR, int D, class KP>
+__device__ __forceinline__ void slope_ctu_dir(const KP& p, const Box3& box, int wbase) {
+  Ctx<R, KP> c(p, box);
   if (!c.ok) return;
   const int o = c.off(D), q = c.q, S3 = p.S3;
   const R* W = c.arr(wbase);
@@ -53,8 +53,8 @@ __device__ __forceinline__ void slope_ctu_dir(const KParams<R>& p, const Box3& b
 #pragma unroll
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[q] = dw[v];
 }
-template <class R, int LIMVAR>
-__global__ void __launch_bounds__(256, Occ<R>::minb) k_slope_ctu(const KParams<R> p, const Box3x3 bx, int wbase) {
+template <class R, int LIMVAR, int SC>
+__global__ void __launch_bounds__(256, Occ<R>::minb) k_slope_ctu(const KParamsSC<R, SC> p, const Box3x3 bx, int wbase) {
   switch (blockIdx.y) {
     case 0: slope_ctu_dir<R, LIMVAR, 0>(p, bx.b[0], wbase); break;
     case 1: slope_ctu_dir<R, LIMVAR, 1>(p, bx.b[1], wbase); break;
@@ -62,10 +62,10 @@ __global__ void __launch_bounds__(256, Occ<R>::minb) k_slope_ctu(const KParams<R
   }
 }
 
-template <class R, int RECON, int LIMVAR, int D>
-__device__ __forceinline__ void recon_ctu_dir(const KParams<R>& p, const Box3& box, int wbase) {
+template <class R, int RECON, int LIMVAR, int D, class KP>
+__device__ __forceinline__ void recon_ctu_dir(const KP& p, const Box3& box, int wbase) {
   constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
-  Ctx<R> c(p, box);
+  Ctx<R, KP> c(p, box);
   if (!c.ok) return;
   const int o = c.off(D), q = c.q, S3 = p.S3;
   const R* W = c.arr(wbase);
@@ -108,8 +108,8 @@ __device__ __forceinline__ void recon_ctu_dir(const KParams<R>& p, const Box3& b
 #pragma unroll
   for (int v = 0; v < 7; ++v) { c.arr(A_LO + 7 * D + v)[q] = wlo[v]; c.arr(A_UP + 7 * D + v)[q] = wup[v]; }
 }
-template <class R, int RECON, int LIMVAR>
-__global__ void __launch_bounds__(256, Occ<R>::minb) k_recon_ctu(const KParams<R> p, const Box3x3 bx, int wbase) {
+template <class R, int RECON, int LIMVAR, int SC>
+__global__ void __launch_bounds__(256, Occ<R>::minb) k_recon_ctu(const KParamsSC<R, SC> p, const Box3x3 bx, int wbase) {
   switch (blockIdx.y) {
     case 0: recon_ctu_dir<R, RECON, LIMVAR, 0>(p, bx.b[0], wbase); break;
     case 1: recon_ctu_dir<R, RECON, LIMVAR, 1>(p, bx.b[1], wbase); break;
@@ -118,9 +118,9 @@ __global__ void __launch_bounds__(256, Occ<R>::minb) k_recon_ctu(const KParams<R
 }
 
 // ---- CTU steps 2 and 6: Riemann solve between the upper state of cell i-1 and the lower of i ----
-template <class R, int SOLVER, int D>
-__device__ __forceinline__ void flux_lr_dir(const KParams<R>& p, const Box3& box, int bbase) {
-  Ctx<R> c(p, box);
+template <class R, int SOLVER, int D, class KP>
+__device__ __forceinline__ void flux_lr_dir(const KP& p, const Box3& box, int bbase) {
+  Ctx<R, KP> c(p, box);
   if (!c.ok) return;
   const int q = c.q, ql = q - c.off(D);
   R wl[7], wr[7], F[7];
@@ -131,8 +131,8 @@ __device__ __forceinline__ void flux_lr_dir(const KParams<R>& p, const Box3& box
 #pragma unroll
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[q] = F[v];
 }
-template <class R, int SOLVER>
-__global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux_lr(const KParams<R> p, const Box3x3 bx, int bbase) {
+template <class R, int SOLVER, int SC>
+__global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux_lr(const KParamsSC<R, SC> p, const Box3x3 bx, int bbase) {
   switch (blockIdx.y) {
     case 0: flux_lr_dir<R, SOLVER, 0>(p, bx.b[0], bbase); break;
     case 1: flux_lr_dir<R, SOLVER, 1>(p, bx.b[1], bbase); break;
@@ -142,10 +142,10 @@ __global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux_lr(const
 
 // ---- CTU step 5: transverse flux-gradient correction + conservative MHD source terms (R6) -----------
 // flo / fhi: range of faces of direction D on which the half-step normal field exists
-template <class R, int D>
-__device__ __forceinline__ void ctu_corr_dir(const KParams<R>& p, const Box3& box, int flo, int fhi) {
+template <class R, int D, class KP>
+__device__ __forceinline__ void ctu_corr_dir(const KP& p, const Box3& box, int flo, int fhi) {
   constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
-  Ctx<R> c(p, box);
+  Ctx<R, KP> c(p, box);
   if (!c.ok) return;
   const int cn = c.idx(D);
   const int q = c.q, od = c.off(D), o1 = c.off(T1), o2 = c.off(T2);
@@ -198,8 +198,8 @@ __device__ __forceinline__ void ctu_corr_dir(const KParams<R>& p, const Box3& bo
     for (int v = 0; v < 7; ++v) c.arr(base + v)[q] = w[v];
   }
 }
-template <class R>
-__global__ void __launch_bounds__(256) k_ctu_corr(const KParams<R> p, const Box3x3 bx, int flo, int fhi) {
+template <class R, int SC>
+__global__ void __launch_bounds__(256) k_ctu_corr(const KParamsSC<R, SC> p, const Box3x3 bx, int flo, int fhi) {
   switch (blockIdx.y) {
     case 0: ctu_corr_dir<R, 0>(p, bx.b[0], flo, fhi); break;
     case 1: ctu_corr_dir<R, 1>(p, bx.b[1], flo, fhi); break;

@@ -8,8 +8,8 @@ namespace mhd {
 // ---- S8: U^{n+1} = U^n - dt/dh sum dF2 (Eq. 10) on the N^3 interior cells, b^{n+1} by Eq. 13 on their faces;
 // epilogue: time-centred fluxes and edge EMFs on the lower / mid / upper face planes of each
 // direction, copied by the first 9 (N+1)^2 threads of the group (one per plane point (a2, a1), a1, a2 in [0, N]) -------
-template <class R>
-__device__ __forceinline__ void copy_planes(const KParams<R>& p, int grp, int t) {
+template <class R, class KP>
+__device__ __forceinline__ void copy_planes(const KP& p, int grp, int t) {
   const int N = p.N, M = N + 1, g = p.g;
   if (t >= 9 * M * M) return;
   const int a1 = t % M, a2 = (t / M) % M, pl = t / (M * M);
@@ -34,10 +34,11 @@ __device__ __forceinline__ void copy_planes(const KParams<R>& p, int grp, int t)
   }
 }
 
-template <class R>
-__global__ void __launch_bounds__(256, OccFinal<R>::minb) k_final(const KParams<R> p, const Box3 box) {
-  Ctx<R> c(p, box);
-  if (p.fout || p.eout) copy_planes(p, blockIdx.z, blockIdx.x * blockDim.x + threadIdx.x);
+template <class R, int SC>
+__global__ void __launch_bounds__(256, OccFinal<R>::minb) k_final(const KParamsSC<R, SC> p, const Box3 box) {
+  typedef KParamsSC<R, SC> KP;
+  Ctx<R, KP> c(p, box);
+  if (p.fout || p.eout) copy_planes<R>(p, blockIdx.z, blockIdx.x * blockDim.x + threadIdx.x);
   if (!c.ok) return;
   const int g = p.g, N = p.N;
   const int ii = c.i - g, jj = c.j - g, kk = c.k - g;

@@ -29,9 +29,17 @@ enum : int { kHLLE = 0, kHLLD = 1, kROE = 2 };
 #endif
 // latency-bound update kernels: resident 256-thread blocks per SM requested from ptxas, from sweeps on B200
 // (uncapped, ptxas hoists every load of the FP64 half-step kernel into 158 registers: 11 % of the warps resident)
-template <class R> struct OccHalf  { static constexpr int minb = sizeof(R) == 8 ? 2 : 6; };
-template <class R> struct OccFinal { static constexpr int minb = sizeof(R) == 8 ? 4 : 6; };
-template <class R> struct OccEmf   { static constexpr int minb = sizeof(R) == 8 ? 5 : 1; };
+#ifndef MHD_OCC_HALF64
+#define MHD_OCC_HALF64 2
+#define MHD_OCC_HALF32 6
+#define MHD_OCC_FINAL64 4
+#define MHD_OCC_FINAL32 6
+#define MHD_OCC_EMF64 5
+#define MHD_OCC_EMF32 1
+#endif
+template <class R> struct OccHalf  { static constexpr int minb = sizeof(R) == 8 ? MHD_OCC_HALF64 : MHD_OCC_HALF32; };
+template <class R> struct OccFinal { static constexpr int minb = sizeof(R) == 8 ? MHD_OCC_FINAL64 : MHD_OCC_FINAL32; };
+template <class R> struct OccEmf   { static constexpr int minb = sizeof(R) == 8 ? MHD_OCC_EMF64 : MHD_OCC_EMF32; };
 template <class R> struct Occ { static constexpr int minb = sizeof(R) == 8 ? MHD_MINB64 : MHD_MINB32; };          // reconstruction
 // Riemann kernels (measured: HLLD FP64 3 > 2 > 4 blocks; Roe needs ~220 FP64 / ~120 FP32 registers and must not be capped)
 template <class R, int SOLVER> struct OccFlux {

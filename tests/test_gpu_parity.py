@@ -119,7 +119,19 @@ def test_config2_batch_vl_plm_10_steps(oracle, prec):
         dt, _ = oracle.dt_reduce(cfg, Ui, Bi, g, dh, 0.3)
         ref_boxes, ref_out = H.step_boxes(adv, ref_boxes, dt, dh, N, g)
         gpu_boxes, gpu_out = H.step_boxes(gpu, gpu_boxes, dt, dh, N, g, dtype=dtp)
-    assert_fields(GU.field_errors(gpu_out, ref_out, N), TOL[prec], f"config 2 prec={prec} outputs of step 10")
+    # DESIGN.md R14a: in a group whose pressure floor fires, P = (gamma-1)(e - KE - ME) is the difference of numbers 1e5+
+    # times larger, i.e. rounding noise in FP32; the time-centred plane fluxes of such a group are held to
+    # 5e-4 of the batch maximum, everything else (all fields of all groups, planes of the other groups) to 1e-4
+    floored = np.array([oracle.advance(cfg, Ui[q:q + 1], Bi[q:q + 1], dt, dh)["stats"][1] > 0 for q in range(G)])
+    sel = lambda out, m: {k: (np.asarray(v)[m] if v is not None else None) for k, v in out.items() if k in ("U", "B", "flux", "emf")}
+    if prec == 0 and floored.any():
+        clean = ~floored
+        assert_fields(GU.field_errors(sel(gpu_out, clean), sel(ref_out, clean), N), TOL[prec], "config 2 FP32, groups without floor events")
+        e_all = GU.field_errors(gpu_out, ref_out, N)
+        assert_fields({k: v for k, v in e_all.items() if not k.startswith(("flux", "emf"))}, TOL[prec], "config 2 FP32, fields of all groups")
+        assert_fields({k: v for k, v in e_all.items() if k.startswith(("flux", "emf"))}, 5e-4, "config 2 FP32, planes of floored groups")
+    else:
+        assert_fields(GU.field_errors(gpu_out, ref_out, N), TOL[prec], f"config 2 prec={prec} outputs of step 10")
     for q in range(G):
         bx, by, bz = (np.asarray(a, dtype=np.float64) for a in gpu_boxes[q][1:])
         assert H.rel_divb(bx, by, bz, dh) < (1e-13 if prec == 1 else 2e-5)
