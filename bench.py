@@ -35,11 +35,11 @@ FLOP_PER_SOLVE = {"hlld": 381, "roe": 1107, "hlle": 361}
 FLOP_PER_CELL_UPDATE = {("vl", "hlld"): 6263.5, ("vl", "roe"): 15289.0, ("ctu", "hlld"): 26067.6, ("ctu", "roe"): 35160.4}   # whole step
 FLOP_PLM_PER_FACE = 140     # two MC-limited primitive slopes + the two face states (VL pass 2)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage kernel at 512 groups, VL+PLM+HLLD, from the
-# ncu --set full captures summarised in profiles/r01_full_top_kernels.md / r01_full_top_kernels_f64.md (MB)
-NCU_TRAFFIC_MB = {"f32": {"load_prim": 569.4, "flux_pass1": 862.9, "emf_pass1": 380.8, "half_step": 888.4, "flux_pass2": 644.2,
-                          "emf_pass2": 242.5, "final_update": 431.0, "dt_reduce": 69.2},
-                  "f64": {"load_prim": 1063.3, "flux_pass1": 1598.1, "emf_pass1": 737.8, "half_step": 1666.0, "flux_pass2": 1078.6,
-                          "emf_pass2": 451.5, "final_update": 848.8, "dt_reduce": 140.8}}
+# ncu --set full captures summarised in profiles/r01c_full_top_kernels.md / r01c_f64_full_top_kernels.md (MB)
+NCU_TRAFFIC_MB = {"f32": {"load_prim": 569.3, "flux_pass1": 863.6, "emf_pass1": 380.7, "half_step": 888.4, "flux_pass2": 642.7,
+                          "emf_pass2": 242.3, "final_update": 430.3, "dt_reduce": 69.1},
+                  "f64": {"load_prim": 1063.4, "flux_pass1": 1599.8, "emf_pass1": 737.4, "half_step": 1665.0, "flux_pass2": 1083.4,
+                          "emf_pass2": 450.6, "final_update": 847.5, "dt_reduce": 141.1}}
 NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
 
 
@@ -54,6 +54,9 @@ def parse():
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"], help="precision of the headline value")
     ap.add_argument("--groups", type=int, default=NGROUPS)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--config5", type=int, default=0, metavar="POOL", help="instead of the batch: BASELINE config 5, 262144 "
+                    "group-updates (= 1024^3 cells) in FP32 streamed from a pinned pool of POOL groups (a multiple of 512, e.g. 4096), "
+                    "VL+PLM and CTU+PPM, with and without transfers")
     ap.add_argument("--grid", type=int, default=0, help="instead of the batch: a periodic n^3 ABC grid (BASELINE config 3 "
                     "state) kept on the device; step = mhd_grid_dt + mhd_grid_advance (pack + scheme + unpack)")
     return ap.parse_args()
@@ -213,7 +216,7 @@ def measure(args, prec_name, rank, world, dist):
                 "peak_source": "nominal: 148 SMs x %d FMA lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if prec_name == "f32" else 64),
                 "peak_fma_measured": mhd.measure_fma_peak(dev.index, prec),
                 "traffic": (NCU_TRAFFIC_MB[prec_name].get(top) * 1e6 if (args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS) else None),
-                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_*)",
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01c_*)",
                 "avg_launch_ms": dur * 1e3, "launches_per_step": n_launch,
                 "share_of_step": stages[top]["ms_per_step"] / (prof_ms / args.steps)}
     # HBM view of the whole step: algorithmic bytes = read the ghost-zoned tile once, write the results once (+ dt read)
@@ -255,6 +258,75 @@ def measure(args, prec_name, rank, world, dist):
                   "api": "mhd_advance_host(chunk_groups=%d, nstreams=%d), pinned host memory" % (chunk, nstr),
                   "h2d_plus_d2h_GBs": (h2d + d2h) * world / 1e9 / (te / args.steps)}
     res["stats"] = solver.get_stats()
+    solver.destroy()
+    return res
+
+
+def measure_config5(args, scheme_name):
+    """BASELINE config 5: 1024^3 cells = 262144 patch groups of the ABC state (config 3), FP32, one step, streamed as
+    16^3 patch-group batches from a pinned host pool (the full set would be 91-118 GB in / 52 GB out):
+    the pool = the patch groups of a 256^3 ABC grid, cycled.  With transfers: mhd_advance_host (H2D, kernels and D2H of
+    successive chunks overlapped on CUDA streams), host wall clock.  Without: the same pool resident on
+    the device, mhd_advance per 512-group batch, CUDA events."""
+    import numpy as np
+    import torch
+    from paper_1804_03479_b200 import inputs, mhd
+    P, total, batch = args.config5, (1024 // N_PS2) ** 3, 512
+    a2 = argparse.Namespace(**{**vars(args), "scheme": scheme_name})
+    sp = scheme_params(a2)
+    g = sp["g"]
+    riem = {"hlle": mhd.HLLE, "hlld": mhd.HLLD, "roe": mhd.ROE}[args.riemann]
+    solver = mhd.Solver(mhd.make_config(N=N_PS2, g=g, scheme=sp["scheme"], recon=sp["recon"], riemann=riem, prec=mhd.FP32, max_groups=P))
+    U, bx, by, bz, dh = inputs.abc_grid(256, seed=1805, p0=0.15, vamp=1e-2)
+    hU, hB = inputs.pack_groups(U, bx, by, bz, N_PS2, g, np.float32)
+    reps = (P + hU.shape[0] - 1) // hU.shape[0]
+    hU, hB = np.tile(hU, (reps, 1))[:P].copy(), np.tile(hB, (reps, 1))[:P].copy()
+    dt0 = 0.3 * dh / 6.0                                         # well below the CFL limit of the state (max speed ~ 2.5)
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    pU, pB = pin(hU), pin(hB)
+    out = solver.alloc_outputs(P, planes=True)
+    hout = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
+    passes = total // P
+    chunk, nstr = 32, 4
+    solver.advance_host(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], P, dt0, dh, chunk, nstr)
+    sampler = ClockSampler(torch.cuda.current_device())
+    torch.cuda.synchronize()
+    sampler.start()
+    t0 = time.perf_counter()
+    for _ in range(passes):
+        solver.advance_host(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], P, dt0, dh, chunk, nstr)
+    torch.cuda.synchronize()
+    te = time.perf_counter() - t0
+    clocks = sampler.result()
+    sz = solver.sizes()
+    h2d = (sz["n_U_in"] + sz["n_B_in"]) * 4 * total
+    d2h = (sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]) * 4 * total
+    # device-resident pool, 512-group batches
+    dU, dB = pU.cuda(), pB.cuda()
+    stream = torch.cuda.current_stream()
+    views = lambda t, b: t[b * batch:(b + 1) * batch]
+    l0 = solver.launch_count()
+
+    def one_pass():
+        for b in range(P // batch):
+            solver.advance(views(dU, b), views(dB, b), views(out["U"], b), views(out["B"], b), views(out["flux"], b), views(out["emf"], b),
+                           batch, dt0, dh, stream)
+    one_pass()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(passes):
+        one_pass()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    cells = total * N_PS2 ** 3
+    res = {"scheme": sp["name"], "with_transfers": {"value": cells / te, "unit": "cell-updates/s", "seconds": te, "h2d_bytes": h2d, "d2h_bytes": d2h,
+                                                     "h2d_plus_d2h_GBs": (h2d + d2h) / 1e9 / te,
+                                                     "api": "mhd_advance_host(chunk_groups=%d, nstreams=%d), pinned pool of %d groups x %d passes" % (chunk, nstr, P, passes)},
+           "without_transfers": {"value": cells / (ms * 1e-3), "unit": "cell-updates/s", "seconds": ms * 1e-3,
+                                 "api": "mhd_advance, %d-group batches of the device-resident pool" % batch},
+           "clocks": clocks, "gpu_launches": solver.launch_count() - l0, "stats": solver.get_stats()}
     solver.destroy()
     return res
 
@@ -375,6 +447,20 @@ def main():
         import torch.distributed as dist_mod
         dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
         dist = dist_mod
+    if args.config5:
+        r = [measure_config5(args, "vl"), measure_config5(args, "ctu")]
+        config.update(workload="BASELINE.json configs[4]: 1024^3 cells = 262144 patch groups of 16^3 of the config-3 ABC state, FP32, one step, "
+                               "streamed from a pinned pool of %d groups (the patch groups of a 256^3 ABC grid, cycled)" % args.config5,
+                      step="mhd_advance_host over the whole stream (with transfers) / mhd_advance per 512-group batch (without)",
+                      groups_per_rank=262144, scheme="VL+PLM and CTU+PPM")
+        print(json.dumps({"metric": "cell-updates/sec", "value": r[0]["without_transfers"]["value"], "unit": "cell-updates/s", "n_gpus": 1,
+                          "steps": 1, "warmup": 1, "ms_per_step": r[0]["without_transfers"]["seconds"] * 1e3, "higher_is_better": True,
+                          "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config,
+                          "clocks": r[0]["clocks"], "gpu_launches": r[0]["gpu_launches"],
+                          "e2e": {"value": r[0]["with_transfers"]["value"], "unit": "cell-updates/s", "h2d_bytes_per_step": r[0]["with_transfers"]["h2d_bytes"],
+                                  "d2h_bytes_per_step": r[0]["with_transfers"]["d2h_bytes"]},
+                          "vl_plm": r[0], "ctu_ppm": r[1]}))
+        return 0
     if args.grid:
         a, b = measure_grid(args, args.prec), measure_grid(args, "f64" if args.prec == "f32" else "f32")
         config.update(workload="BASELINE.json config 3 state: periodic %d^3 ABC grid (beta 0.1) resident on the device, cut "

@@ -246,12 +246,19 @@ int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
   }
 }
 
+// a batch that needs several slices is cut into equal ones (no small last slice whose launches cannot fill the GPU)
+inline int balanced_slice(const mhd_solver* s, int ngroups) {
+  const int nslices = (ngroups + s->slice_groups - 1) / s->slice_groups;
+  return (ngroups + nslices - 1) / nslices;
+}
+
 // slices of one batch on ONE stream with ONE workspace (host path, profiling)
 template <class R>
 int advance_serial(mhd_solver* s, const void* Ui, const void* Bi, void* Uo, void* Bo, void* fo, void* eo, void* ws,
                    int ngroups, double dt, double dh, cudaStream_t st) {
-  for (int first = 0; first < ngroups; first += s->slice_groups) {
-    const int ng = std::min(s->slice_groups, ngroups - first);
+  const int per = balanced_slice(s, ngroups);
+  for (int first = 0; first < ngroups; first += per) {
+    const int ng = std::min(per, ngroups - first);
     KParams<R> p = make_params<R>(s, Ui, Bi, Uo, Bo, fo, eo, ws, first, dt, dh);
     int rc = run_slice<R>(s, p, ng, st);
     if (rc != MHD_OK) return rc;
@@ -263,14 +270,15 @@ int advance_serial(mhd_solver* s, const void* Ui, const void* Bi, void* Uo, void
 template <class R>
 int advance_lanes(mhd_solver* s, const void* Ui, const void* Bi, void* Uo, void* Bo, void* fo, void* eo,
                   int ngroups, double dt, double dh, cudaStream_t user) {
-  const int nslices = (ngroups + s->slice_groups - 1) / s->slice_groups;
+  const int per = balanced_slice(s, ngroups);
+  const int nslices = (ngroups + per - 1) / per;
   const int nl = std::min(s->nlanes, nslices);
   if (s->prof_on || nl <= 1) return advance_serial<R>(s, Ui, Bi, Uo, Bo, fo, eo, s->dev[0].ws, ngroups, dt, dh, user);
   CU(cudaEventRecord(s->fork, user));
   for (int l = 0; l < nl; ++l) CU(cudaStreamWaitEvent(s->dev[l].stream, s->fork, 0));
   int i = 0;
-  for (int first = 0; first < ngroups; first += s->slice_groups, ++i) {
-    const int ng = std::min(s->slice_groups, ngroups - first);
+  for (int first = 0; first < ngroups; first += per, ++i) {
+    const int ng = std::min(per, ngroups - first);
     DevLane& L = s->dev[i % nl];
     KParams<R> p = make_params<R>(s, Ui, Bi, Uo, Bo, fo, eo, L.ws, first, dt, dh);
     int rc = run_slice<R>(s, p, ng, L.stream);
