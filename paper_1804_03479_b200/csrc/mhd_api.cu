@@ -181,6 +181,7 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
   const int lim = s->cfg.limvar + 2 * s->cfg.limiter;     // template parameter LIM of the slope kernels
 #define GRID1(b) dim3(blocks_for(b, TPB), 1, ng)
 #define GRID3(b) dim3(blocks_for(b, TPB), 3, ng)
+  int f2 = A_F;                                   // where the pass-2 fluxes are
   const Box3 ball = box(0, S, 0, S, 0, S);
   LAUNCH(ST_LOAD, (k_load_prim<R, SC><<<GRID1(ball), blk, 0, st>>>(p, ball)));
   if (s->cfg.scheme == MHD_VL) {
@@ -189,7 +190,7 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
     // pass 2 only where the final update needs it: faces n in [g, g+N], t in [g-1, g+N]; edges of the interior faces
     const Box3x3 bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1), be2 = edge_boxes(g, g + N, g, g + N);
     LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER, SC><<<GRID3(bf1), blk, 0, st>>>(p, bf1))));          // step 1
-    LAUNCH(ST_EMF1, (k_emf<R, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 2
+    LAUNCH(ST_EMF1, (k_emf<R, A_F, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 2
     LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 3
     if (s->cfg.recon == MHD_PLM) {
       LIM_SWITCH(lim, LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, LIM, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2)))));   // steps 4+5
@@ -201,7 +202,7 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
       LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPPMNoTrace, LIM, SC><<<GRID3(brc), blk, 0, st>>>(p, brc, A_WH))));
       LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2, A_BH))));
     }
-    LAUNCH(ST_EMF2, (k_emf<R, SC><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 6
+    LAUNCH(ST_EMF2, (k_emf<R, A_F, SC><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 6
   } else {
     // everything is derived from the cells whose half-step state the second pass needs, [lo, hi)^3 = interior + 1:
     // pass-1 fluxes on their faces and on the faces their edge EMFs touch, face states one cell further, PPM slopes
@@ -220,15 +221,16 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
       LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, LIM, SC><<<GRID3(brc), blk, 0, st>>>(p, brc, A_W))));
     }                                                                                                          // step 1
     LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER, SC><<<GRID3(bf1), blk, 0, st>>>(p, bf1, A_B))));      // step 2
-    LAUNCH(ST_EMF1, (k_emf<R, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 3
+    LAUNCH(ST_EMF1, (k_emf<R, A_F, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 3
     LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 4
-    LAUNCH(ST_CORR, (k_ctu_corr<R, SC><<<GRID3(bco), blk, 0, st>>>(p, bco, lo, hi)));                    // step 5
-    LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2, A_BH))));     // step 6
-    LAUNCH(ST_EMF2, (k_emf<R, SC><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 7
+    LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_ctu<R, SOLVER, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2))));        // steps 5 + 6
+    LAUNCH(ST_EMF2, (k_emf<R, A_F2, SC><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                               // step 7
+    f2 = A_F2;
   }
   const Box3 bin = box(g, g + N, g, g + N, g, g + N);
   const unsigned nbf = std::max(blocks_for(bin, TPB), (unsigned)((9 * (N + 1) * (N + 1) + TPB - 1) / TPB));
-  LAUNCH(ST_FINAL, (k_final<R, SC><<<dim3(nbf, 1, ng), blk, 0, st>>>(p, bin)));                                    // step 7 / 8
+  if (f2 == A_F) LAUNCH(ST_FINAL, (k_final<R, A_F, SC><<<dim3(nbf, 1, ng), blk, 0, st>>>(p, bin)));                // step 7 / 8
+  else LAUNCH(ST_FINAL, (k_final<R, A_F2, SC><<<dim3(nbf, 1, ng), blk, 0, st>>>(p, bin)));
 #undef GRID1
 #undef GRID3
   CU(cudaGetLastError());

@@ -29,7 +29,8 @@ enum : int {
   A_VL_END = 49,
   A_LO = 49,    // 21: CTU state at the lower d-face of each cell, [d][v]
   A_UP = 70,    // 21: CTU state at the upper d-face
-  A_CTU_END = 91
+  A_F2 = 91,    // 21: CTU pass-2 fluxes (the fused correction + Riemann kernel still reads the pass-1 fluxes while it writes)
+  A_CTU_END = 112
 };
 
 template <class R> struct KParams {
@@ -192,14 +193,14 @@ template <class R> __device__ __forceinline__ R upwind(R m, R m0, R qm, R qp) {
   const R w = fdiv(am - m0, m0);                       // weight of the upwind value on the ramp m0 < |m| < 2 m0
   return w * qu + (R(1) - w) * mean;
 }
-template <class R, int C, class KP>
+template <class R, int C, int FBASE, class KP>
 __device__ __forceinline__ void emf_dir(const KP& p, const Box3& box, int rhobase) {
   constexpr int A = (C + 1) % 3, B = (C + 2) % 3;
   Ctx<R, KP> c(p, box);
   if (!c.ok) return;
   const int q = c.q, qa = q - c.off(A), qb = q - c.off(B), qab = qa - c.off(B);
-  const R* Fa5 = c.arr(A_F + 7 * A + 5); const R* Fa0 = c.arr(A_F + 7 * A + 0);
-  const R* Fb6 = c.arr(A_F + 7 * B + 6); const R* Fb0 = c.arr(A_F + 7 * B + 0);
+  const R* Fa5 = c.arr(FBASE + 7 * A + 5); const R* Fa0 = c.arr(FBASE + 7 * A + 0);
+  const R* Fb6 = c.arr(FBASE + 7 * B + 6); const R* Fb0 = c.arr(FBASE + 7 * B + 0);
   const R* ec = c.arr(A_EC + C); const R* rho = c.arr(rhobase);
   const R Ea_q = -Fa5[q], Ea_qb = -Fa5[qb], Eb_q = Fb6[q], Eb_qa = Fb6[qa];
   const R ec_q = ec[q], ec_qa = ec[qa], ec_qb = ec[qb], ec_qab = ec[qab];
@@ -209,12 +210,12 @@ __device__ __forceinline__ void emf_dir(const KP& p, const Box3& box, int rhobas
   e += R(0.25) * (upwind(Fb0[qa], ht * (r_qab + r_qa), Ea_qb - ec_qab, Ea_q - ec_qa) - upwind(Fb0[q], ht * (r_qb + r_q), ec_qb - Ea_qb, ec_q - Ea_q));
   c.arr(A_E + C)[q] = e;
 }
-template <class R, int SC>
+template <class R, int FBASE, int SC>
 __global__ void __launch_bounds__(256, OccEmf<R>::minb) k_emf(const KParamsSC<R, SC> p, const Box3x3 bx, int rhobase) {
   switch (blockIdx.y) {
-    case 0: emf_dir<R, 0>(p, bx.b[0], rhobase); break;
-    case 1: emf_dir<R, 1>(p, bx.b[1], rhobase); break;
-    default: emf_dir<R, 2>(p, bx.b[2], rhobase); break;
+    case 0: emf_dir<R, 0, FBASE>(p, bx.b[0], rhobase); break;
+    case 1: emf_dir<R, 1, FBASE>(p, bx.b[1], rhobase); break;
+    default: emf_dir<R, 2, FBASE>(p, bx.b[2], rhobase); break;
   }
 }
 
@@ -227,14 +228,14 @@ __device__ __forceinline__ R ct_face(const Ctx<R, KP>& c, const R* bsrc, int x, 
 }
 
 // Eq. 10: sum over x, y, z (in this order) of the flux differences of cell q, conserved order
-template <class R, class KP>
+template <int FBASE, class R, class KP>
 __device__ __forceinline__ void flux_div(const Ctx<R, KP>& c, R (&dU)[5]) {
 #pragma unroll
   for (int v = 0; v < 5; ++v) dU[v] = R(0);
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     const int t1 = (d + 1) % 3, t2 = (d + 2) % 3, qu = c.q + c.off(d);
-    const R* F = c.arr(A_F + 7 * d);
+    const R* F = c.arr(FBASE + 7 * d);
     const size_t S3 = c.p.S3;
     dU[0] += F[qu] - F[c.q];
     dU[1 + d] += F[S3 + qu] - F[S3 + c.q];
@@ -262,7 +263,7 @@ __global__ void __launch_bounds__(256, OccHalf<R>::minb) k_half(const KParamsSC<
   const R qh = (R(0.5) * p.dt) / p.dh;
   R u[5], dU[5];
   load_U_in(p, c, u);
-  flux_div(c, dU);
+  flux_div<A_F>(c, dU);
 #pragma unroll
   for (int v = 0; v < 5; ++v) u[v] = u[v] - qh * dU[v];
   const int q = c.q;

@@ -140,70 +140,89 @@ __global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux_lr(const
   }
 }
 
-// ---- CTU step 5: transverse flux-gradient correction + conservative MHD source terms (R6) -----------
-// flo / fhi: range of faces of direction D on which the half-step normal field exists
+// ---- CTU steps 5 + 6: transverse flux-gradient correction + conservative MHD source terms (R6) of
+// the two states of a face, then the Riemann solve.  The corrected states never go to memory: the face reads the
+// step-1 states of its two cells (upper state of cell i-1, lower state of cell i), everything the correction of each
+// cell needs (pass-1 fluxes and edge EMFs of the transverse directions, time-n field gradients), and writes the pass-2
+// flux into its own arrays (A_F2) because neighbouring faces still read the pass-1 fluxes.
+// The part of the correction shared by the two faces of a cell:
+template <class R> struct CtuCorr {
+  R dF0, dF1, dF2, dF3, dF4;   // transverse flux differences in the generic order of D: (rho, M_D, M_T1, M_T2, e)
+  R dB1, dB2;                  // CT update of the transverse field by the step-3 edge EMFs along D
+  R dbn, m1, m2;               // dB_D/dD and the limited source factors
+  R Bcn, Bc1, Bc2, v1, v2;     // time-n cell-centred field and transverse velocity
+};
 template <class R, int D, class KP>
-__device__ __forceinline__ void ctu_corr_dir(const KP& p, const Box3& box, int flo, int fhi) {
+__device__ __forceinline__ void ctu_corr_cell(const Ctx<R, KP>& c, const KP& p, int q, R qh, CtuCorr<R>& k) {
   constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
-  Ctx<R, KP> c(p, box);
-  if (!c.ok) return;
-  const int cn = c.idx(D);
-  const int q = c.q, od = c.off(D), o1 = c.off(T1), o2 = c.off(T2);
+  const int od = c.off(D), o1 = c.off(T1), o2 = c.off(T2);
   const size_t S3 = p.S3;
-  const R hdt = R(0.5) * p.dt, qh = hdt / p.dh;
   R w0[7];
   load_gen<R, D>(c.arr(A_W), p.S3, q, w0);
-  const R Bcn = c.arr(A_W + 5 + D)[q];
+  k.Bcn = c.arr(A_W + 5 + D)[q];
   // F[T1] is stored in generic order (T1, T2, D): its momentum slots (Mn, Mt1, Mt2) are (M_T1, M_T2, M_D);
   // F[T2] is in order (T2, D, T1): (M_T2, M_D, M_T1).  Permute into the generic order of D: (rho, M_D, M_T1, M_T2, e).
   const R* F1 = c.arr(A_F + 7 * T1); const R* F2 = c.arr(A_F + 7 * T2);
   auto d1 = [&](int comp) { return F1[comp * S3 + q + o1] - F1[comp * S3 + q]; };
   auto d2 = [&](int comp) { return F2[comp * S3 + q + o2] - F2[comp * S3 + q]; };
-  const R dF0 = d1(0) + d2(0), dF1 = d1(3) + d2(2), dF2 = d1(1) + d2(3), dF3 = d1(2) + d2(1), dF4 = d1(4) + d2(4);
+  k.dF0 = d1(0) + d2(0); k.dF1 = d1(3) + d2(2); k.dF2 = d1(1) + d2(3); k.dF3 = d1(2) + d2(1); k.dF4 = d1(4) + d2(4);
   const R* En = c.arr(A_E + D);
   const R Emm = En[q], Epm = En[q + o1], Emp = En[q + o2], Epp = En[q + o1 + o2];
-  const R dB1 = -qh * R(0.5) * ((Emp - Emm) + (Epp - Epm));
-  const R dB2 = qh * R(0.5) * ((Epm - Emm) + (Epp - Emp));
+  k.dB1 = -qh * R(0.5) * ((Emp - Emm) + (Epp - Epm));
+  k.dB2 = qh * R(0.5) * ((Epm - Emm) + (Epp - Emp));
   const R* bn_ = c.arr(A_B + D); const R* b1_ = c.arr(A_B + T1); const R* b2_ = c.arr(A_B + T2);
   const R idh = R(1) / p.dh;
-  const R dbn = (bn_[q + od] - bn_[q]) * idh, db1 = (b1_[q + o1] - b1_[q]) * idh, db2 = (b2_[q + o2] - b2_[q]) * idh;
-  const R m1 = lim_minmod(dbn, -db2), m2 = lim_minmod(dbn, -db1);
-  const R Bc1 = w0[5], Bc2 = w0[6], v1 = w0[2], v2 = w0[3];
-#pragma unroll
-  for (int side = 0; side < 2; ++side) {
-    const int face = cn + side;
-    if (face < flo || face > fhi) continue;
-    const int qf = q + (side ? od : 0);
-    const int base = (side ? A_UP : A_LO) + 7 * D;
-    R w[7], u[7];
-#pragma unroll
-    for (int v = 0; v < 7; ++v) w[v] = c.arr(base + v)[q];
-    const R bnn = bn_[qf];
-    u[0] = w[0]; u[1] = w[0] * w[1]; u[2] = w[0] * w[2]; u[3] = w[0] * w[3];
-    u[4] = w[4] * p.gm1inv + R(0.5) * w[0] * (sqr(w[1]) + sqr(w[2]) + sqr(w[3])) + R(0.5) * (sqr(bnn) + sqr(w[5]) + sqr(w[6]));
-    u[5] = w[5]; u[6] = w[6];
-    u[0] -= qh * dF0; u[1] -= qh * dF1; u[2] -= qh * dF2; u[3] -= qh * dF3; u[4] -= qh * dF4;
-    u[5] += dB1; u[6] += dB2;
-    u[1] += hdt * Bcn * dbn; u[2] += hdt * Bc1 * dbn; u[3] += hdt * Bc2 * dbn;
-    u[5] += hdt * v1 * m1; u[6] += hdt * v2 * m2;
-    u[4] += hdt * (Bc1 * v1 * m1 + Bc2 * v2 * m2);
-    const R bh = c.arr(A_BH + D)[qf];
-    R rho = u[0];
-    if (rho < p.min_dens) { rho = p.min_dens; count_event(p.stats + 0); }
-    const R ir = frcp(rho);
-    w[0] = rho; w[1] = u[1] * ir; w[2] = u[2] * ir; w[3] = u[3] * ir; w[5] = u[5]; w[6] = u[6];
-    w[4] = p.gm1 * (u[4] - R(0.5) * rho * (sqr(w[1]) + sqr(w[2]) + sqr(w[3])) - R(0.5) * (sqr(bh) + sqr(w[5]) + sqr(w[6])));
-    if (w[4] < p.min_pres) { w[4] = p.min_pres; count_event(p.stats + 1); }
-#pragma unroll
-    for (int v = 0; v < 7; ++v) c.arr(base + v)[q] = w[v];
-  }
+  k.dbn = (bn_[q + od] - bn_[q]) * idh;
+  const R db1 = (b1_[q + o1] - b1_[q]) * idh, db2 = (b2_[q + o2] - b2_[q]) * idh;
+  k.m1 = lim_minmod(k.dbn, -db2); k.m2 = lim_minmod(k.dbn, -db1);
+  k.Bc1 = w0[5]; k.Bc2 = w0[6]; k.v1 = w0[2]; k.v2 = w0[3];
 }
-template <class R, int SC>
-__global__ void __launch_bounds__(256) k_ctu_corr(const KParamsSC<R, SC> p, const Box3x3 bx, int flo, int fhi) {
+// one state w of the cell (at the face whose time-n normal field is bnn and half-step normal field bh): to conserved
+// variables, correct, back to primitive variables with the floors of R9
+template <class R, class KP>
+__device__ __forceinline__ void ctu_corr_apply(const KP& p, const CtuCorr<R>& k, R hdt, R qh, R bnn, R bh, R (&w)[7]) {
+  R u[7];
+  u[0] = w[0]; u[1] = w[0] * w[1]; u[2] = w[0] * w[2]; u[3] = w[0] * w[3];
+  u[4] = w[4] * p.gm1inv + R(0.5) * w[0] * (sqr(w[1]) + sqr(w[2]) + sqr(w[3])) + R(0.5) * (sqr(bnn) + sqr(w[5]) + sqr(w[6]));
+  u[5] = w[5]; u[6] = w[6];
+  u[0] -= qh * k.dF0; u[1] -= qh * k.dF1; u[2] -= qh * k.dF2; u[3] -= qh * k.dF3; u[4] -= qh * k.dF4;
+  u[5] += k.dB1; u[6] += k.dB2;
+  u[1] += hdt * k.Bcn * k.dbn; u[2] += hdt * k.Bc1 * k.dbn; u[3] += hdt * k.Bc2 * k.dbn;
+  u[5] += hdt * k.v1 * k.m1; u[6] += hdt * k.v2 * k.m2;
+  u[4] += hdt * (k.Bc1 * k.v1 * k.m1 + k.Bc2 * k.v2 * k.m2);
+  R rho = u[0];
+  if (rho < p.min_dens) { rho = p.min_dens; count_event(p.stats + 0); }
+  const R ir = frcp(rho);
+  w[0] = rho; w[1] = u[1] * ir; w[2] = u[2] * ir; w[3] = u[3] * ir; w[5] = u[5]; w[6] = u[6];
+  w[4] = p.gm1 * (u[4] - R(0.5) * rho * (sqr(w[1]) + sqr(w[2]) + sqr(w[3])) - R(0.5) * (sqr(bh) + sqr(w[5]) + sqr(w[6])));
+  if (w[4] < p.min_pres) { w[4] = p.min_pres; count_event(p.stats + 1); }
+}
+template <class R, int SOLVER, int D, class KP>
+__device__ __forceinline__ void flux2_ctu_dir(const KP& p, const Box3& box) {
+  Ctx<R, KP> c(p, box);
+  if (!c.ok) return;
+  const int q = c.q, ql = q - c.off(D);
+  const R hdt = R(0.5) * p.dt, qh = hdt / p.dh;
+  R wl[7], wr[7], F[7];
+#pragma unroll
+  for (int v = 0; v < 7; ++v) { wl[v] = c.arr(A_UP + 7 * D + v)[ql]; wr[v] = c.arr(A_LO + 7 * D + v)[q]; }
+  const R bnn = c.arr(A_B + D)[q], bh = c.arr(A_BH + D)[q];
+  CtuCorr<R> k;
+  ctu_corr_cell<R, D>(c, p, ql, qh, k);
+  ctu_corr_apply(p, k, hdt, qh, bnn, bh, wl);
+  ctu_corr_cell<R, D>(c, p, q, qh, k);
+  ctu_corr_apply(p, k, hdt, qh, bnn, bh, wr);
+  const bool fb = riemann<R, SOLVER>(wl, wr, bh, p.gam, p.gm1inv, F);
+  if (fb) count_event(p.stats + 2);
+#pragma unroll
+  for (int v = 0; v < 7; ++v) c.arr(A_F2 + 7 * D + v)[q] = F[v];
+}
+template <class R, int SOLVER, int SC>
+__global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux2_ctu(const KParamsSC<R, SC> p, const Box3x3 bx) {
   switch (blockIdx.y) {
-    case 0: ctu_corr_dir<R, 0>(p, bx.b[0], flo, fhi); break;
-    case 1: ctu_corr_dir<R, 1>(p, bx.b[1], flo, fhi); break;
-    default: ctu_corr_dir<R, 2>(p, bx.b[2], flo, fhi); break;
+    case 0: flux2_ctu_dir<R, SOLVER, 0>(p, bx.b[0]); break;
+    case 1: flux2_ctu_dir<R, SOLVER, 1>(p, bx.b[1]); break;
+    default: flux2_ctu_dir<R, SOLVER, 2>(p, bx.b[2]); break;
   }
 }
 

@@ -8,7 +8,7 @@ namespace mhd {
 // ---- S8: U^{n+1} = U^n - dt/dh sum dF2 (Eq. 10) on the N^3 interior cells, b^{n+1} by Eq. 13 on their faces;
 // epilogue: time-centred fluxes and edge EMFs on the lower / mid / upper face planes of each
 // direction, copied by the first 9 (N+1)^2 threads of the group (one per plane point (a2, a1), a1, a2 in [0, N]) -------
-template <class R, class KP>
+template <class R, int FBASE, class KP>
 __device__ __forceinline__ void copy_planes(const KP& p, int grp, int t) {
   const int N = p.N, M = N + 1, g = p.g;
   if (t >= 9 * M * M) return;
@@ -20,7 +20,7 @@ __device__ __forceinline__ void copy_planes(const KP& p, int grp, int t) {
   const int q = (iz * p.S + iy) * p.S + ix;
   const R* w = p.ws + (size_t)grp * p.narr * p.S3;
   if (p.fout && a1 < N && a2 < N) {
-    const R* F = w + (size_t)(A_F + 7 * d) * p.S3;
+    const R* F = w + (size_t)(FBASE + 7 * d) * p.S3;
     const R f0 = F[q], fn = F[(size_t)p.S3 + q], f1 = F[(size_t)2 * p.S3 + q], f2 = F[(size_t)3 * p.S3 + q], f4 = F[(size_t)4 * p.S3 + q];
     R* fo = p.fout + (size_t)grp * p.nF + (size_t)pl * 5 * N * N + (size_t)a2 * N + a1;
     const size_t NN = (size_t)N * N;
@@ -34,18 +34,18 @@ __device__ __forceinline__ void copy_planes(const KP& p, int grp, int t) {
   }
 }
 
-template <class R, int SC>
+template <class R, int FBASE, int SC>
 __global__ void __launch_bounds__(256, OccFinal<R>::minb) k_final(const KParamsSC<R, SC> p, const Box3 box) {
   typedef KParamsSC<R, SC> KP;
   Ctx<R, KP> c(p, box);
-  if (p.fout || p.eout) copy_planes<R>(p, blockIdx.z, blockIdx.x * blockDim.x + threadIdx.x);
+  if (p.fout || p.eout) copy_planes<R, FBASE>(p, blockIdx.z, blockIdx.x * blockDim.x + threadIdx.x);
   if (!c.ok) return;
   const int g = p.g, N = p.N;
   const int ii = c.i - g, jj = c.j - g, kk = c.k - g;
   const R qh = p.dt / p.dh;
   R u[5], dU[5];
   load_U_in(p, c, u);
-  flux_div(c, dU);
+  flux_div<FBASE>(c, dU);
   R* Uo = p.Uout + (size_t)c.grp * p.nUo;
   const size_t N3 = (size_t)N * N * N, cq = ((size_t)kk * N + jj) * N + ii;
 #pragma unroll
