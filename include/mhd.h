@@ -64,8 +64,8 @@ typedef struct {
 
 enum { MHD_OK = 0, MHD_EINVAL = -1, MHD_ECUDA = -2, MHD_ENOMEM = -3 };
 
-/* Create a solver.  Allocates the device workspace (sized for an L2-resident slice of groups, not for
- * max_groups).  Returns MHD_EINVAL for a bad configuration (incl. too small a ghost width), MHD_ECUDA /
+/* Create a solver.  Allocates the device workspace (for min(max_groups, what fits a 6 GB budget) groups: larger
+ * batches are processed in equal slices).  Returns MHD_EINVAL for a bad configuration (incl. too small a ghost width), MHD_ECUDA /
  * MHD_ENOMEM for device errors.  *out is NULL on failure. */
 int mhd_create(const mhd_config* cfg, mhd_solver** out);
 int mhd_destroy(mhd_solver* s);
