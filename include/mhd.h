@@ -157,7 +157,7 @@ int mhd_amr_prolong(mhd_solver* s, const void* Uc, const void* bxc, const void* 
 /* Per-stage device timing for the roofline report: when on, every stage launch is bracketed by CUDA events on its
  * stream (up to 16384 launches since the last mhd_set_profiling call; later ones are not recorded).
  * mhd_get_profile synchronises the device, fills the summed milliseconds and launch counts of each stage
- * (arrays of at least 10 entries) and returns the number of stages; mhd_profile_stage_name names stage i. */
+ * (arrays of at least 16 entries) and returns the number of stages; mhd_profile_stage_name names stage i. */
 int mhd_set_profiling(mhd_solver* s, int on);
 int mhd_get_profile(mhd_solver* s, double* ms_per_stage, unsigned long long* launches_per_stage, int nstages);
 const char* mhd_profile_stage_name(int stage);

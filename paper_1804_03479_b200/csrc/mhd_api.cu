@@ -14,6 +14,7 @@
 #include "mhd_grid.cuh"
 #include "mhd_amr.cuh"
 #include "mhd_prolong.cuh"
+#include "mhd_ctu_pass1.cuh"
 
 using namespace mhd;
 
@@ -63,6 +64,7 @@ struct mhd_solver {
   int lane_groups = 0, lane_count = 0;
   // optional per-stage timing (mhd_set_profiling): pairs of events around every stage launch; slices then run
   // one after the other on the caller's stream so that the stage times do not overlap
+  bool no_fused_pass1 = false;              // MHD_NO_FUSED_PASS1=1: the staged CTU steps 1 + 2 also for the standard group (tests)
   bool prof_on = false;
   std::vector<cudaEvent_t> prof_ev;         // 2 per recorded launch
   std::vector<int> prof_stage;              // stage id per recorded launch
@@ -112,9 +114,9 @@ KParams<R> make_params(const mhd_solver* s, const void* Ui, const void* Bi, void
     default: { constexpr int LIM = 5; CALL; } break; \
   }
 
-enum Stage : int { ST_LOAD = 0, ST_RECON, ST_FLUX1, ST_EMF1, ST_HALF, ST_CORR, ST_FLUX2, ST_EMF2, ST_FINAL, ST_DT, ST_COUNT };
+enum Stage : int { ST_LOAD = 0, ST_RECON, ST_FLUX1, ST_EMF1, ST_HALF, ST_CORR, ST_FLUX2, ST_EMF2, ST_FINAL, ST_DT, ST_PASS1, ST_COUNT };
 const char* const kStageNames[ST_COUNT] = { "load_prim", "recon_ctu", "flux_pass1", "emf_pass1", "half_step", "ctu_corr",
-                                            "flux_pass2", "emf_pass2", "final_update", "dt_reduce" };
+                                            "flux_pass2", "emf_pass2", "final_update", "dt_reduce", "ctu_pass1_fused" };
 constexpr size_t kProfMaxLaunches = 16384;
 
 inline void prof_begin(mhd_solver* s, int stage, cudaStream_t st) {
@@ -213,14 +215,26 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
     const Box3 bh = box(lo, hi, lo, hi, lo, hi);
     const Box3x3 bco = dir_boxes(g - 1, g + N + 1, g - 1, g + N + 1), bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1);
     const Box3x3 be2 = edge_boxes(g, g + N, g, g + N);
-    if (s->cfg.recon == MHD_PLM) {
-      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, LIM, SC><<<GRID3(brc), blk, 0, st>>>(p, brc, A_W))));
-    } else {
-      const Box3x3 bsl = dir_boxes(lo - 2, hi + 2, lo - 1, hi + 1);
-      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_slope_ctu<R, LIM, SC><<<GRID3(bsl), blk, 0, st>>>(p, bsl, A_W))));
-      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, LIM, SC><<<GRID3(brc), blk, 0, st>>>(p, brc, A_W))));
-    }                                                                                                          // step 1
-    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER, SC><<<GRID3(bf1), blk, 0, st>>>(p, bf1, A_B))));      // step 2
+    // standard patch group in FP32 with PPM, MC limiter in characteristic variables and HLLD: steps 1 + 2 in one kernel
+    // (mhd_ctu_pass1.cuh); everything else: slopes -> states -> Riemann solve as three kernels
+    bool fused1 = false;
+    if constexpr (SC == 25 && sizeof(R) == 4) {
+      fused1 = N == 16 && g == 4 && s->cfg.recon == MHD_PPM && lim == 1 && sol == MHD_HLLD && !s->no_fused_pass1;
+      if (fused1) {
+        const size_t shm = (size_t)21 * kP1Threads * sizeof(R);
+        LAUNCH(ST_PASS1, (k_ctu_pass1<R, kHLLD, 1, SC><<<dim3(kP1Across, 3, ng), kP1Threads, shm, st>>>(p)));
+      }
+    }
+    if (!fused1) {
+      if (s->cfg.recon == MHD_PLM) {
+        LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPLM, LIM, SC><<<GRID3(brc), blk, 0, st>>>(p, brc, A_W))));
+      } else {
+        const Box3x3 bsl = dir_boxes(lo - 2, hi + 2, lo - 1, hi + 1);
+        LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_slope_ctu<R, LIM, SC><<<GRID3(bsl), blk, 0, st>>>(p, bsl, A_W))));
+        LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPPM, LIM, SC><<<GRID3(brc), blk, 0, st>>>(p, brc, A_W))));
+      }                                                                                                        // step 1
+      LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER, SC><<<GRID3(bf1), blk, 0, st>>>(p, bf1, A_B))));    // step 2
+    }
     LAUNCH(ST_EMF1, (k_emf<R, A_F, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 3
     LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 4
     LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_ctu<R, SOLVER, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2))));        // steps 5 + 6
@@ -339,6 +353,7 @@ int mhd_create(const mhd_config* cfg, mhd_solver** out) {
   if (!(s->cfg.emf_tie > 0.0)) s->cfg.emf_tie = cfg->prec == MHD_FP32 ? 1e-5 : 1e-12;
   s->N = cfg->ps2; s->g = cfg->nghost; s->T = s->N + 2 * s->g; s->S = s->T + 1;
   s->S3 = (size_t)s->S * s->S * s->S;
+  s->no_fused_pass1 = getenv("MHD_NO_FUSED_PASS1") != nullptr;
   s->narr = (cfg->scheme == MHD_VL && cfg->recon == MHD_PLM) ? A_VL_END : A_CTU_END;   // face-state arrays: CTU, VL + PPM
   s->esz = cfg->prec == MHD_FP32 ? 4 : 8;
   const size_t N = s->N, T = s->T;

@@ -198,6 +198,24 @@ def test_no_stage_reads_an_unwritten_workspace_value(scheme, recon, g, prec, mon
                 assert np.array_equal(out[k], ref[k]), (riemann, limvar, k)
 
 
+def test_fused_ctu_pass1_equals_the_staged_kernels_bitwise(monkeypatch):
+    """CTU steps 1 + 2 of the standard FP32 patch group run in one pencil kernel (csrc/mhd_ctu_pass1.cuh); with
+    MHD_NO_FUSED_PASS1 the same solver runs slopes -> states -> Riemann solve as three kernels: identical bits, identical
+    floor / fallback counters, on a config-2 type batch (supersonic, floors active after a few steps)"""
+    U, B, dh = small_batch(5, g=4, dtype=np.float32)
+    kw = dict(N=16, g=4, scheme=1, recon=1, riemann=1, limvar=1, prec=0, max_groups=5)
+    fused = GU.GpuRunner(**kw)
+    a = fused(U, B, 2e-3, dh)
+    monkeypatch.setenv("MHD_NO_FUSED_PASS1", "1")
+    staged = GU.GpuRunner(**kw)
+    b = staged(U, B, 2e-3, dh)
+    monkeypatch.delenv("MHD_NO_FUSED_PASS1")
+    for k in ("U", "B", "flux", "emf"):
+        assert np.array_equal(a[k], b[k]), k
+    assert fused.stats() == staged.stats()
+    assert fused.solver.launch_count() < staged.solver.launch_count()      # and it really is another launch sequence
+
+
 @pytest.mark.parametrize("which,prec", [("abc", 1), ("abc", 0), ("blast", 1)])
 def test_configs_3_4_full_size_256_cubed_on_sampled_groups(oracle, which, prec):
     """BASELINE.json configs 3 / 4 at full size: 256^3 -> 4096 groups of 16^3 (g = 4), CTU+PPM+HLLD+CT, one step through
