@@ -221,8 +221,10 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
     if constexpr (SC == 25 && sizeof(R) == 4) {
       fused1 = N == 16 && g == 4 && s->cfg.recon == MHD_PPM && lim == 1 && sol == MHD_HLLD && !s->no_fused_pass1;
       if (fused1) {
-        const size_t shm = (size_t)21 * kP1Threads * sizeof(R);
-        LAUNCH(ST_PASS1, (k_ctu_pass1<R, kHLLD, 1, SC><<<dim3(kP1Across, 3, ng), kP1Threads, shm, st>>>(p)));
+        constexpr int ACROSS = kP1Across;
+        const size_t shm = (size_t)21 * kP1Along * ACROSS * sizeof(R);
+        const dim3 grd(kP1Across * (kP1Across / ACROSS), 3, ng);
+        LAUNCH(ST_PASS1, (k_ctu_pass1<R, kHLLD, 1, ACROSS, SC><<<grd, kP1Along * ACROSS, shm, st>>>(p)));
       }
     }
     if (!fused1) {

@@ -10,8 +10,10 @@
 // from shared memory and its right state from registers.  Same device functions as the staged kernels, same operands;
 // the values that the staged path rounds by storing them (slopes, states) pass through an empty asm here, so that no
 // multiply of one stage is contracted with an add of the next: bitwise the same result as the staged kernels.
-// Measured (B200, 512 groups): FP32 HLLD 0.79 ms against 1.14 ms for the three kernels; FP64 and Roe need more than the
-// 68 registers two resident blocks leave and are no faster with one block, so they keep the staged path.
+// Measured (B200, 512 groups): FP32 HLLD 0.79 ms against 1.14 ms for the three kernels.  FP64 and Roe need more than the
+// 68 registers two resident blocks leave: FP32 Roe with one block 1.29 ms (staged 1.29); FP64 HLLD with one 480-thread
+// block 2.18 ms, with two half-plane blocks (ACROSS = 10) 2.01 ms against 2.15 ms staged -- and the FP64 build was not
+// bitwise equal to the staged kernels, so FP64 and Roe keep the staged path.
 #pragma once
 #include "mhd_kernels2.cuh"
 
@@ -22,18 +24,19 @@ __device__ __forceinline__ void opaque(double& x) { asm volatile("" : "+d"(x)); 
 
 constexpr int kP1Along = 24;                       // cells along D: the whole tile, T = 24
 constexpr int kP1Across = 20;                      // cells across: g-2 .. g+N+1
-constexpr int kP1Threads = kP1Along * kP1Across;   // 480
+// a block covers ACROSS of the 20 cells across (20: the whole plane, 480 threads; 10: half of it, 240 threads)
 
-template <class R, int SOLVER, int LIM, int D, class KP>
-__device__ __forceinline__ void ctu_pass1_plane(const KP& p, R* __restrict__ sm, int grp, int plane) {
+template <class R, int SOLVER, int LIM, int ACROSS, int D, class KP>
+__device__ __forceinline__ void ctu_pass1_plane(const KP& p, R* __restrict__ sm, int grp, int plane, int part) {
   constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
-  constexpr int sD = D == 0 ? 1 : kP1Across;       // distance of the neighbour along D in the block
+  constexpr int kP1Threads = kP1Along * ACROSS;
+  constexpr int sD = D == 0 ? 1 : ACROSS;          // distance of the neighbour along D in the block
   const int t = threadIdx.x;
   const int g = p.g, lo = g - 1;
   // a: index along D (0 .. 23 <-> tile cell a), b: in-plane index across, plane: the third axis
   int a, b;
-  if (D == 0) { a = t % kP1Along; b = t / kP1Along; } else { b = t % kP1Across; a = t / kP1Across; }
-  const int ta = lo - 1 + b, tp = lo - 1 + plane;  // tile indices across / of the plane
+  if (D == 0) { a = t % kP1Along; b = t / kP1Along; } else { b = t % ACROSS; a = t / ACROSS; }
+  const int ta = lo - 1 + part * ACROSS + b, tp = lo - 1 + plane;  // tile indices across / of the plane
   const int i = D == 0 ? a : ta, j = D == 1 ? a : (D == 0 ? ta : tp), k = D == 2 ? a : tp;
   const int S = p.S, S2 = p.S2, S3 = p.S3;
   const int q = (k * S + j) * S + i;
@@ -98,18 +101,20 @@ __device__ __forceinline__ void ctu_pass1_plane(const KP& p, R* __restrict__ sm,
   }
 }
 
-// grid: (20 planes, 3 directions, groups); 480 threads; dynamic shared memory 21 * 480 * sizeof(R)
-// two resident 480-thread blocks per SM: 68 registers per thread, enough for FP32 HLLD (64, no spill)
-template <class R, int SOLVER> struct OccPass1 { static constexpr int minb = (sizeof(R) == 4 && SOLVER != kROE) ? 2 : 1; };
+// grid: (20 planes x 20 / ACROSS parts, 3 directions, groups); 24 * ACROSS threads; dynamic shared memory 21 * threads * sizeof(R)
+// resident blocks per SM asked from ptxas: FP32 HLLD fits the 68 registers that two 480-thread blocks leave (64, no spill)
+template <class R, int SOLVER> struct OccPass1 { static constexpr int minb = sizeof(R) == 4 ? 2 : 1; };
 
-template <class R, int SOLVER, int LIM, int SC>
-__global__ void __launch_bounds__(kP1Threads, OccPass1<R, SOLVER>::minb) k_ctu_pass1(const KParamsSC<R, SC> p) {
+template <class R, int SOLVER, int LIM, int ACROSS, int SC>
+__global__ void __launch_bounds__(kP1Along * ACROSS, OccPass1<R, SOLVER>::minb) k_ctu_pass1(const KParamsSC<R, SC> p) {
   extern __shared__ unsigned char smem_raw[];
   R* sm = reinterpret_cast<R*>(smem_raw);
+  constexpr int parts = kP1Across / ACROSS;
+  const int plane = blockIdx.x / parts, part = blockIdx.x - plane * parts;
   switch (blockIdx.y) {
-    case 0: ctu_pass1_plane<R, SOLVER, LIM, 0>(p, sm, blockIdx.z, blockIdx.x); break;
-    case 1: ctu_pass1_plane<R, SOLVER, LIM, 1>(p, sm, blockIdx.z, blockIdx.x); break;
-    default: ctu_pass1_plane<R, SOLVER, LIM, 2>(p, sm, blockIdx.z, blockIdx.x); break;
+    case 0: ctu_pass1_plane<R, SOLVER, LIM, ACROSS, 0>(p, sm, blockIdx.z, plane, part); break;
+    case 1: ctu_pass1_plane<R, SOLVER, LIM, ACROSS, 1>(p, sm, blockIdx.z, plane, part); break;
+    default: ctu_pass1_plane<R, SOLVER, LIM, ACROSS, 2>(p, sm, blockIdx.z, plane, part); break;
   }
 }
 
