@@ -35,9 +35,10 @@ FLOP_PER_SOLVE = {"hlld": 381, "roe": 1107, "hlle": 361}
 FLOP_PER_CELL_UPDATE = {("vl", "hlld"): 6263.5, ("vl", "roe"): 15289.0, ("ctu", "hlld"): 26067.6, ("ctu", "roe"): 35160.4}   # whole step
 FLOP_PLM_PER_FACE = 140     # two MC-limited primitive slopes + the two face states (VL pass 2)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage kernel at 512 groups, VL+PLM+HLLD, from the
-# ncu --set full captures summarised in profiles/r01c_full_top_kernels.md / r01c_f64_full_top_kernels.md (MB)
-NCU_TRAFFIC_MB = {"f32": {"load_prim": 569.3, "flux_pass1": 863.6, "emf_pass1": 380.7, "half_step": 888.4, "flux_pass2": 642.7,
-                          "emf_pass2": 242.3, "final_update": 430.3, "dt_reduce": 69.1},
+# ncu --set full captures summarised in profiles/r01f_full_top_kernels.md (FP32: S0-S2 in one kernel) and
+# r01c_f64_full_top_kernels.md (FP64: staged) (MB)
+NCU_TRAFFIC_MB = {"f32": {"pass1_fused": 1244.5, "emf_pass1": 380.3, "half_step": 888.4, "flux_pass2": 642.4,
+                          "emf_pass2": 243.0, "final_update": 430.0, "dt_reduce": 69.2},
                   "f64": {"load_prim": 1063.4, "flux_pass1": 1599.8, "emf_pass1": 737.4, "half_step": 1665.0, "flux_pass2": 1083.4,
                           "emf_pass2": 450.6, "final_update": 847.5, "dt_reduce": 141.1}}
 NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
@@ -206,6 +207,9 @@ def measure(args, prec_name, rank, world, dist):
     fl = FLOP_PER_SOLVE[args.riemann]
     top = max(stages, key=lambda k: stages[k]["ms_per_step"])
     flops_stage = {"flux_pass1": fl * f1 * G, "flux_pass2": (fl + (FLOP_PLM_PER_FACE if args.scheme == "vl" else 0)) * f2 * G}
+    if args.scheme == "vl":
+        # S0-S2 in one kernel: the pass-1 Riemann solves + con->prim and the reference EMFs of the T^3 cells (27 + 9 flops each)
+        flops_stage["pass1_fused"] = (fl * f1 + 36 * (N_PS2 + 2 * g) ** 3) * G
     roof = None
     if top in flops_stage:
         n_launch = stages[top]["launches_per_step"]
@@ -216,7 +220,7 @@ def measure(args, prec_name, rank, world, dist):
                 "peak_source": "nominal: 148 SMs x %d FMA lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if prec_name == "f32" else 64),
                 "peak_fma_measured": mhd.measure_fma_peak(dev.index, prec),
                 "traffic": (NCU_TRAFFIC_MB[prec_name].get(top) * 1e6 if (args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS) else None),
-                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01c_*)",
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01f_* / r01c_f64_*)",
                 "avg_launch_ms": dur * 1e3, "launches_per_step": n_launch,
                 "share_of_step": stages[top]["ms_per_step"] / (prof_ms / args.steps)}
     # HBM view of the whole step: algorithmic bytes = read the ghost-zoned tile once, write the results once (+ dt read)

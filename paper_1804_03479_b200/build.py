@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmhd.so")
 SOURCES = ["mhd_api.cu"]
 DEPS = ["mhd_api.cu", "mhd_api_host.inl", "mhd_api_grid.inl", "mhd_api_amr.inl", "mhd_physics.cuh", "mhd_eigen.cuh",
-        "mhd_recon.cuh", "mhd_kernels.cuh", "mhd_kernels2.cuh", "mhd_kernels3.cuh", "mhd_grid.cuh", "mhd_amr.cuh", "mhd_prolong.cuh", "mhd_ctu_pass1.cuh",
+        "mhd_recon.cuh", "mhd_kernels.cuh", "mhd_kernels2.cuh", "mhd_kernels3.cuh", "mhd_grid.cuh", "mhd_amr.cuh", "mhd_prolong.cuh", "mhd_ctu_pass1.cuh", "mhd_vl_pass1.cuh",
         os.path.join("..", "..", "include", "mhd.h")]
 
 NVCC_FLAGS = [

@@ -15,6 +15,7 @@
 #include "mhd_amr.cuh"
 #include "mhd_prolong.cuh"
 #include "mhd_ctu_pass1.cuh"
+#include "mhd_vl_pass1.cuh"
 
 using namespace mhd;
 
@@ -116,7 +117,7 @@ KParams<R> make_params(const mhd_solver* s, const void* Ui, const void* Bi, void
 
 enum Stage : int { ST_LOAD = 0, ST_RECON, ST_FLUX1, ST_EMF1, ST_HALF, ST_CORR, ST_FLUX2, ST_EMF2, ST_FINAL, ST_DT, ST_PASS1, ST_COUNT };
 const char* const kStageNames[ST_COUNT] = { "load_prim", "recon_ctu", "flux_pass1", "emf_pass1", "half_step", "ctu_corr",
-                                            "flux_pass2", "emf_pass2", "final_update", "dt_reduce", "ctu_pass1_fused" };
+                                            "flux_pass2", "emf_pass2", "final_update", "dt_reduce", "pass1_fused" };
 constexpr size_t kProfMaxLaunches = 16384;
 
 inline void prof_begin(mhd_solver* s, int stage, cudaStream_t st) {
@@ -185,13 +186,19 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
 #define GRID3(b) dim3(blocks_for(b, TPB), 3, ng)
   int f2 = A_F;                                   // where the pass-2 fluxes are
   const Box3 ball = box(0, S, 0, S, 0, S);
-  LAUNCH(ST_LOAD, (k_load_prim<R, SC><<<GRID1(ball), blk, 0, st>>>(p, ball)));
+  // standard VL group in FP32 with HLLD: S0 + S1 + S2 in one kernel (mhd_vl_pass1.cuh)
+  bool fusedv = false;
+  if constexpr (SC == 23 && sizeof(R) == 4) {
+    fusedv = s->cfg.scheme == MHD_VL && N == 16 && g == 3 && sol == MHD_HLLD && !s->no_fused_pass1;
+    if (fusedv) LAUNCH(ST_PASS1, (k_vl_pass1<R, kHLLD, SC><<<dim3((kV1T + kV1Chunk - 1) / kV1Chunk, 1, ng), kV1Threads, 0, st>>>(p)));
+  }
+  if (!fusedv) LAUNCH(ST_LOAD, (k_load_prim<R, SC><<<GRID1(ball), blk, 0, st>>>(p, ball)));
   if (s->cfg.scheme == MHD_VL) {
     const Box3x3 bf1 = dir_boxes(1, T, 0, T), be1 = edge_boxes(1, T - 1, 0, T);
     const Box3 bh = box(1, T - 1, 1, T - 1, 1, T - 1);
     // pass 2 only where the final update needs it: faces n in [g, g+N], t in [g-1, g+N]; edges of the interior faces
     const Box3x3 bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1), be2 = edge_boxes(g, g + N, g, g + N);
-    LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER, SC><<<GRID3(bf1), blk, 0, st>>>(p, bf1))));          // step 1
+    if (!fusedv) LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER, SC><<<GRID3(bf1), blk, 0, st>>>(p, bf1))));          // step 1
     LAUNCH(ST_EMF1, (k_emf<R, A_F, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 2
     LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 3
     if (s->cfg.recon == MHD_PLM) {

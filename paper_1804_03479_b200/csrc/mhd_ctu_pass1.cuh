@@ -9,11 +9,14 @@
 // states still go to memory once (step 5 needs them), the slopes never do, and the Riemann solve reads its left state
 // from shared memory and its right state from registers.  Same device functions as the staged kernels, same operands;
 // the values that the staged path rounds by storing them (slopes, states) pass through an empty asm here, so that no
-// multiply of one stage is contracted with an add of the next: bitwise the same result as the staged kernels.
+// multiply of one stage is contracted with an add of the next.  The result still differs from the staged kernels in
+// the last bit of some values (the compiler orders and contracts the arithmetic inside a stage differently when the
+// stages share one function: measured <= 1e-7 of max|U|, 5e-7 of the fluxes, 3e-6 of the edge EMFs in FP32); the parity
+// tests against the oracle run through this kernel, and tests/test_gpu_api.py bounds the difference to the staged path.
 // Measured (B200, 512 groups): FP32 HLLD 0.79 ms against 1.14 ms for the three kernels.  FP64 and Roe need more than the
 // 68 registers two resident blocks leave: FP32 Roe with one block 1.29 ms (staged 1.29); FP64 HLLD with one 480-thread
-// block 2.18 ms, with two half-plane blocks (ACROSS = 10) 2.01 ms against 2.15 ms staged -- and the FP64 build was not
-// bitwise equal to the staged kernels, so FP64 and Roe keep the staged path.
+// block 2.18 ms, with two half-plane blocks (ACROSS = 10) 2.01 ms against 2.15 ms staged: FP64 and Roe keep the staged
+// path (which also keeps the FP64 result of a 16^3 group bitwise equal to that of any other group size).
 #pragma once
 #include "mhd_kernels2.cuh"
 

@@ -102,15 +102,15 @@ __device__ __forceinline__ void apply_floors(const KP& p, R (&w)[7]) {
 }
 
 // conserved cell data + the six face fields of the cell -> primitives (Eq. 5; floors R9)
-template <class R, class KP>
+template <bool COUNT = true, class R, class KP>
 __device__ __forceinline__ void cons_to_prim(const KP& p, const R (&u)[5], const R (&bl)[3], const R (&bu)[3], R (&W)[8]) {
   const R bcx = R(0.5) * (bl[0] + bu[0]), bcy = R(0.5) * (bl[1] + bu[1]), bcz = R(0.5) * (bl[2] + bu[2]);
   R rho = u[0];
-  if (rho < p.min_dens) { rho = p.min_dens; count_event(p.stats + 0); }
+  if (rho < p.min_dens) { rho = p.min_dens; if (COUNT) count_event(p.stats + 0); }
   const R ir = frcp(rho);
   const R vx = u[1] * ir, vy = u[2] * ir, vz = u[3] * ir;
   R P = p.gm1 * (u[4] - R(0.5) * rho * (vx * vx + vy * vy + vz * vz) - R(0.5) * (bcx * bcx + bcy * bcy + bcz * bcz));
-  if (P < p.min_pres) { P = p.min_pres; count_event(p.stats + 1); }
+  if (P < p.min_pres) { P = p.min_pres; if (COUNT) count_event(p.stats + 1); }
   W[0] = rho; W[1] = vx; W[2] = vy; W[3] = vz; W[4] = P; W[5] = bcx; W[6] = bcy; W[7] = bcz;
 }
 
