@@ -84,10 +84,15 @@ __device__ __forceinline__ void ctu_pass1_plane(const KP& p, R* __restrict__ sm,
     const R s1 = hdt * w0[2] * lim_minmod(dbn, -db1), s2 = hdt * w0[3] * lim_minmod(dbn, -db2);
     wlo[5] += s1; wup[5] += s1; wlo[6] += s2; wup[6] += s2;
     apply_floors(p, wlo); apply_floors(p, wup);
+    // step 5 + 6 reads the lower state of cells g .. g+N and the upper state of cells g-1 .. g+N-1 along D, across
+    // g-1 .. g+N: only those go to memory (the pass-1 solve below takes its states from the block)
+    const bool keep = ta >= g - 1 && ta <= g + p.N && tp >= g - 1 && tp <= g + p.N;
+    const bool keep_lo = keep && a >= g && a <= g + p.N, keep_up = keep && a >= g - 1 && a <= g + p.N - 1;
 #pragma unroll
     for (int v = 0; v < 7; ++v) {
       opaque(wlo[v]); opaque(wup[v]);
-      arr(A_LO + 7 * D + v)[q] = wlo[v]; arr(A_UP + 7 * D + v)[q] = wup[v];
+      if (keep_lo) arr(A_LO + 7 * D + v)[q] = wlo[v];
+      if (keep_up) arr(A_UP + 7 * D + v)[q] = wup[v];
       sU[v * kP1Threads + t] = wup[v];
     }
   }
