@@ -200,7 +200,7 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
     const Box3x3 bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1), be2 = edge_boxes(g, g + N, g, g + N);
     if (!fusedv) LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER, SC><<<GRID3(bf1), blk, 0, st>>>(p, bf1))));          // step 1
     LAUNCH(ST_EMF1, (k_emf<R, A_F, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 2
-    LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 3
+    LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh, 1)));                                         // step 3
     if (s->cfg.recon == MHD_PLM) {
       LIM_SWITCH(lim, LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, LIM, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2)))));   // steps 4+5
     } else {
@@ -245,7 +245,7 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
       LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER, SC><<<GRID3(bf1), blk, 0, st>>>(p, bf1, A_B))));    // step 2
     }
     LAUNCH(ST_EMF1, (k_emf<R, A_F, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 3
-    LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh)));                                            // step 4
+    LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh, 0)));                                         // step 4
     LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_ctu<R, SOLVER, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2))));        // steps 5 + 6
     LAUNCH(ST_EMF2, (k_emf<R, A_F2, SC><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                               // step 7
     f2 = A_F2;

@@ -256,7 +256,7 @@ __device__ __forceinline__ void load_U_in(const KP& p, const Ctx<R, KP>& c, R (&
 
 // ---- S4: half-step state: U^{n+1/2}, b^{n+1/2} on the faces of the cells, W^{n+1/2} -------
 template <class R, int SC>
-__global__ void __launch_bounds__(256, OccHalf<R>::minb) k_half(const KParamsSC<R, SC> p, const Box3 box) {
+__global__ void __launch_bounds__(256, OccHalf<R>::minb) k_half(const KParamsSC<R, SC> p, const Box3 box, const int full) {
   typedef KParamsSC<R, SC> KP;
   Ctx<R, KP> c(p, box);
   if (!c.ok) return;
@@ -277,7 +277,13 @@ __global__ void __launch_bounds__(256, OccHalf<R>::minb) k_half(const KParamsSC<
   if (c.k == box.lo[2] + box.n[2] - 1) c.arr(A_BH + 2)[q + p.S2] = bu[2];
   R W[8];
   cons_to_prim(p, u, bl, bu, W);
-  store_prim(c, A_WH, W);
+  if (full) { store_prim(c, A_WH, W); return; }
+  // CTU: only the density and the reference EMFs of the half-step state are read later (steps 5 + 6 take the half-step
+  // normal field; the EMF kernel of step 7 takes rho and -(v x Bc))
+  c.arr(A_WH)[q] = W[0];
+  c.arr(A_EC + 0)[q] = W[3] * W[6] - W[2] * W[7];
+  c.arr(A_EC + 1)[q] = W[1] * W[7] - W[3] * W[5];
+  c.arr(A_EC + 2)[q] = W[2] * W[5] - W[1] * W[6];
 }
 
 }  // namespace mhd
