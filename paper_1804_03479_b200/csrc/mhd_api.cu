@@ -194,7 +194,8 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
   }
   if (!fusedv) LAUNCH(ST_LOAD, (k_load_prim<R, SC><<<GRID1(ball), blk, 0, st>>>(p, ball)));
   if (s->cfg.scheme == MHD_VL) {
-    const Box3x3 bf1 = dir_boxes(1, T, 0, T), be1 = edge_boxes(1, T - 1, 0, T);
+    // pass-1 edge EMFs only where the half step reads them: transverse indices 1 .. T-1, along the edge 1 .. T-2
+    const Box3x3 bf1 = dir_boxes(1, T, 0, T), be1 = edge_boxes(1, T - 1, 1, T - 1);
     const Box3 bh = box(1, T - 1, 1, T - 1, 1, T - 1);
     // pass 2 only where the final update needs it: faces n in [g, g+N], t in [g-1, g+N]; edges of the interior faces
     const Box3x3 bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1), be2 = edge_boxes(g, g + N, g, g + N);

@@ -5,7 +5,7 @@
 // block owns the x-y plane of the tile (22 x 22 cells, one thread per cell) and marches over a chunk of planes along z:
 // the primitives of the plane go to shared memory for the x- and y-neighbours, the plane below stays in registers for
 // the z-face, so every Riemann solve takes its left state from shared memory or registers and its right state from
-// registers.  The primitives are still written once (the EMF and half-step kernels need them); they are not read back.
+// registers.  Of the primitives only the density goes to memory (the EMF kernel reads it beside the reference EMFs).
 // Same device functions and operands as the staged kernels; values the staged path rounds by storing pass through an
 // empty asm (no multiply of one stage contracted with an add of the next); last-bit differences to the staged kernels
 // remain (see mhd_ctu_pass1.cuh).  Measured (B200, 512 groups, FP32 HLLD): 0.40 ms against 0.16 + 0.29 ms.
@@ -73,8 +73,11 @@ __global__ void __launch_bounds__(kV1Threads, 2) k_vl_pass1(const KParamsSC<R, S
     R W[8];
     v1_load_prim<R, true>(p, U, Bx, By, Bz, i, j, k, bl, W);
     const int q = (k * S + j) * S + i;
+    // of the primitives only the density is read again (by the EMF kernel, beside the reference EMFs): the rest of W
+    // lives in shared memory and registers for the solves below and never goes to memory
+    arr(A_W)[q] = W[0];
 #pragma unroll
-    for (int v = 0; v < 8; ++v) { arr(A_W + v)[q] = W[v]; sW[v * kV1Threads + t] = W[v]; }
+    for (int v = 0; v < 8; ++v) sW[v * kV1Threads + t] = W[v];
     arr(A_EC + 0)[q] = W[3] * W[6] - W[2] * W[7];
     arr(A_EC + 1)[q] = W[1] * W[7] - W[3] * W[5];
     arr(A_EC + 2)[q] = W[2] * W[5] - W[1] * W[6];
