@@ -219,7 +219,8 @@ def measure(args, prec_name, rank, world, dist):
         roof = {"bound": "alu", "kernel": top, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
                 "peak_source": "nominal: 148 SMs x %d FMA lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if prec_name == "f32" else 64),
                 "peak_fma_measured": mhd.measure_fma_peak(dev.index, prec),
-                "traffic": (NCU_TRAFFIC_MB[prec_name].get(top) * 1e6 if (args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS) else None),
+                "traffic": (NCU_TRAFFIC_MB[prec_name][top] * 1e6 if (args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS
+                                                                        and top in NCU_TRAFFIC_MB[prec_name]) else None),
                 "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01f_* / r01c_f64_*)",
                 "avg_launch_ms": dur * 1e3, "launches_per_step": n_launch,
                 "share_of_step": stages[top]["ms_per_step"] / (prof_ms / args.steps)}
@@ -227,7 +228,7 @@ def measure(args, prec_name, rank, world, dist):
     sz = solver.sizes()
     bytes_step = (sz["n_U_in"] + sz["n_B_in"] + sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]
                   + sz["n_U_out"] + sz["n_B_out"]) * esz * G
-    if args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS:
+    if args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS and set(stages) == set(NCU_TRAFFIC_MB[prec_name]):
         tot = sum(NCU_TRAFFIC_MB[prec_name].values()) * 1e6
         res["dram_traffic"] = {"bytes_per_step_ncu": tot, "GBs": tot / 1e9 / (res["ms_per_step"] * 1e-3),
                                "frac_of_hbm_peak": tot / 1e9 / (res["ms_per_step"] * 1e-3) / hbm_peak()[0],

@@ -188,7 +188,7 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
   const Box3 ball = box(0, S, 0, S, 0, S);
   // standard VL group in FP32 with HLLD: S0 + S1 + S2 in one kernel (mhd_vl_pass1.cuh)
   bool fusedv = false;
-  if constexpr (SC == 23 && sizeof(R) == 4) {
+  if constexpr (SC == 23) {
     fusedv = s->cfg.scheme == MHD_VL && N == 16 && g == 3 && sol == MHD_HLLD && !s->no_fused_pass1;
     if (fusedv) LAUNCH(ST_PASS1, (k_vl_pass1<R, kHLLD, SC><<<dim3((kV1T + kV1Chunk - 1) / kV1Chunk, 1, ng), kV1Threads, 0, st>>>(p)));
   }

@@ -15,8 +15,7 @@
 // tests against the oracle run through this kernel, and tests/test_gpu_api.py bounds the difference to the staged path.
 // Measured (B200, 512 groups): FP32 HLLD 0.79 ms against 1.14 ms for the three kernels.  FP64 and Roe need more than the
 // 68 registers two resident blocks leave: FP32 Roe with one block 1.29 ms (staged 1.29); FP64 HLLD with one 480-thread
-// block 2.18 ms, with two half-plane blocks (ACROSS = 10) 2.01 ms against 2.15 ms staged: FP64 and Roe keep the staged
-// path (which also keeps the FP64 result of a 16^3 group bitwise equal to that of any other group size).
+// block 2.18 ms, with two half-plane blocks (ACROSS = 10) 2.01 ms against 2.15 ms staged: FP64 and Roe keep the staged path.
 #pragma once
 #include "mhd_kernels2.cuh"
 

@@ -8,7 +8,8 @@
 // registers.  Of the primitives only the density goes to memory (the EMF kernel reads it beside the reference EMFs).
 // Same device functions and operands as the staged kernels; values the staged path rounds by storing pass through an
 // empty asm (no multiply of one stage contracted with an add of the next); last-bit differences to the staged kernels
-// remain (see mhd_ctu_pass1.cuh).  Measured (B200, 512 groups, FP32 HLLD): 0.40 ms against 0.16 + 0.29 ms.
+// remain (see mhd_ctu_pass1.cuh).  Measured (B200, 512 groups, HLLD): FP32 0.32 ms against 0.16 + 0.29 ms for
+// k_load_prim + k_flux1_vl, FP64 0.69 ms against 0.30 + 0.56 ms.
 #pragma once
 #include "mhd_ctu_pass1.cuh"
 
@@ -53,10 +54,13 @@ __device__ __forceinline__ void v1_load_prim(const KP& p, const R* __restrict__ 
 // grid: (ceil(22 / kV1Chunk) chunks, 1, groups); 484 threads; static shared memory 2 x 8 x 484 values.
 // (Tried: staging the next plane's 11 inputs per thread through shared memory with cp.async while the solves run --
 // slower, 0.46 against 0.39 ms: eleven 4-byte asynchronous copies per thread cost more than the latency they hide.)
+// FP32: two resident blocks (64 registers), the plane buffer double-buffered (one barrier per plane); FP64: one block (up
+// to 128 registers), a single buffer inside the 48 KB of static shared memory and a second barrier per plane
 template <class R, int SOLVER, int SC>
-__global__ void __launch_bounds__(kV1Threads, 2) k_vl_pass1(const KParamsSC<R, SC> p) {
+__global__ void __launch_bounds__(kV1Threads, sizeof(R) == 4 ? 2 : 1) k_vl_pass1(const KParamsSC<R, SC> p) {
   constexpr int T = kV1T;
-  __shared__ R sWbuf[2 * 8 * kV1Threads];
+  constexpr int NBUF = sizeof(R) == 4 ? 2 : 1;
+  __shared__ R sWbuf[NBUF * 8 * kV1Threads];
   const int t = threadIdx.x, i = t % T, j = t / T, grp = blockIdx.z;
   const int k0 = blockIdx.x * kV1Chunk, k1 = min(k0 + kV1Chunk, T);
   const int S = p.S, S3 = p.S3;
@@ -69,7 +73,7 @@ __global__ void __launch_bounds__(kV1Threads, 2) k_vl_pass1(const KParamsSC<R, S
   R Wp[8], bl[3];
   if (k0 > 0) v1_load_prim<R, false>(p, U, Bx, By, Bz, i, j, k0 - 1, bl, Wp);     // plane below the chunk: primitives only
   for (int k = k0; k < k1; ++k) {
-    R* sW = sWbuf + (k & 1) * 8 * kV1Threads;
+    R* sW = sWbuf + (NBUF == 2 ? (k & 1) : 0) * 8 * kV1Threads;
     R W[8];
     v1_load_prim<R, true>(p, U, Bx, By, Bz, i, j, k, bl, W);
     const int q = (k * S + j) * S + i;
@@ -104,6 +108,7 @@ __global__ void __launch_bounds__(kV1Threads, 2) k_vl_pass1(const KParamsSC<R, S
     }
 #pragma unroll
     for (int v = 0; v < 8; ++v) Wp[v] = W[v];
+    if (NBUF == 1) __syncthreads();        // single buffer: everybody has read plane k before it is overwritten
   }
 }
 

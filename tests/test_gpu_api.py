@@ -99,17 +99,27 @@ def test_uniform_state_is_a_fixed_point_on_the_gpu(prec):
         assert gpu.stats() == (0, 0, 0)
 
 
-def test_decomposition_is_bitwise_on_the_gpu():
-    """P9 on the device: 32^3 advanced as one group of 32^3 and as 8 groups of 16^3 gives the same bits."""
+def test_decomposition_is_bitwise_on_the_gpu(monkeypatch):
+    """P9 on the device: 32^3 advanced as one group of 32^3 and as 8 groups of 16^3.  With the staged kernels for both
+    (MHD_NO_FUSED_PASS1) the bits are the same; the standard 16^3 group normally runs its first pass in the fused kernels
+    (csrc/mhd_vl_pass1.cuh, mhd_ctu_pass1.cuh), which agree with the staged ones to rounding: 1e-13 in FP64 (a ghost-width
+    or tile-logic error would show at 1e-3)."""
     n = 32
     U, bx, by, bz, dh = inputs.random_group_grid(n, 5)
     dt = 0.2 * dh
     for scheme, recon, g in ((0, 0, 3), (1, 1, 4)):
         a = H.step_grid(GU.GpuRunner(N=32, g=g, scheme=scheme, recon=recon, max_groups=1), U, bx, by, bz, dt, dh, 32, g)
-        b = H.step_grid(GU.GpuRunner(N=16, g=g, scheme=scheme, recon=recon, max_groups=8), U, bx, by, bz, dt, dh, 16, g)
+        monkeypatch.setenv("MHD_NO_FUSED_PASS1", "1")
+        staged = GU.GpuRunner(N=16, g=g, scheme=scheme, recon=recon, max_groups=8)
+        monkeypatch.delenv("MHD_NO_FUSED_PASS1")
+        b = H.step_grid(staged, U, bx, by, bz, dt, dh, 16, g)
         for x, y in zip(a[:4], b[:4]):
             assert np.array_equal(x, y)
         assert b[5] == 0.0
+        c = H.step_grid(GU.GpuRunner(N=16, g=g, scheme=scheme, recon=recon, max_groups=8), U, bx, by, bz, dt, dh, 16, g)
+        for x, y in zip(a[:4], c[:4]):
+            assert np.abs(x - y).max() <= 1e-13 * np.abs(x).max()
+        assert c[5] == 0.0                      # faces shared by two groups: bitwise equal with the fused kernels too
 
 
 @pytest.mark.parametrize("prec", [1, 0])
