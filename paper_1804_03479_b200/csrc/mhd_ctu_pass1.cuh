@@ -13,9 +13,10 @@
 // the last bit of some values (the compiler orders and contracts the arithmetic inside a stage differently when the
 // stages share one function: measured <= 1e-7 of max|U|, 5e-7 of the fluxes, 3e-6 of the edge EMFs in FP32); the parity
 // tests against the oracle run through this kernel, and tests/test_gpu_api.py bounds the difference to the staged path.
-// Measured (B200, 512 groups): FP32 HLLD 0.79 ms against 1.14 ms for the three kernels.  FP64 and Roe need more than the
-// 68 registers two resident blocks leave: FP32 Roe with one block 1.29 ms (staged 1.29); FP64 HLLD with one 480-thread
-// block 2.18 ms, with two half-plane blocks (ACROSS = 10) 2.01 ms against 2.15 ms staged: FP64 and Roe keep the staged path.
+// Measured (B200, 512 groups, HLLD): FP32 0.74 ms against 1.14 ms for the three kernels (two resident 480-thread blocks, 64
+// registers); FP64 1.95 ms against 2.16 ms with half-plane blocks (240 threads, two resident, 128 registers; one 480-thread
+// block: 2.18 ms).  Roe needs ~110 FP32 registers: 1.29 ms fused with one block against 1.29 ms staged -- Roe, other
+// limiters, PLM and other group sizes keep the staged kernels.
 #pragma once
 #include "mhd_kernels2.cuh"
 
@@ -109,8 +110,9 @@ __device__ __forceinline__ void ctu_pass1_plane(const KP& p, R* __restrict__ sm,
 }
 
 // grid: (20 planes x 20 / ACROSS parts, 3 directions, groups); 24 * ACROSS threads; dynamic shared memory 21 * threads * sizeof(R)
-// resident blocks per SM asked from ptxas: FP32 HLLD fits the 68 registers that two 480-thread blocks leave (64, no spill)
-template <class R, int SOLVER> struct OccPass1 { static constexpr int minb = sizeof(R) == 4 ? 2 : 1; };
+// resident blocks per SM asked from ptxas: FP32 HLLD fits the 68 registers that two 480-thread blocks leave (64, no
+// spill); FP64 runs half planes (240 threads), two resident blocks with up to 128 registers
+template <class R, int SOLVER> struct OccPass1 { static constexpr int minb = 2; };
 
 template <class R, int SOLVER, int LIM, int ACROSS, int SC>
 __global__ void __launch_bounds__(kP1Along * ACROSS, OccPass1<R, SOLVER>::minb) k_ctu_pass1(const KParamsSC<R, SC> p) {
