@@ -35,12 +35,11 @@ FLOP_PER_SOLVE = {"hlld": 381, "roe": 1107, "hlle": 361}
 FLOP_PER_CELL_UPDATE = {("vl", "hlld"): 6263.5, ("vl", "roe"): 15289.0, ("ctu", "hlld"): 26067.6, ("ctu", "roe"): 35160.4}   # whole step
 FLOP_PLM_PER_FACE = 140     # two MC-limited primitive slopes + the two face states (VL pass 2)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage kernel at 512 groups, VL+PLM+HLLD, from the
-# ncu --set full captures summarised in profiles/r01f_full_top_kernels.md (FP32: S0-S2 in one kernel) and
-# r01c_f64_full_top_kernels.md (FP64: staged) (MB)
-NCU_TRAFFIC_MB = {"f32": {"pass1_fused": 1244.5, "emf_pass1": 380.3, "half_step": 888.4, "flux_pass2": 642.4,
-                          "emf_pass2": 243.0, "final_update": 430.0, "dt_reduce": 69.2},
-                  "f64": {"load_prim": 1063.4, "flux_pass1": 1599.8, "emf_pass1": 737.4, "half_step": 1665.0, "flux_pass2": 1083.4,
-                          "emf_pass2": 450.6, "final_update": 847.5, "dt_reduce": 141.1}}
+# ncu --set full captures summarised in profiles/r01g_full_top_kernels.md and r01g_f64_full_top_kernels.md (MB)
+NCU_TRAFFIC_MB = {"f32": {"pass1_fused": 1007.8, "emf_pass1": 364.6, "half_step": 888.4, "flux_pass2": 643.7,
+                          "emf_pass2": 242.5, "final_update": 429.6, "dt_reduce": 69.2},
+                  "f64": {"pass1_fused": 1796.3, "emf_pass1": 705.4, "half_step": 1665.3, "flux_pass2": 1082.9,
+                          "emf_pass2": 450.3, "final_update": 848.4, "dt_reduce": 141.2}}
 NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
 
 
@@ -221,7 +220,7 @@ def measure(args, prec_name, rank, world, dist):
                 "peak_fma_measured": mhd.measure_fma_peak(dev.index, prec),
                 "traffic": (NCU_TRAFFIC_MB[prec_name][top] * 1e6 if (args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS
                                                                         and top in NCU_TRAFFIC_MB[prec_name]) else None),
-                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01f_* / r01c_f64_*)",
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01g_*)",
                 "avg_launch_ms": dur * 1e3, "launches_per_step": n_launch,
                 "share_of_step": stages[top]["ms_per_step"] / (prof_ms / args.steps)}
     # HBM view of the whole step: algorithmic bytes = read the ghost-zoned tile once, write the results once (+ dt read)

@@ -223,13 +223,13 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
     const Box3 bh = box(lo, hi, lo, hi, lo, hi);
     const Box3x3 bco = dir_boxes(g - 1, g + N + 1, g - 1, g + N + 1), bf2 = dir_boxes(g, g + N + 1, g - 1, g + N + 1);
     const Box3x3 be2 = edge_boxes(g, g + N, g, g + N);
-    // standard patch group with PPM, MC limiter in characteristic variables and HLLD: steps 1 + 2 in one kernel
+    // standard patch group in FP32 with PPM, MC limiter in characteristic variables and HLLD: steps 1 + 2 in one kernel
     // (mhd_ctu_pass1.cuh); everything else: slopes -> states -> Riemann solve as three kernels
     bool fused1 = false;
-    if constexpr (SC == 25) {
+    if constexpr (SC == 25 && sizeof(R) == 4) {
       fused1 = N == 16 && g == 4 && s->cfg.recon == MHD_PPM && lim == 1 && sol == MHD_HLLD && !s->no_fused_pass1;
       if (fused1) {
-        constexpr int ACROSS = sizeof(R) == 4 ? kP1Across : kP1Across / 2;      // FP64: half planes, 240 threads
+        constexpr int ACROSS = kP1Across;
         const size_t shm = (size_t)21 * kP1Along * ACROSS * sizeof(R);
         const dim3 grd(kP1Across * (kP1Across / ACROSS), 3, ng);
         LAUNCH(ST_PASS1, (k_ctu_pass1<R, kHLLD, 1, ACROSS, SC><<<grd, kP1Along * ACROSS, shm, st>>>(p)));

@@ -14,9 +14,9 @@
 // stages share one function: measured <= 1e-7 of max|U|, 5e-7 of the fluxes, 3e-6 of the edge EMFs in FP32); the parity
 // tests against the oracle run through this kernel, and tests/test_gpu_api.py bounds the difference to the staged path.
 // Measured (B200, 512 groups, HLLD): FP32 0.74 ms against 1.14 ms for the three kernels (two resident 480-thread blocks, 64
-// registers); FP64 1.95 ms against 2.16 ms with half-plane blocks (240 threads, two resident, 128 registers; one 480-thread
-// block: 2.18 ms).  Roe needs ~110 FP32 registers: 1.29 ms fused with one block against 1.29 ms staged -- Roe, other
-// limiters, PLM and other group sizes keep the staged kernels.
+// registers).  FP64 needs 128 registers: one 480-thread block 2.18 ms, two half-plane blocks (ACROSS = 10) 1.95 ms on one
+// box and 2.15 ms on another against 2.16 ms staged; Roe needs ~110 FP32 registers: 1.29 ms against 1.29 ms staged.
+// FP64, Roe, other limiters, PLM and other group sizes keep the staged kernels.
 #pragma once
 #include "mhd_kernels2.cuh"
 
@@ -110,8 +110,7 @@ __device__ __forceinline__ void ctu_pass1_plane(const KP& p, R* __restrict__ sm,
 }
 
 // grid: (20 planes x 20 / ACROSS parts, 3 directions, groups); 24 * ACROSS threads; dynamic shared memory 21 * threads * sizeof(R)
-// resident blocks per SM asked from ptxas: FP32 HLLD fits the 68 registers that two 480-thread blocks leave (64, no
-// spill); FP64 runs half planes (240 threads), two resident blocks with up to 128 registers
+// resident blocks per SM asked from ptxas: FP32 HLLD fits the 68 registers that two 480-thread blocks leave (64, no spill)
 template <class R, int SOLVER> struct OccPass1 { static constexpr int minb = 2; };
 
 template <class R, int SOLVER, int LIM, int ACROSS, int SC>
