@@ -186,11 +186,15 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
 #define GRID3(b) dim3(blocks_for(b, TPB), 3, ng)
   int f2 = A_F;                                   // where the pass-2 fluxes are
   const Box3 ball = box(0, S, 0, S, 0, S);
-  // standard VL group in FP32 with HLLD: S0 + S1 + S2 in one kernel (mhd_vl_pass1.cuh)
+  // standard VL group with HLLD or Roe: S0 + S1 + S2 in one kernel (mhd_vl_pass1.cuh)
   bool fusedv = false;
   if constexpr (SC == 23) {
-    fusedv = s->cfg.scheme == MHD_VL && N == 16 && g == 3 && sol == MHD_HLLD && !s->no_fused_pass1;
-    if (fusedv) LAUNCH(ST_PASS1, (k_vl_pass1<R, kHLLD, SC><<<dim3((kV1T + kV1Chunk - 1) / kV1Chunk, 1, ng), kV1Threads, 0, st>>>(p)));
+    fusedv = s->cfg.scheme == MHD_VL && N == 16 && g == 3 && sol != MHD_HLLE && !s->no_fused_pass1;
+    const dim3 gv((kV1T + kV1Chunk - 1) / kV1Chunk, 1, ng);
+    if (fusedv && sol == MHD_HLLD) LAUNCH(ST_PASS1, (k_vl_pass1<R, kHLLD, SC><<<gv, kV1Threads, 0, st>>>(p)));
+    if constexpr (sizeof(R) == 4) {      // Roe in FP64 spills at 128 registers: 2.30 ms against 2.17 ms staged
+      if (fusedv && sol == MHD_ROE) LAUNCH(ST_PASS1, (k_vl_pass1<R, kROE, SC><<<gv, kV1Threads, 0, st>>>(p)));
+    } else if (sol == MHD_ROE) fusedv = false;
   }
   if (!fusedv) LAUNCH(ST_LOAD, (k_load_prim<R, SC><<<GRID1(ball), blk, 0, st>>>(p, ball)));
   if (s->cfg.scheme == MHD_VL) {

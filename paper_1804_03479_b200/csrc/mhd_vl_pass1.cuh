@@ -9,7 +9,8 @@
 // Same device functions and operands as the staged kernels; values the staged path rounds by storing pass through an
 // empty asm (no multiply of one stage contracted with an add of the next); last-bit differences to the staged kernels
 // remain (see mhd_ctu_pass1.cuh).  Measured (B200, 512 groups, HLLD): FP32 0.32 ms against 0.16 + 0.29 ms for
-// k_load_prim + k_flux1_vl, FP64 0.69 ms against 0.30 + 0.56 ms.
+// k_load_prim + k_flux1_vl, FP64 0.69 ms against 0.30 + 0.56 ms; Roe FP32 (one block, 128 registers) 0.55 ms against
+// 0.16 + 0.57 ms; Roe FP64 spills (2.30 ms against 2.17 ms) and keeps the staged kernels.
 #pragma once
 #include "mhd_ctu_pass1.cuh"
 
@@ -54,10 +55,11 @@ __device__ __forceinline__ void v1_load_prim(const KP& p, const R* __restrict__ 
 // grid: (ceil(22 / kV1Chunk) chunks, 1, groups); 484 threads; static shared memory 2 x 8 x 484 values.
 // (Tried: staging the next plane's 11 inputs per thread through shared memory with cp.async while the solves run --
 // slower, 0.46 against 0.39 ms: eleven 4-byte asynchronous copies per thread cost more than the latency they hide.)
-// FP32: two resident blocks (64 registers), the plane buffer double-buffered (one barrier per plane); FP64: one block (up
-// to 128 registers), a single buffer inside the 48 KB of static shared memory and a second barrier per plane
+// FP32 HLLD: two resident blocks (64 registers), the plane buffer double-buffered (one barrier per plane); FP64 and Roe:
+// one block (up to 128 registers); FP64 with a single buffer inside the 48 KB of static shared memory and a second
+// barrier per plane
 template <class R, int SOLVER, int SC>
-__global__ void __launch_bounds__(kV1Threads, sizeof(R) == 4 ? 2 : 1) k_vl_pass1(const KParamsSC<R, SC> p) {
+__global__ void __launch_bounds__(kV1Threads, (sizeof(R) == 4 && SOLVER != kROE) ? 2 : 1) k_vl_pass1(const KParamsSC<R, SC> p) {
   constexpr int T = kV1T;
   constexpr int NBUF = sizeof(R) == 4 ? 2 : 1;
   __shared__ R sWbuf[NBUF * 8 * kV1Threads];
