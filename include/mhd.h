@@ -97,6 +97,15 @@ int mhd_advance_host(mhd_solver* s, const void* U_in, const void* B_in, void* U_
 int mhd_dt_reduce(mhd_solver* s, const void* U, const void* B, int ngroups, int nghost_of_arrays,
                   double dh, double cfl, double* dt_out, double* maxspeed_out, void* cuda_stream);
 
+/* mhd_advance followed by mhd_dt_reduce(U_out, B_out, ngroups, 0, dh, cfl, ...) as ONE call: the full update (S8,
+ * PAPER.md:183, :197) also evaluates the CFL speed (S9) of every cell it writes and reduces it on the
+ * device, so the new state is not read back for the time step.  Arguments as mhd_advance (DEVICE pointers) plus cfl;
+ * dt_out (required) and maxspeed_out (nullable) are HOST pointers.  Results (outputs, dt, maxspeed) are bit-identical
+ * to the two separate calls.  ngroups >= 1.  Blocking: synchronises cuda_stream like mhd_dt_reduce. */
+int mhd_advance_dt(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out, void* flux_out,
+                   void* emf_out, int ngroups, double dt, double dh, double cfl, double* dt_out, double* maxspeed_out,
+                   void* cuda_stream);
+
 /* Cumulative event counters since creation (density floors, pressure floors, Roe->HLLE fallbacks).
  * Synchronises the device; asynchronous kernel faults surface here as MHD_ECUDA. */
 int mhd_get_stats(mhd_solver* s, unsigned long long* n_floor_dens, unsigned long long* n_floor_pres,

@@ -60,6 +60,7 @@ struct mhd_solver {
   cudaEvent_t fork = nullptr;
   unsigned long long* d_stats = nullptr;    // 3 counters
   unsigned long long* d_red = nullptr;      // dt reduction cell
+  unsigned long long* red_now = nullptr;    // set by mhd_advance_dt around its launches: the final update also reduces the CFL speed
   unsigned long long launches = 0;
   HostLane lanes[kMaxStreams];
   int lane_groups = 0, lane_count = 0;
@@ -89,6 +90,7 @@ KParams<R> make_params(const mhd_solver* s, const void* Ui, const void* Bi, void
   p.eout = eo ? static_cast<R*>(eo) + (size_t)first * s->nE : nullptr;
   p.ws = static_cast<R*>(ws);
   p.stats = s->d_stats;
+  p.red = s->red_now;
   p.N = s->N; p.g = s->g; p.T = s->T; p.S = s->S; p.S2 = s->S * s->S; p.S3 = (int)s->S3; p.narr = s->narr;
   p.nUi = (long long)s->nUi; p.nBi = (long long)s->nBi; p.nUo = (long long)s->nUo; p.nBo = (long long)s->nBo;
   p.nF = (long long)s->nF; p.nE = (long long)s->nE;
@@ -257,8 +259,14 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
   }
   const Box3 bin = box(g, g + N, g, g + N, g, g + N);
   const unsigned nbf = std::max(blocks_for(bin, TPB), (unsigned)((9 * (N + 1) * (N + 1) + TPB - 1) / TPB));
-  if (f2 == A_F) LAUNCH(ST_FINAL, (k_final<R, A_F, SC><<<dim3(nbf, 1, ng), blk, 0, st>>>(p, bin)));                // step 7 / 8
-  else LAUNCH(ST_FINAL, (k_final<R, A_F2, SC><<<dim3(nbf, 1, ng), blk, 0, st>>>(p, bin)));
+  const dim3 gfin(nbf, 1, ng);                                                                                   // step 7 / 8
+  if (p.red) {                                                                                                   // + S9 (mhd_advance_dt)
+    if (f2 == A_F) LAUNCH(ST_FINAL, (k_final<R, A_F, SC, true><<<gfin, blk, 0, st>>>(p, bin)));
+    else LAUNCH(ST_FINAL, (k_final<R, A_F2, SC, true><<<gfin, blk, 0, st>>>(p, bin)));
+  } else {
+    if (f2 == A_F) LAUNCH(ST_FINAL, (k_final<R, A_F, SC, false><<<gfin, blk, 0, st>>>(p, bin)));
+    else LAUNCH(ST_FINAL, (k_final<R, A_F2, SC, false><<<gfin, blk, 0, st>>>(p, bin)));
+  }
 #undef GRID1
 #undef GRID3
   CU(cudaGetLastError());
@@ -442,6 +450,29 @@ int mhd_advance(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, 
   return s->cfg.prec == MHD_FP32
              ? advance_lanes<float>(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, st)
              : advance_lanes<double>(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, st);
+}
+
+// mhd_advance with the CFL reduction (S9) of its own output fused into the final update (S8)
+int mhd_advance_dt(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out, void* flux_out,
+                   void* emf_out, int ngroups, double dt, double dh, double cfl, double* dt_out, double* maxspeed_out,
+                   void* cuda_stream) {
+  if (!s || !dt_out || ngroups < 1 || !(cfl > 0.0)) return MHD_EINVAL;
+  CU(cudaSetDevice(s->cfg.device));
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  CU(cudaMemsetAsync(s->d_red, 0, sizeof(unsigned long long), st));
+  s->red_now = s->d_red;
+  const int rc = mhd_advance(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, cuda_stream);
+  s->red_now = nullptr;
+  if (rc != MHD_OK) return rc;
+  unsigned long long bits = 0;
+  CU(cudaMemcpyAsync(&bits, s->d_red, sizeof bits, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  double smax;
+  if (s->cfg.prec == MHD_FP32) { unsigned int b32 = (unsigned int)(bits & 0xffffffffu); float f; memcpy(&f, &b32, 4); smax = f; }
+  else memcpy(&smax, &bits, 8);
+  if (maxspeed_out) *maxspeed_out = smax;
+  *dt_out = cfl * dh / smax;
+  return MHD_OK;
 }
 
 }  // extern "C"

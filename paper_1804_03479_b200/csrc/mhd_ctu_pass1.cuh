@@ -22,8 +22,7 @@
 
 namespace mhd {
 
-__device__ __forceinline__ void opaque(float& x) { asm volatile("" : "+f"(x)); }
-__device__ __forceinline__ void opaque(double& x) { asm volatile("" : "+d"(x)); }
+// opaque(): mhd_kernels.cuh
 
 constexpr int kP1Along = 24;                       // cells along D: the whole tile, T = 24
 constexpr int kP1Across = 20;                      // cells across: g-2 .. g+N+1

@@ -38,6 +38,7 @@ template <class R> struct KParams {
   R* Uout; R* Bout; R* fout; R* eout;
   R* ws;
   unsigned long long* stats;        // [0] density floors, [1] pressure floors, [2] Riemann fallbacks
+  unsigned long long* red;          // mhd_advance_dt: cell of the fused CFL reduction (bit pattern of the largest speed), else null
   int N, g, T, S, S2, S3, narr;
   long long nUi, nBi, nUo, nBo, nF, nE;
   R gam, gm1, gm1inv, dt, dh, min_dens, min_pres;
@@ -84,6 +85,10 @@ template <class R, class KP> struct Ctx {
 };
 
 __device__ __forceinline__ void count_event(unsigned long long* ctr) { atomicAdd(ctr, 1ULL); }
+
+// a value the staged path rounds by storing it: the compiler must materialise it here (no contraction across stages)
+__device__ __forceinline__ void opaque(float& x) { asm volatile("" : "+f"(x)); }
+__device__ __forceinline__ void opaque(double& x) { asm volatile("" : "+d"(x)); }
 
 // generic 1-D state of cell q for direction D from an 8-array primitive block
 template <class R, int D>

@@ -34,36 +34,24 @@ __device__ __forceinline__ void copy_planes(const KP& p, int grp, int t) {
   }
 }
 
-template <class R, int FBASE, int SC>
-__global__ void __launch_bounds__(256, OccFinal<R>::minb) k_final(const KParamsSC<R, SC> p, const Box3 box) {
-  typedef KParamsSC<R, SC> KP;
-  Ctx<R, KP> c(p, box);
-  if (p.fout || p.eout) copy_planes<R, FBASE>(p, blockIdx.z, blockIdx.x * blockDim.x + threadIdx.x);
-  if (!c.ok) return;
-  const int g = p.g, N = p.N;
-  const int ii = c.i - g, jj = c.j - g, kk = c.k - g;
-  const R qh = p.dt / p.dh;
-  R u[5], dU[5];
-  load_U_in(p, c, u);
-  flux_div<FBASE>(c, dU);
-  R* Uo = p.Uout + (size_t)c.grp * p.nUo;
-  const size_t N3 = (size_t)N * N * N, cq = ((size_t)kk * N + jj) * N + ii;
+// largest signal speed of a cell (R13) from its conserved data and its six face fields
+template <class R>
+__device__ __forceinline__ R cell_signal_speed(const R (&u)[5], const R (&bl)[3], const R (&bu)[3], R gam, R min_dens, R min_pres) {
+  const R Bc[3] = { R(0.5) * (bl[0] + bu[0]), R(0.5) * (bl[1] + bu[1]), R(0.5) * (bl[2] + bu[2]) };
+  const R rho = Num<R>::max(u[0], min_dens);
+  const R v[3] = { u[1] / rho, u[2] / rho, u[3] / rho };
+  const R b2 = Bc[0] * Bc[0] + Bc[1] * Bc[1] + Bc[2] * Bc[2];
+  R P = (gam - R(1)) * (u[4] - R(0.5) * rho * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) - R(0.5) * b2);
+  P = Num<R>::max(P, min_pres);
+  R smax = R(0);
 #pragma unroll
-  for (int v = 0; v < 5; ++v) Uo[v * N3 + cq] = u[v] - qh * dU[v];
-  R* Bx = p.Bout + (size_t)c.grp * p.nBo;
-  R* By = Bx + (size_t)N * N * (N + 1);
-  R* Bz = By + (size_t)N * N * (N + 1);
-  const int q = c.q;
-  Bx[((size_t)kk * N + jj) * (N + 1) + ii] = ct_face<R, 0>(c, c.arr(A_B + 0), q, qh);
-  By[((size_t)kk * (N + 1) + jj) * N + ii] = ct_face<R, 1>(c, c.arr(A_B + 1), q, qh);
-  Bz[((size_t)kk * N + jj) * N + ii] = ct_face<R, 2>(c, c.arr(A_B + 2), q, qh);
-  if (ii == N - 1) Bx[((size_t)kk * N + jj) * (N + 1) + N] = ct_face<R, 0>(c, c.arr(A_B + 0), q + 1, qh);
-  if (jj == N - 1) By[((size_t)kk * (N + 1) + N) * N + ii] = ct_face<R, 1>(c, c.arr(A_B + 1), q + p.S, qh);
-  if (kk == N - 1) Bz[((size_t)N * N + jj) * N + ii] = ct_face<R, 2>(c, c.arr(A_B + 2), q + p.S2, qh);
+  for (int d = 0; d < 3; ++d) {
+    const R bn2 = Bc[d] * Bc[d];
+    smax = Num<R>::max(smax, Num<R>::abs(v[d]) + fast_speed(rho, P, bn2, b2 - bn2, gam));
+  }
+  return smax;
 }
-
-// ---- S9: CFL (PAPER.md:172, :250; R13): max over interior cells and directions of |v_d| + c_f,d -------------------
-// speeds are >= 0, so their IEEE bit patterns order like unsigned integers: one atomicMax per block.
+// speeds are >= 0, so their IEEE bit patterns order like unsigned integers: one atomicMax per block
 template <class R> struct Bits;
 template <> struct Bits<float> {
   typedef unsigned int U;
@@ -73,33 +61,9 @@ template <> struct Bits<double> {
   typedef unsigned long long U;
   static __device__ __forceinline__ U enc(double x) { return (U)__double_as_longlong(x); }
 };
-
+// block of 256 threads, every thread calls
 template <class R>
-__global__ void __launch_bounds__(256) k_dt(const R* __restrict__ U, const R* __restrict__ B, int N, int ng, long long nU,
-                                            long long nB, R gam, R min_dens, R min_pres, unsigned long long* out) {
-  const int T = N + 2 * ng;
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  R smax = R(0);
-  if (t < N * N * N) {
-    const int i = t % N + ng, j = (t / N) % N + ng, k = t / (N * N) + ng;
-    const R* u = U + (size_t)blockIdx.z * nU;
-    const R* bx = B + (size_t)blockIdx.z * nB;
-    const R* by = bx + (size_t)T * T * (T + 1);
-    const R* bz = by + (size_t)T * T * (T + 1);
-    const size_t T3 = (size_t)T * T * T, cq = ((size_t)k * T + j) * T + i;
-    const size_t qx = ((size_t)k * T + j) * (T + 1) + i, qy = ((size_t)k * (T + 1) + j) * T + i;
-    const R Bc[3] = { R(0.5) * (bx[qx] + bx[qx + 1]), R(0.5) * (by[qy] + by[qy + T]), R(0.5) * (bz[cq] + bz[cq + (size_t)T * T]) };
-    const R rho = Num<R>::max(u[cq], min_dens);
-    const R v[3] = { u[T3 + cq] / rho, u[2 * T3 + cq] / rho, u[3 * T3 + cq] / rho };
-    const R b2 = Bc[0] * Bc[0] + Bc[1] * Bc[1] + Bc[2] * Bc[2];
-    R P = (gam - R(1)) * (u[4 * T3 + cq] - R(0.5) * rho * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) - R(0.5) * b2);
-    P = Num<R>::max(P, min_pres);
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      const R bn2 = Bc[d] * Bc[d];
-      smax = Num<R>::max(smax, Num<R>::abs(v[d]) + fast_speed(rho, P, bn2, b2 - bn2, gam));
-    }
-  }
+__device__ __forceinline__ void block_max_to(R smax, unsigned long long* out) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) smax = Num<R>::max(smax, __shfl_xor_sync(0xffffffffu, smax, o));
   __shared__ R red[8];
@@ -111,6 +75,76 @@ __global__ void __launch_bounds__(256) k_dt(const R* __restrict__ U, const R* __
     for (int o = 4; o > 0; o >>= 1) m = Num<R>::max(m, __shfl_xor_sync(0xffffffffu, m, o));
     if (threadIdx.x == 0) atomicMax(reinterpret_cast<typename Bits<R>::U*>(out), Bits<R>::enc(m));
   }
+}
+
+// DT (mhd_advance_dt): S9 on the cell's own new state in the same kernel -- the thread also evaluates the upper faces of
+// its cell (the same expression as the neighbour's lower face, hence the same bits) and the block reduces the speeds
+template <class R, int FBASE, int SC, bool DT>
+__global__ void __launch_bounds__(256, OccFinal<R>::minb) k_final(const KParamsSC<R, SC> p, const Box3 box) {
+  typedef KParamsSC<R, SC> KP;
+  Ctx<R, KP> c(p, box);
+  if (p.fout || p.eout) copy_planes<R, FBASE>(p, blockIdx.z, blockIdx.x * blockDim.x + threadIdx.x);
+  if (!DT && !c.ok) return;
+  R smax = R(0);
+  if (c.ok) {
+    const int g = p.g, N = p.N;
+    const int ii = c.i - g, jj = c.j - g, kk = c.k - g;
+    const R qh = p.dt / p.dh;
+    R u[5], dU[5];
+    load_U_in(p, c, u);
+    flux_div<FBASE>(c, dU);
+    R* Uo = p.Uout + (size_t)c.grp * p.nUo;
+    const size_t N3 = (size_t)N * N * N, cq = ((size_t)kk * N + jj) * N + ii;
+#pragma unroll
+    for (int v = 0; v < 5; ++v) { u[v] = u[v] - qh * dU[v]; Uo[v * N3 + cq] = u[v]; }
+    R* Bx = p.Bout + (size_t)c.grp * p.nBo;
+    R* By = Bx + (size_t)N * N * (N + 1);
+    R* Bz = By + (size_t)N * N * (N + 1);
+    const int q = c.q;
+    R bl[3], bu[3];
+    bl[0] = ct_face<R, 0>(c, c.arr(A_B + 0), q, qh);
+    bl[1] = ct_face<R, 1>(c, c.arr(A_B + 1), q, qh);
+    bl[2] = ct_face<R, 2>(c, c.arr(A_B + 2), q, qh);
+    Bx[((size_t)kk * N + jj) * (N + 1) + ii] = bl[0];
+    By[((size_t)kk * (N + 1) + jj) * N + ii] = bl[1];
+    Bz[((size_t)kk * N + jj) * N + ii] = bl[2];
+    if (DT || ii == N - 1) bu[0] = ct_face<R, 0>(c, c.arr(A_B + 0), q + 1, qh);
+    if (DT || jj == N - 1) bu[1] = ct_face<R, 1>(c, c.arr(A_B + 1), q + p.S, qh);
+    if (DT || kk == N - 1) bu[2] = ct_face<R, 2>(c, c.arr(A_B + 2), q + p.S2, qh);
+    if (ii == N - 1) Bx[((size_t)kk * N + jj) * (N + 1) + N] = bu[0];
+    if (jj == N - 1) By[((size_t)kk * (N + 1) + N) * N + ii] = bu[1];
+    if (kk == N - 1) Bz[((size_t)N * N + jj) * N + ii] = bu[2];
+    if (DT) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v) opaque(u[v]);
+#pragma unroll
+      for (int v = 0; v < 3; ++v) { opaque(bl[v]); opaque(bu[v]); }
+      smax = cell_signal_speed(u, bl, bu, p.gam, p.min_dens, p.min_pres);
+    }
+  }
+  if (DT) block_max_to(smax, p.red);
+}
+
+// ---- S9: CFL (PAPER.md:172, :250; R13): max over interior cells and directions of |v_d| + c_f,d -------------------
+template <class R>
+__global__ void __launch_bounds__(256) k_dt(const R* __restrict__ U, const R* __restrict__ B, int N, int ng, long long nU,
+                                            long long nB, R gam, R min_dens, R min_pres, unsigned long long* out) {
+  const int T = N + 2 * ng;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  R smax = R(0);
+  if (t < N * N * N) {
+    const int i = t % N + ng, j = (t / N) % N + ng, k = t / (N * N) + ng;
+    const R* u_ = U + (size_t)blockIdx.z * nU;
+    const R* bx = B + (size_t)blockIdx.z * nB;
+    const R* by = bx + (size_t)T * T * (T + 1);
+    const R* bz = by + (size_t)T * T * (T + 1);
+    const size_t T3 = (size_t)T * T * T, cq = ((size_t)k * T + j) * T + i;
+    const size_t qx = ((size_t)k * T + j) * (T + 1) + i, qy = ((size_t)k * (T + 1) + j) * T + i;
+    const R bl[3] = { bx[qx], by[qy], bz[cq] }, bu[3] = { bx[qx + 1], by[qy + T], bz[cq + (size_t)T * T] };
+    const R u[5] = { u_[cq], u_[T3 + cq], u_[2 * T3 + cq], u_[3 * T3 + cq], u_[4 * T3 + cq] };
+    smax = cell_signal_speed(u, bl, bu, gam, min_dens, min_pres);
+  }
+  block_max_to(smax, out);
 }
 
 // ---- register-only FMA chains: measured FP32 / FP64 FMA peak (ALU roofline denominator) ----------------

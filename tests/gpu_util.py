@@ -33,6 +33,17 @@ class GpuRunner:
         res = {k: (v.cpu().numpy() if v is not None else None) for k, v in out.items()}
         return res
 
+    def advance_dt(self, U_in, B_in, dt, dh, cfl):
+        """mhd_advance_dt: outputs as __call__, plus (dt_next, maxspeed)"""
+        torch = self.torch
+        G = U_in.shape[0]
+        Ui = torch.from_numpy(np.ascontiguousarray(U_in, dtype=self.dtype)).cuda()
+        Bi = torch.from_numpy(np.ascontiguousarray(B_in, dtype=self.dtype)).cuda()
+        out = self.solver.alloc_outputs(G, planes=self.planes)
+        dtn, smax = self.solver.advance_dt(Ui, Bi, out["U"], out["B"], out["flux"], out["emf"], G, dt, dh, cfl)
+        res = {k: (v.cpu().numpy() if v is not None else None) for k, v in out.items()}
+        return res, dtn, smax
+
     def dt(self, U, B, ng, dh, cfl):
         torch = self.torch
         G = U.shape[0]

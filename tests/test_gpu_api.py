@@ -141,6 +141,33 @@ def test_dt_reduce_matches_the_oracle(oracle, prec):
     assert max(per_group) == s
 
 
+@pytest.mark.parametrize("N,g,scheme,recon", [(16, 3, 0, 0), (16, 4, 1, 1), (8, 3, 0, 0), (24, 4, 1, 1)])
+@pytest.mark.parametrize("prec", [1, 0])
+def test_advance_dt_equals_advance_then_dt_reduce_bitwise(oracle, prec, N, g, scheme, recon, monkeypatch):
+    """mhd_advance_dt (S9 fused into the final update) = mhd_advance + mhd_dt_reduce on its outputs, bit for bit;
+    the reduced speed also agrees with the oracle's CFL reduction of the oracle's own new state."""
+    dtp = GU.np_dtype(prec)
+    G = 7
+    U, B, dh = small_batch(G, N=N, g=g, dtype=dtp)
+    cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon)
+    dt0, _ = oracle.dt_reduce(cfg, U.astype(np.float64), B.astype(np.float64), g, dh, 0.3)
+    for slices in (None, "3"):                       # one slice; ragged slices on concurrent lanes
+        if slices:
+            monkeypatch.setenv("MHD_SLICE_GROUPS", slices)
+        gpu = GU.GpuRunner(N=N, g=g, scheme=scheme, recon=recon, prec=prec, max_groups=G)
+        a = gpu(U, B, dt0, dh)
+        dt_a, s_a = gpu.dt(a["U"], a["B"], 0, dh, 0.3)
+        b, dt_b, s_b = gpu.advance_dt(U, B, dt0, dh, 0.3)
+        for k in ("U", "B", "flux", "emf"):
+            assert np.array_equal(a[k], b[k]), k
+        assert s_a == s_b and dt_a == dt_b
+    ref = oracle.advance(cfg, U.astype(np.float64), B.astype(np.float64), dt0, dh)
+    ref_dt, ref_s = oracle.dt_reduce(cfg, ref["U"], ref["B"], 0, dh, 0.3)
+    assert abs(s_b - ref_s) <= (1e-11 if prec == 1 else 1e-4) * ref_s
+    with pytest.raises(gpu.mhd.MHDError):            # no groups: the time step is undefined
+        gpu.solver.advance_dt(None, None, None, None, None, None, 0, dt0, dh, 0.3)
+
+
 @pytest.mark.parametrize("prec", [1, 0])
 @pytest.mark.parametrize("chunk,nstreams", [(4, 3), (16, 1), (5, 2)])
 def test_advance_host_equals_advance_bitwise(prec, chunk, nstreams):
