@@ -128,6 +128,11 @@ int mhd_grid_unpack(mhd_solver* s, const void* U_out, const void* B_out, int nx,
                     void* bz, void* cuda_stream);
 int mhd_grid_advance(mhd_solver* s, void* U, void* bx, void* by, void* bz, int nx, int ny, int nz, double dt, double dh,
                      void* cuda_stream);
+/* mhd_grid_advance followed by mhd_grid_dt of the new grid state as one call (the final update reduces the CFL speed,
+ * see mhd_advance_dt): the time step of the next step costs no extra pass over the grid.  dt_out (required) and
+ * maxspeed_out (nullable) are HOST pointers; bit-identical to the two separate calls; synchronises cuda_stream. */
+int mhd_grid_advance_dt(mhd_solver* s, void* U, void* bx, void* by, void* bz, int nx, int ny, int nz, double dt, double dh,
+                        double cfl, double* dt_out, double* maxspeed_out, void* cuda_stream);
 int mhd_grid_dt(mhd_solver* s, const void* U, const void* bx, const void* by, const void* bz, int nx, int ny, int nz, double dh,
                 double cfl, double* dt_out, double* maxspeed_out, void* cuda_stream);
 

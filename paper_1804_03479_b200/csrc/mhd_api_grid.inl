@@ -66,8 +66,11 @@ int mhd_grid_unpack(mhd_solver* s, const void* U_out, const void* B_out, int nx,
                                  : grid_unpack_t<double>(s, U_out, B_out, d, U, bx, by, bz, st);
 }
 
-int mhd_grid_advance(mhd_solver* s, void* U, void* bx, void* by, void* bz, int nx, int ny, int nz, double dt, double dh,
-                     void* cuda_stream) {
+}  // extern "C"
+
+// pack -> all stages -> unpack; red != nullptr: the final update also reduces the CFL speed into *red
+static int grid_advance_impl(mhd_solver* s, void* U, void* bx, void* by, void* bz, int nx, int ny, int nz, double dt, double dh,
+                             unsigned long long* red, void* cuda_stream) {
   if (!s || !U || !bx || !by || !bz) return MHD_EINVAL;
   if (!(dt > 0.0) || !(dh > 0.0) || !std::isfinite(dt) || !std::isfinite(dh)) return MHD_EINVAL;
   GridDims d;
@@ -84,6 +87,8 @@ int mhd_grid_advance(mhd_solver* s, void* U, void* bx, void* by, void* bz, int n
     s->grid_groups = G;
   }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (red) CU(cudaMemsetAsync(red, 0, sizeof(unsigned long long), st));
+  s->red_now = red;
   if (s->cfg.prec == MHD_FP32) {
     rc = grid_pack_t<float>(s, U, bx, by, bz, d, s->g, s->gUi, s->gBi, st);
     if (rc == MHD_OK) rc = advance_lanes<float>(s, s->gUi, s->gBi, s->gUo, s->gBo, nullptr, nullptr, G, dt, dh, st);
@@ -93,7 +98,32 @@ int mhd_grid_advance(mhd_solver* s, void* U, void* bx, void* by, void* bz, int n
     if (rc == MHD_OK) rc = advance_lanes<double>(s, s->gUi, s->gBi, s->gUo, s->gBo, nullptr, nullptr, G, dt, dh, st);
     if (rc == MHD_OK) rc = grid_unpack_t<double>(s, s->gUo, s->gBo, d, U, bx, by, bz, st);
   }
+  s->red_now = nullptr;
   return rc;
+}
+
+extern "C" {
+
+int mhd_grid_advance(mhd_solver* s, void* U, void* bx, void* by, void* bz, int nx, int ny, int nz, double dt, double dh,
+                     void* cuda_stream) {
+  return grid_advance_impl(s, U, bx, by, bz, nx, ny, nz, dt, dh, nullptr, cuda_stream);
+}
+
+int mhd_grid_advance_dt(mhd_solver* s, void* U, void* bx, void* by, void* bz, int nx, int ny, int nz, double dt, double dh,
+                        double cfl, double* dt_out, double* maxspeed_out, void* cuda_stream) {
+  if (!s || !dt_out || !(cfl > 0.0)) return MHD_EINVAL;
+  const int rc = grid_advance_impl(s, U, bx, by, bz, nx, ny, nz, dt, dh, s->d_red, cuda_stream);
+  if (rc != MHD_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  unsigned long long bits = 0;
+  CU(cudaMemcpyAsync(&bits, s->d_red, sizeof bits, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  double smax;
+  if (s->cfg.prec == MHD_FP32) { unsigned int b32 = (unsigned int)(bits & 0xffffffffu); float f; memcpy(&f, &b32, 4); smax = f; }
+  else memcpy(&smax, &bits, 8);
+  if (maxspeed_out) *maxspeed_out = smax;
+  *dt_out = cfl * dh / smax;
+  return MHD_OK;
 }
 
 int mhd_grid_dt(mhd_solver* s, const void* U, const void* bx, const void* by, const void* bz, int nx, int ny, int nz, double dh,

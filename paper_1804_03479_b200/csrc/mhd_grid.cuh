@@ -8,7 +8,7 @@
 // bz[nz+1][ny][nx], x fastest; the last face of each periodic direction duplicates the first.
 // Group g = (gz*my + gy)*mx + gx (gx fastest) covers cells [gx*N, (gx+1)*N) x ... plus `ng` ghost cells per side.
 #pragma once
-#include "mhd_kernels.cuh"
+#include "mhd_kernels3.cuh"
 
 namespace mhd {
 
@@ -83,33 +83,11 @@ __global__ void __launch_bounds__(256) k_dt_grid(const R* __restrict__ U, const 
   if (t < n3) {
     const int i = (int)(t % d.nx), j = (int)((t / d.nx) % d.ny), k = (int)(t / ((size_t)d.nx * d.ny));
     const size_t qx = ((size_t)k * d.ny + j) * (d.nx + 1) + i, qy = ((size_t)k * (d.ny + 1) + j) * d.nx + i;
-    const R Bc[3] = { R(0.5) * (bx[qx] + bx[qx + 1]), R(0.5) * (by[qy] + by[qy + d.nx]),
-                      R(0.5) * (bz[t] + bz[t + (size_t)d.nx * d.ny]) };
-    const R rho = Num<R>::max(U[t], min_dens);
-    const R v[3] = { U[n3 + t] / rho, U[2 * n3 + t] / rho, U[3 * n3 + t] / rho };
-    const R b2 = Bc[0] * Bc[0] + Bc[1] * Bc[1] + Bc[2] * Bc[2];
-    R P = (gam - R(1)) * (U[4 * n3 + t] - R(0.5) * rho * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) - R(0.5) * b2);
-    P = Num<R>::max(P, min_pres);
-#pragma unroll
-    for (int dd = 0; dd < 3; ++dd) {
-      const R bn2 = Bc[dd] * Bc[dd];
-      smax = Num<R>::max(smax, Num<R>::abs(v[dd]) + fast_speed(rho, P, bn2, b2 - bn2, gam));
-    }
+    const R bl[3] = { bx[qx], by[qy], bz[t] }, bu[3] = { bx[qx + 1], by[qy + d.nx], bz[t + (size_t)d.nx * d.ny] };
+    const R u[5] = { U[t], U[n3 + t], U[2 * n3 + t], U[3 * n3 + t], U[4 * n3 + t] };
+    smax = cell_signal_speed(u, bl, bu, gam, min_dens, min_pres);
   }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) smax = Num<R>::max(smax, __shfl_xor_sync(0xffffffffu, smax, o));
-  __shared__ R red[8];
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = smax;
-  __syncthreads();
-  if (threadIdx.x < 32) {
-    R m = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : R(0);
-#pragma unroll
-    for (int o = 4; o > 0; o >>= 1) m = Num<R>::max(m, __shfl_xor_sync(0xffffffffu, m, o));
-    if (threadIdx.x == 0) {
-      if (sizeof(R) == 8) atomicMax(out, (unsigned long long)__double_as_longlong((double)m));
-      else atomicMax(reinterpret_cast<unsigned int*>(out), __float_as_uint((float)m));
-    }
-  }
+  block_max_to(smax, out);
 }
 
 }  // namespace mhd

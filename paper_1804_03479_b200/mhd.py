@@ -21,7 +21,7 @@ MC, MINMOD, VANLEER = 0, 1, 2
 OK, EINVAL, ECUDA, ENOMEM = 0, -1, -2, -3
 
 EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance_host", "mhd_dt_reduce", "mhd_advance_dt",
-           "mhd_get_stats", "mhd_launch_count", "mhd_grid_pack", "mhd_grid_unpack", "mhd_grid_advance", "mhd_grid_dt", "mhd_amr_restrict", "mhd_amr_fixup", "mhd_amr_prolong", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
+           "mhd_get_stats", "mhd_launch_count", "mhd_grid_pack", "mhd_grid_unpack", "mhd_grid_advance", "mhd_grid_advance_dt", "mhd_grid_dt", "mhd_amr_restrict", "mhd_amr_fixup", "mhd_amr_prolong", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
            "mhd_measure_fma_peak", "mhd_strerror"]
 
 
@@ -65,6 +65,8 @@ def lib():
         L.mhd_grid_pack.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, vp, vp, vp]
         L.mhd_grid_unpack.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, vp, vp]
         L.mhd_grid_advance.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, vp]
+        L.mhd_grid_advance_dt.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                          C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
         L.mhd_grid_dt.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
                                   C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
         ip = C.POINTER(C.c_int)
@@ -196,6 +198,13 @@ class Solver:
         nz, ny, nx = shape
         _check(lib().mhd_grid_advance(self._h, _ptr(U), _ptr(bx), _ptr(by), _ptr(bz), nx, ny, nz, float(dt), float(dh),
                                       _stream_ptr(stream)))
+
+    def grid_advance_dt(self, U, bx, by, bz, shape, dt, dh, cfl, stream=None):
+        nz, ny, nx = shape
+        dtn, sm = C.c_double(), C.c_double()
+        _check(lib().mhd_grid_advance_dt(self._h, _ptr(U), _ptr(bx), _ptr(by), _ptr(bz), nx, ny, nz, float(dt), float(dh),
+                                         float(cfl), C.byref(dtn), C.byref(sm), _stream_ptr(stream)))
+        return dtn.value, sm.value
 
     def grid_dt(self, U, bx, by, bz, shape, dh, cfl, stream=None):
         nz, ny, nx = shape

@@ -67,6 +67,27 @@ def device_run(gpu, grid, shape, dh, nsteps, cfl=0.3, dts=None):
     return used
 
 
+@pytest.mark.parametrize("prec", [1, 0])
+@pytest.mark.parametrize("N,g,scheme,recon", [(16, 3, 0, 0), (8, 4, 1, 1)])
+def test_grid_advance_dt_is_the_two_calls_bitwise(prec, N, g, scheme, recon):
+    """mhd_grid_advance_dt: the dt of the next step comes out of the final update; same bits as mhd_grid_advance + mhd_grid_dt"""
+    n = 2 * N
+    dtp = GU.np_dtype(prec)
+    U, bx, by, bz, dh = inputs.abc_grid(n, seed=1806, p0=0.15, vamp=1e-2)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=scheme, recon=recon, prec=prec, max_groups=8)
+    a, b = to_dev((U, bx, by, bz), dtp), to_dev((U, bx, by, bz), dtp)
+    shape = (n, n, n)
+    dt = gpu.solver.grid_dt(*a, shape, dh, 0.3)[0]
+    for _ in range(5):
+        gpu.solver.grid_advance(*a, shape, dt, dh)
+        dt_a, s_a = gpu.solver.grid_dt(*a, shape, dh, 0.3)
+        dt_b, s_b = gpu.solver.grid_advance_dt(*b, shape, dt, dh, 0.3)
+        assert (dt_a, s_a) == (dt_b, s_b)
+        dt = dt_b
+    for x, y in zip(a, b):
+        assert gpu.torch.equal(x, y)
+
+
 def test_config1_on_the_device_equals_the_host_prepared_path_and_the_oracle(oracle):
     n, N, g = 32, 16, 3
     U, bx, by, bz, dh = inputs.abc_grid(n, seed=1804, p0=1.0, vamp=1e-3)
