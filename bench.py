@@ -5,8 +5,8 @@
 
 Workload (config.workload): BASELINE.json configs[1] -- a batch of 512 patch groups of 16^3 cells (+3 ghost cells,
 VL+PLM+HLLD+CT; flux_out and emf_out requested), seeded synthetic state of paper_1804_03479_b200.inputs.config2_batch
-(DESIGN.md "Input recipe").  One "step" = one pass of the whole hot path over the batch: mhd_advance (S0-S8) followed by
-mhd_dt_reduce (S9) on its output.  The headline line is FP32 (the paper's headline precision); the same run measures
+(DESIGN.md "Input recipe").  One "step" = one pass of the whole hot path over the batch: mhd_advance_dt = S0-S8 with the
+CFL reduction (S9) of the new state fused into the final update (bit-identical to mhd_advance + mhd_dt_reduce).  The headline line is FP32 (the paper's headline precision); the same run measures
 FP64 and reports it under "fp64".  The batch (177 MB FP32 / 355 MB FP64 of input) is larger than the 126 MB L2, so
 no explicit L2 flush is needed between iterations (config.l2: "inputs larger than L2").
 
@@ -35,11 +35,11 @@ FLOP_PER_SOLVE = {"hlld": 381, "roe": 1107, "hlle": 361}
 FLOP_PER_CELL_UPDATE = {("vl", "hlld"): 6263.5, ("vl", "roe"): 15289.0, ("ctu", "hlld"): 26067.6, ("ctu", "roe"): 35160.4}   # whole step
 FLOP_PLM_PER_FACE = 140     # two MC-limited primitive slopes + the two face states (VL pass 2)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage kernel at 512 groups, VL+PLM+HLLD, from the
-# ncu --set full captures summarised in profiles/r01g_full_top_kernels.md and r01g_f64_full_top_kernels.md (MB)
-NCU_TRAFFIC_MB = {"f32": {"pass1_fused": 1007.8, "emf_pass1": 364.6, "half_step": 888.4, "flux_pass2": 643.7,
-                          "emf_pass2": 242.5, "final_update": 429.6, "dt_reduce": 69.2},
-                  "f64": {"pass1_fused": 1796.3, "emf_pass1": 705.4, "half_step": 1665.3, "flux_pass2": 1082.9,
-                          "emf_pass2": 450.3, "final_update": 848.4, "dt_reduce": 141.2}}
+# ncu --set full captures summarised in profiles/r01h_full_top_kernels.md and r01h_f64_full_top_kernels.md (MB)
+NCU_TRAFFIC_MB = {"f32": {"pass1_fused": 1008.2, "emf_pass1": 364.8, "half_step": 888.0, "flux_pass2": 643.3,
+                          "emf_pass2": 242.6, "final_update": 432.1},
+                  "f64": {"pass1_fused": 1796.8, "emf_pass1": 705.0, "half_step": 1665.8, "flux_pass2": 1083.8,
+                          "emf_pass2": 451.0, "final_update": 850.4}}
 NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
 
 
@@ -141,7 +141,7 @@ def make_batch(G, g, npdt):
 
 
 def measure(args, prec_name, rank, world, dist):
-    """Time K steps of (mhd_advance + mhd_dt_reduce) on device-resident data, then the per-stage profile, then e2e."""
+    """Time K steps of mhd_advance_dt on device-resident data, then the per-stage profile, then e2e."""
     import numpy as np
     import torch
     from paper_1804_03479_b200 import mhd, shard
@@ -221,13 +221,13 @@ def measure(args, prec_name, rank, world, dist):
                 "peak_fma_measured": mhd.measure_fma_peak(dev.index, prec),
                 "traffic": (NCU_TRAFFIC_MB[prec_name][top] * 1e6 if (args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS
                                                                         and top in NCU_TRAFFIC_MB[prec_name]) else None),
-                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01g_*)",
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01h_*)",
                 "avg_launch_ms": dur * 1e3, "launches_per_step": n_launch,
                 "share_of_step": stages[top]["ms_per_step"] / (prof_ms / args.steps)}
-    # HBM view of the whole step: algorithmic bytes = read the ghost-zoned tile once, write the results once (+ dt read)
+    # HBM view of the whole step: algorithmic bytes = read the ghost-zoned tile once, write the results once (the CFL
+    # reduction is fused into the final update: no second read of the new state)
     sz = solver.sizes()
-    bytes_step = (sz["n_U_in"] + sz["n_B_in"] + sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]
-                  + sz["n_U_out"] + sz["n_B_out"]) * esz * G
+    bytes_step = (sz["n_U_in"] + sz["n_B_in"] + sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]) * esz * G
     if args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS and set(stages) == set(NCU_TRAFFIC_MB[prec_name]):
         tot = sum(NCU_TRAFFIC_MB[prec_name].values()) * 1e6
         res["dram_traffic"] = {"bytes_per_step_ncu": tot, "GBs": tot / 1e9 / (res["ms_per_step"] * 1e-3),
