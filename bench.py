@@ -57,6 +57,8 @@ def parse():
     ap.add_argument("--config5", type=int, default=0, metavar="POOL", help="instead of the batch: BASELINE config 5, 262144 "
                     "group-updates (= 1024^3 cells) in FP32 streamed from a pinned pool of POOL groups (a multiple of 512, e.g. 4096), "
                     "VL+PLM and CTU+PPM, with and without transfers")
+    ap.add_argument("--sweep", action="store_true", help="instead of the batch: throughput against the number of patch groups per "
+                    "call (8 ... 4096; the axis of the paper's Fig. 18), FP32 and FP64, device-resident")
     ap.add_argument("--grid", type=int, default=0, help="instead of the batch: a periodic n^3 ABC grid (BASELINE config 3 "
                     "state) kept on the device; step = mhd_grid_advance_dt (pack + scheme with fused dt + unpack)")
     return ap.parse_args()
@@ -336,6 +338,42 @@ def measure_config5(args, scheme_name):
     return res
 
 
+def measure_sweep(args, prec_name):
+    """Cell-updates/s of mhd_advance_dt against the number of patch groups per call (the saturation curve of PAPER.md:467, Fig. 18)."""
+    import numpy as np
+    import torch
+    from paper_1804_03479_b200 import mhd
+    sp = scheme_params(args)
+    g = sp["g"]
+    prec = mhd.FP32 if prec_name == "f32" else mhd.FP64
+    npdt = np.float32 if prec_name == "f32" else np.float64
+    riem = {"hlle": mhd.HLLE, "hlld": mhd.HLLD, "roe": mhd.ROE}[args.riemann]
+    stream = torch.cuda.current_stream()
+    curve = []
+    for G in (8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096):
+        solver = mhd.Solver(mhd.make_config(N=N_PS2, g=g, scheme=sp["scheme"], recon=sp["recon"], riemann=riem, prec=prec, max_groups=G))
+        hU, hB, dh = make_batch(G, g, npdt)
+        dU, dB = torch.from_numpy(hU).cuda(), torch.from_numpy(hB).cuda()
+        out = solver.alloc_outputs(G, planes=True)
+        dt0, _ = solver.dt_reduce(dU, dB, G, g, dh, 0.3)
+        steps = max(args.steps, min(400, 8192 // G))          # short calls: more repetitions
+        for _ in range(args.warmup):
+            solver.advance_dt(dU, dB, out["U"], out["B"], out["flux"], out["emf"], G, dt0, dh, 0.3, stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(steps):
+            solver.advance_dt(dU, dB, out["U"], out["B"], out["flux"], out["emf"], G, dt0, dh, 0.3, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        curve.append({"groups": G, "cells": G * N_PS2 ** 3, "ms_per_step": ms, "value": G * N_PS2 ** 3 / (ms * 1e-3)})
+        solver.destroy()
+        del dU, dB, out
+        torch.cuda.empty_cache()
+    return curve
+
+
 def measure_grid(args, prec_name):
     """Uniform periodic grid resident on the device (NEXT-1): K steps of mhd_grid_advance_dt."""
     import numpy as np
@@ -467,6 +505,21 @@ def main():
                           "e2e": {"value": r[0]["with_transfers"]["value"], "unit": "cell-updates/s", "h2d_bytes_per_step": r[0]["with_transfers"]["h2d_bytes"],
                                   "d2h_bytes_per_step": r[0]["with_transfers"]["d2h_bytes"]},
                           "vl_plm": r[0], "ctu_ppm": r[1]}))
+        return 0
+    if args.sweep:
+        sampler = ClockSampler(torch.cuda.current_device())
+        sampler.start()
+        c32, c64 = measure_sweep(args, "f32"), measure_sweep(args, "f64")
+        clocks = sampler.result()
+        config.update(workload="BASELINE.json configs[1] state, 8 ... 4096 patch groups of 16^3 per call (the axis of the paper's Fig. 18, "
+                               "PAPER.md:467), %s+%s+CT, device-resident" % (sp_name, args.riemann.upper()),
+                      step="mhd_advance_dt", groups_per_rank=[c["groups"] for c in c32])
+        top = max(c32, key=lambda c: c["value"])
+        print(json.dumps({"metric": "cell-updates/sec", "value": top["value"], "unit": "cell-updates/s", "n_gpus": 1, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": top["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                          "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config, "clocks": clocks,
+                          "curve_f32": c32, "curve_f64": c64,
+                          "paper_context": "P100: throughput saturates above ~2e6 cells per call (PAPER.md:467)"}))
         return 0
     if args.grid:
         a, b = measure_grid(args, args.prec), measure_grid(args, "f64" if args.prec == "f32" else "f32")
