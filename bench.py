@@ -34,12 +34,12 @@ PAPER_P100 = {"f32": 1.2e8, "f64": 5.5e7}       # PAPER.md:12, :465-467 (Tesla P
 FLOP_PER_SOLVE = {"hlld": 381, "roe": 1107, "hlle": 361}
 FLOP_PER_CELL_UPDATE = {("vl", "hlld"): 6263.5, ("vl", "roe"): 15289.0, ("ctu", "hlld"): 26067.6, ("ctu", "roe"): 35160.4}   # whole step
 FLOP_PLM_PER_FACE = 140     # two MC-limited primitive slopes + the two face states (VL pass 2)
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage kernel at 512 groups, VL+PLM+HLLD, from the
+# dram__bytes_read.sum + dram__bytes_write.sum of each stage's launches of one 512-group step (two slices of 256), VL+PLM+HLLD, from the
 # ncu --set full captures summarised in profiles/r01h_full_top_kernels.md and r01h_f64_full_top_kernels.md (MB)
-NCU_TRAFFIC_MB = {"f32": {"pass1_fused": 1008.2, "emf_pass1": 364.8, "half_step": 888.0, "flux_pass2": 643.3,
-                          "emf_pass2": 242.6, "final_update": 432.1},
-                  "f64": {"pass1_fused": 1796.8, "emf_pass1": 705.0, "half_step": 1665.8, "flux_pass2": 1083.8,
-                          "emf_pass2": 451.0, "final_update": 850.4}}
+NCU_TRAFFIC_MB = {"f32": {"pass1_fused": 968.0, "emf_pass1": 351.3, "half_step": 856.6, "flux_pass2": 609.4,
+                          "emf_pass2": 229.2, "final_update": 418.6},
+                  "f64": {"pass1_fused": 1756.3, "emf_pass1": 691.7, "half_step": 1631.1, "flux_pass2": 1058.2,
+                          "emf_pass2": 438.1, "final_update": 831.7}}
 NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
 
 
@@ -221,9 +221,10 @@ def measure(args, prec_name, rank, world, dist):
         roof = {"bound": "alu", "kernel": top, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
                 "peak_source": "nominal: 148 SMs x %d FMA lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if prec_name == "f32" else 64),
                 "peak_fma_measured": mhd.measure_fma_peak(dev.index, prec),
-                "traffic": (NCU_TRAFFIC_MB[prec_name][top] * 1e6 if (args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS
-                                                                        and top in NCU_TRAFFIC_MB[prec_name]) else None),
-                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01h_*)",
+                "traffic": (NCU_TRAFFIC_MB[prec_name][top] * 1e6 / n_launch if (args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS
+                                                                                   and top in NCU_TRAFFIC_MB[prec_name]) else None),
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum of the stage's launches of one step, "
+                                "profiles/r01h_*, / launches per step)",
                 "avg_launch_ms": dur * 1e3, "launches_per_step": n_launch,
                 "share_of_step": stages[top]["ms_per_step"] / (prof_ms / args.steps)}
     # HBM view of the whole step: algorithmic bytes = read the ghost-zoned tile once, write the results once (the CFL
