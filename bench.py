@@ -474,6 +474,7 @@ def main():
         cb.update(value=val, seconds=t, sample="%d of the %d patch groups per step (advance + dt), FP64 oracle, OpenMP over "
                                                  "groups" % (sample, args.groups))
         cb.pop("best_pass_value", None)
+        config = dict(config, step="the same step on the oracle: mhdref advance (S0-S8) + dt_reduce (S9) of its output")
         line = {"impl": "reference", "metric": "cell-updates/sec", "value": val, "unit": "cell-updates/s", "n_gpus": args.gpus,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config,

@@ -67,6 +67,23 @@ def test_ragged_slices_are_bitwise_identical(slice_groups, monkeypatch):
     assert np.array_equal(c["U"][::-1], b["U"]) and np.array_equal(c["emf"][::-1], b["emf"])
 
 
+@pytest.mark.parametrize("prec", [1, 0])
+def test_one_slice_per_lane_equals_one_slice_bitwise(prec, monkeypatch):
+    """A batch of >= 256 groups is cut into one slice per lane (two concurrent streams); one lane = one slice: same bits,
+    same reduced CFL speed."""
+    dtp = GU.np_dtype(prec)
+    U16, B16, dh = small_batch(16, dtype=dtp)
+    G = 259                                                      # two lanes: slices of 130 and 129 groups
+    U, B = np.tile(U16, (17, 1))[:G].copy(), np.tile(B16, (17, 1))[:G].copy()
+    a, dt_a, s_a = GU.GpuRunner(prec=prec, max_groups=G).advance_dt(U, B, 2e-3, dh, 0.3)
+    monkeypatch.setenv("MHD_LANES", "1")
+    b, dt_b, s_b = GU.GpuRunner(prec=prec, max_groups=G).advance_dt(U, B, 2e-3, dh, 0.3)
+    for k in ("U", "B", "flux", "emf"):
+        assert np.array_equal(a[k], b[k]), k
+    assert (dt_a, s_a) == (dt_b, s_b)
+    assert np.array_equal(a["U"][:16], a["U"][16:32]) and np.array_equal(a["U"][:3], a["U"][256:259])   # tiled inputs, both lanes
+
+
 @pytest.mark.parametrize("N,g,scheme,recon", [(8, 3, 0, 0), (32, 3, 0, 0), (16, 4, 0, 0), (8, 4, 1, 1), (24, 5, 1, 1), (32, 3, 1, 0)])
 def test_other_group_sizes_and_wider_ghosts(oracle, N, g, scheme, recon):
     """ps2 != 16 and ghost widths above the minimum (extra layers must not matter)."""
