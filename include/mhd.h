@@ -90,6 +90,13 @@ int mhd_advance_host(mhd_solver* s, const void* U_in, const void* B_in, void* U_
                      void* flux_out, void* emf_out, int ngroups, double dt, double dh,
                      int chunk_groups, int nstreams);
 
+/* mhd_advance_host with the CFL reduction of the new state fused into every chunk's final update (see mhd_advance_dt):
+ * the complete path S0-S9 through HOST buffers.  dt_out (required) and maxspeed_out (nullable) are HOST pointers; outputs
+ * bit-identical to mhd_advance_host, dt bit-identical to mhd_advance_dt.  ngroups >= 1.  Blocking. */
+int mhd_advance_host_dt(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out,
+                        void* flux_out, void* emf_out, int ngroups, double dt, double dh,
+                        int chunk_groups, int nstreams, double cfl, double* dt_out, double* maxspeed_out);
+
 /* CFL time step (R13): dt = cfl * dh / max over interior cells and directions d of
  * (|v_d| + c_f,d), cell-centred B = face mean.  U, B: DEVICE arrays of ngroups groups whose ghost width is
  * nghost_of_arrays (0: the U_out/B_out layout; cfg.nghost: the U_in/B_in layout).  dt_out (required) and

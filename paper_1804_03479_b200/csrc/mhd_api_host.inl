@@ -21,12 +21,9 @@ int ensure_lanes(mhd_solver* s, int nstreams, int chunk_groups) {
   return MHD_OK;
 }
 
-}  // namespace
-
-extern "C" {
-
-int mhd_advance_host(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out, void* flux_out,
-                     void* emf_out, int ngroups, double dt, double dh, int chunk_groups, int nstreams) {
+// red != nullptr: the final update of every chunk also reduces the CFL speed into *red (zeroed on lane 0 before any chunk)
+int advance_host_impl(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out, void* flux_out,
+                      void* emf_out, int ngroups, double dt, double dh, int chunk_groups, int nstreams, unsigned long long* red) {
   if (!s || !U_in || !B_in || !U_out || !B_out) return MHD_EINVAL;
   if (ngroups < 0 || nstreams < 1 || nstreams > kMaxStreams) return MHD_EINVAL;
   if (chunk_groups < 1 || chunk_groups > s->cfg.max_groups) return MHD_EINVAL;
@@ -42,25 +39,57 @@ int mhd_advance_host(mhd_solver* s, const void* U_in, const void* B_in, void* U_
   // the lane's slice size must not exceed its workspace
   const int saved_slice = s->slice_groups;
   s->slice_groups = std::min(saved_slice, chunk_groups);
+  if (red) {
+    CU(cudaMemsetAsync(red, 0, sizeof(unsigned long long), s->lanes[0].stream));
+    CU(cudaEventRecord(s->fork, s->lanes[0].stream));
+    for (int l = 1; l < nstreams; ++l) CU(cudaStreamWaitEvent(s->lanes[l].stream, s->fork, 0));
+  }
+  s->red_now = red;
   int c = 0;
   for (int first = 0; first < ngroups; first += chunk_groups, ++c) {
     const size_t ng = (size_t)std::min(chunk_groups, ngroups - first), f = (size_t)first;
     HostLane& L = s->lanes[c % nstreams];
     cudaError_t ce = cudaMemcpyAsync(L.Ui, hUi + f * s->nUi * e, ng * s->nUi * e, cudaMemcpyHostToDevice, L.stream);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(L.Bi, hBi + f * s->nBi * e, ng * s->nBi * e, cudaMemcpyHostToDevice, L.stream);
-    if (ce != cudaSuccess) { s->slice_groups = saved_slice; return cuda_fail(ce, "mhd_advance_host H2D"); }
+    if (ce != cudaSuccess) { s->slice_groups = saved_slice; s->red_now = nullptr; return cuda_fail(ce, "mhd_advance_host H2D"); }
     rc = s->cfg.prec == MHD_FP32
              ? advance_serial<float>(s, L.Ui, L.Bi, L.Uo, L.Bo, hf ? L.fo : nullptr, he ? L.eo : nullptr, L.ws, (int)ng, dt, dh, L.stream)
              : advance_serial<double>(s, L.Ui, L.Bi, L.Uo, L.Bo, hf ? L.fo : nullptr, he ? L.eo : nullptr, L.ws, (int)ng, dt, dh, L.stream);
-    if (rc != MHD_OK) { s->slice_groups = saved_slice; return rc; }
+    if (rc != MHD_OK) { s->slice_groups = saved_slice; s->red_now = nullptr; return rc; }
     ce = cudaMemcpyAsync(hUo + f * s->nUo * e, L.Uo, ng * s->nUo * e, cudaMemcpyDeviceToHost, L.stream);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(hBo + f * s->nBo * e, L.Bo, ng * s->nBo * e, cudaMemcpyDeviceToHost, L.stream);
     if (ce == cudaSuccess && hf) ce = cudaMemcpyAsync(hf + f * s->nF * e, L.fo, ng * s->nF * e, cudaMemcpyDeviceToHost, L.stream);
     if (ce == cudaSuccess && he) ce = cudaMemcpyAsync(he + f * s->nE * e, L.eo, ng * s->nE * e, cudaMemcpyDeviceToHost, L.stream);
-    if (ce != cudaSuccess) { s->slice_groups = saved_slice; return cuda_fail(ce, "mhd_advance_host D2H"); }
+    if (ce != cudaSuccess) { s->slice_groups = saved_slice; s->red_now = nullptr; return cuda_fail(ce, "mhd_advance_host D2H"); }
   }
   s->slice_groups = saved_slice;
+  s->red_now = nullptr;
   for (int l = 0; l < nstreams; ++l) CU(cudaStreamSynchronize(s->lanes[l].stream));
+  return MHD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mhd_advance_host(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out, void* flux_out,
+                     void* emf_out, int ngroups, double dt, double dh, int chunk_groups, int nstreams) {
+  return advance_host_impl(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, chunk_groups, nstreams, nullptr);
+}
+
+int mhd_advance_host_dt(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out, void* flux_out,
+                        void* emf_out, int ngroups, double dt, double dh, int chunk_groups, int nstreams, double cfl,
+                        double* dt_out, double* maxspeed_out) {
+  if (!s || !dt_out || ngroups < 1 || !(cfl > 0.0)) return MHD_EINVAL;
+  const int rc = advance_host_impl(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, chunk_groups, nstreams, s->d_red);
+  if (rc != MHD_OK) return rc;
+  unsigned long long bits = 0;
+  CU(cudaMemcpy(&bits, s->d_red, sizeof bits, cudaMemcpyDeviceToHost));      // every lane is synchronised
+  double smax;
+  if (s->cfg.prec == MHD_FP32) { unsigned int b32 = (unsigned int)(bits & 0xffffffffu); float f; memcpy(&f, &b32, 4); smax = f; }
+  else memcpy(&smax, &bits, 8);
+  if (maxspeed_out) *maxspeed_out = smax;
+  *dt_out = cfl * dh / smax;
   return MHD_OK;
 }
 

@@ -20,7 +20,7 @@ LIM_PRIM, LIM_CHAR = 0, 1
 MC, MINMOD, VANLEER = 0, 1, 2
 OK, EINVAL, ECUDA, ENOMEM = 0, -1, -2, -3
 
-EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance_host", "mhd_dt_reduce", "mhd_advance_dt",
+EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance_host", "mhd_advance_host_dt", "mhd_dt_reduce", "mhd_advance_dt",
            "mhd_get_stats", "mhd_launch_count", "mhd_grid_pack", "mhd_grid_unpack", "mhd_grid_advance", "mhd_grid_advance_dt", "mhd_grid_dt", "mhd_amr_restrict", "mhd_amr_fixup", "mhd_amr_prolong", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
            "mhd_measure_fma_peak", "mhd_strerror"]
 
@@ -56,6 +56,8 @@ def lib():
         L.mhd_advance_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int]
         L.mhd_dt_reduce.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_double),
                                     C.POINTER(C.c_double), vp]
+        L.mhd_advance_host_dt.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int,
+                                          C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.mhd_advance_dt.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, C.c_double,
                                      C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
         ull = C.POINTER(C.c_ulonglong)
@@ -170,6 +172,14 @@ class Solver:
         _check(lib().mhd_advance_host(self._h, _ptr(U_in), _ptr(B_in), _ptr(U_out), _ptr(B_out), _ptr(flux_out),
                                       _ptr(emf_out), int(ngroups), float(dt), float(dh), int(chunk_groups),
                                       int(nstreams)))
+
+    def advance_host_dt(self, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, chunk_groups, nstreams, cfl):
+        """mhd_advance_host_dt: HOST arrays; blocking; returns (dt_next, maxspeed)."""
+        dtn, sm = C.c_double(), C.c_double()
+        _check(lib().mhd_advance_host_dt(self._h, _ptr(U_in), _ptr(B_in), _ptr(U_out), _ptr(B_out), _ptr(flux_out),
+                                         _ptr(emf_out), int(ngroups), float(dt), float(dh), int(chunk_groups),
+                                         int(nstreams), float(cfl), C.byref(dtn), C.byref(sm)))
+        return dtn.value, sm.value
 
     def advance_dt(self, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, cfl, stream=None):
         dtn, sm = C.c_double(), C.c_double()

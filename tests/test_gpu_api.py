@@ -206,6 +206,14 @@ def test_advance_host_equals_advance_bitwise(prec, chunk, nstreams):
     oU, oB = np.empty((G, s.n_U_out), dtype=dtp), np.empty((G, s.n_B_out), dtype=dtp)
     s.advance_host(U, B, oU, oB, None, None, G, 2e-3, dh, chunk, nstreams)
     assert np.array_equal(oU, ref["U"]) and np.array_equal(oB, ref["B"])
+    # mhd_advance_host_dt: same outputs, and the CFL speed every chunk's final update reduced equals mhd_advance_dt's
+    _, dt_d, s_d = gpu.advance_dt(U, B, 2e-3, dh, 0.3)
+    for v in ho.values():
+        v.zero_()
+    dt_h, s_h = s.advance_host_dt(hU, hB, ho["U"], ho["B"], ho["flux"], ho["emf"], G, 2e-3, dh, chunk, nstreams, 0.3)
+    for k in ("U", "B", "flux", "emf"):
+        assert np.array_equal(ho[k].numpy(), ref[k]), k
+    assert (dt_h, s_h) == (dt_d, s_d)
 
 
 @pytest.mark.parametrize("prec,scheme,recon,g", [(0, 0, 0, 3), (1, 0, 0, 3), (0, 1, 1, 4), (1, 1, 1, 4)])
