@@ -343,6 +343,34 @@ int riemann(int solver, const double WL[7], const double WR[7], double Bn, doubl
   return roe(WL, WR, Bn, gam, F);
 }
 
+// ---------------------------------------------------------------------------------
+// Edge EMF (readings R10, R10a = SURVEY C6 with the tie of DESIGN.md section 2.1)
+// ---------------------------------------------------------------------------------
+// upwind switch on the face mass flux m between the candidates qm (from the "-" side) and qp: qm if m > 0, qp if m < 0,
+// the mean if m = 0.  R10a: "m = 0" means |m| <= m0 = tie * (mean density of the two cells rm, rp) [tie = emf_tie dh/dt],
+// i.e. less than emf_tie of the cell mass crosses the face in dt; between m0 and 2 m0 the switch ramps linearly from
+// the mean to the upwind value so that the EMF is a continuous function of m.  tie = 0 is the exact tie of SURVEY C6.
+double emf_upwind(double tie, double m, double rm, double rp, double qm, double qp) {
+  double m0 = tie * 0.5 * (rm + rp), am = std::fabs(m);
+  if (am <= m0) return 0.5 * (qm + qp);
+  if (am < 2.0 * m0) {
+    double w = (am - m0) / m0;                       // 0..1: weight of the upwind value
+    double qu = m > 0.0 ? qm : qp;
+    return w * qu + (1.0 - w) * (0.5 * (qm + qp));
+  }
+  return m > 0.0 ? qm : qp;
+}
+// SURVEY C6 for the edge along c at (a-1/2, b-1/2), (a,b,c) cyclic.  Face EMFs (E_c from the face fluxes):
+// Ea_lo = Ea(a-1/2, b-1), Ea_hi = Ea(a-1/2, b), Eb_lo = Eb(a-1, b-1/2), Eb_hi = Eb(a, b-1/2); mass fluxes through the same
+// four faces; ec[4], rho[4] = reference EMF and density of the cells (a-1,b-1), (a,b-1), (a-1,b), (a,b)
+double edge_emf_formula(double Ea_lo, double Ea_hi, double Eb_lo, double Eb_hi, double ma_lo, double ma_hi, double mb_lo,
+                        double mb_hi, const double ec[4], const double rho[4], double tie) {
+  double e = 0.25 * (Ea_hi + Ea_lo + Eb_hi + Eb_lo);
+  e += 0.25 * (emf_upwind(tie, ma_lo, rho[0], rho[1], Eb_lo - ec[0], Eb_hi - ec[1]) - emf_upwind(tie, ma_hi, rho[2], rho[3], ec[2] - Eb_lo, ec[3] - Eb_hi));
+  e += 0.25 * (emf_upwind(tie, mb_lo, rho[0], rho[2], Ea_lo - ec[0], Ea_hi - ec[2]) - emf_upwind(tie, mb_hi, rho[1], rho[3], ec[1] - Ea_lo, ec[3] - Ea_hi));
+  return e;
+}
+
 // =====================================================================================
 // one patch group
 // =====================================================================================
@@ -425,21 +453,7 @@ struct Group {
       auto Ea = [&](size_t q) { return -F[a][5][q]; };
       auto Eb = [&](size_t q) { return F[bdir][6][q]; };
       auto ec = [&](size_t q) { return Wc[1 + bdir][q] * Wc[5 + a][q] - Wc[1 + a][q] * Wc[5 + bdir][q]; };  // -(v x B)_c
-      // upwinding by the sign of the face mass flux m (reading R10): q- if m > 0, q+ if m < 0, the mean if m = 0.
-      // Reading R10a: "m = 0" means |m| <= m0 = emf_tie * (mean density of the two cells) * dh/dt, i.e. less than emf_tie
-      // of the cell mass crosses the face in dt (zero at working precision); between m0 and 2 m0 the switch ramps
-      // linearly from the mean to the upwind value, so that the EMF is a continuous function of m.
-      const double tie = c.emf_tie * dh / dt;
-      auto up = [tie](double m, double rm, double rp, double qm, double qp) {
-        double m0 = tie * 0.5 * (rm + rp), am = std::fabs(m);
-        if (am <= m0) return 0.5 * (qm + qp);
-        if (am < 2.0 * m0) {
-          double w = (am - m0) / m0;                       // 0..1: weight of the upwind value
-          double qu = m > 0.0 ? qm : qp;
-          return w * qu + (1.0 - w) * (0.5 * (qm + qp));
-        }
-        return m > 0.0 ? qm : qp;
-      };
+      const double tie = c.emf_tie * dh / dt;               // R10a: m0 = tie * (mean density of the two cells)
       const Arr& rho = Wc[0];
       int idx[3];
       for (idx[cdir] = clo; idx[cdir] < chi; ++idx[cdir])
@@ -447,11 +461,11 @@ struct Group {
           for (idx[a] = alo; idx[a] <= ahi; ++idx[a]) {
             size_t q = t.id(idx[0], idx[1], idx[2]);      // cell (a,b); its lower a-face is "a-1/2"
             size_t qa = q - oa, qb = q - ob, qab = q - oa - ob;
-            double e = 0.25 * (Ea(q) + Ea(qb) + Eb(q) + Eb(qa));
             double ma_lo = F[a][0][qb], ma_hi = F[a][0][q];       // mass flux through a-face (a-1/2, b-1) and (a-1/2, b)
             double mb_lo = F[bdir][0][qa], mb_hi = F[bdir][0][q]; // through b-face (a-1, b-1/2) and (a, b-1/2)
-            e += 0.25 * (up(ma_lo, rho[qab], rho[qb], Eb(qa) - ec(qab), Eb(q) - ec(qb)) - up(ma_hi, rho[qa], rho[q], ec(qa) - Eb(qa), ec(q) - Eb(q)));
-            e += 0.25 * (up(mb_lo, rho[qab], rho[qa], Ea(qb) - ec(qab), Ea(q) - ec(qa)) - up(mb_hi, rho[qb], rho[q], ec(qb) - Ea(qb), ec(q) - Ea(q)));
+            // cells in the order (a-1,b-1), (a,b-1), (a-1,b), (a,b)
+            const double ecs[4] = { ec(qab), ec(qb), ec(qa), ec(q) }, rhos[4] = { rho[qab], rho[qb], rho[qa], rho[q] };
+            double e = edge_emf_formula(Ea(qb), Ea(q), Eb(qa), Eb(q), ma_lo, ma_hi, mb_lo, mb_hi, ecs, rhos, tie);
             E[cdir][q] = e;
           }
     }
@@ -847,6 +861,11 @@ int mhdref_eig_roe(const double* WL, const double* WR, double Bn, double gamma, 
   eig_cons(r, Bn, gamma, lam, rr, ll);
   std::memcpy(R, rr, sizeof rr); std::memcpy(L, ll, sizeof ll);
   return 0;
+}
+// R10a unit entry points: the CT upwind switch (tie = emf_tie * dh / dt) and the C6 edge formula
+double mhdref_emf_up(double m, double rm, double rp, double qm, double qp, double tie) { return emf_upwind(tie, m, rm, rp, qm, qp); }
+double mhdref_edge_emf(const double* Eface /*Ea_lo, Ea_hi, Eb_lo, Eb_hi*/, const double* mface /*same order*/, const double* ec, const double* rho, double tie) {
+  return edge_emf_formula(Eface[0], Eface[1], Eface[2], Eface[3], mface[0], mface[1], mface[2], mface[3], ec, rho, tie);
 }
 double mhdref_mc(double a, double b) { return mc(a, b); }
 // slope limiter by index (0 MC, 1 minmod, 2 van Leer), for the limiter pins

@@ -14,6 +14,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "mhd_oracle.cpp")
 _LIB = os.path.join(_HERE, "libmhdref.so")
+_SRC32 = os.path.join(_HERE, "mhd_oracle_f32.cpp")
+_LIB32 = os.path.join(_HERE, "libmhdref_f32.so")
+_FLAGS = ["-O2", "-fno-fast-math", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC"]
 
 VL, CTU = 0, 1
 PLM, PPM = 0, 1
@@ -31,9 +34,17 @@ class Config(C.Structure):
 def build(force: bool = False) -> str:
     """Compile the oracle (g++ -O2, no fast-math, no FMA contraction, OpenMP over groups)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["g++", "-O2", "-fno-fast-math", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
-                               "-o", _LIB, _SRC])
+        subprocess.check_call(["g++"] + _FLAGS + ["-o", _LIB, _SRC])
+    build32(force)
     return _LIB
+
+
+def build32(force: bool = False) -> str:
+    """The same source instantiated in single precision (mhd_oracle_f32.cpp): the FP32 control of DESIGN.md section 9."""
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC32))
+    if force or not os.path.exists(_LIB32) or os.path.getmtime(_LIB32) < newest:
+        subprocess.check_call(["g++"] + _FLAGS + ["-o", _LIB32, _SRC32])
+    return _LIB32
 
 
 _lib = None
@@ -58,7 +69,25 @@ def lib():
         _lib.mhdref_mc.restype = C.c_double
         _lib.mhdref_limiter.argtypes = [C.c_int, C.c_double, C.c_double]
         _lib.mhdref_limiter.restype = C.c_double
+        _lib.mhdref_emf_up.argtypes = [C.c_double] * 6
+        _lib.mhdref_emf_up.restype = C.c_double
+        _lib.mhdref_edge_emf.argtypes = [dp, dp, dp, dp, C.c_double]
+        _lib.mhdref_edge_emf.restype = C.c_double
     return _lib
+
+
+_lib32 = None
+
+
+def lib32():
+    global _lib32
+    if _lib32 is None:
+        _lib32 = C.CDLL(build32())
+        fp, dp = C.POINTER(C.c_float), C.POINTER(C.c_double)
+        _lib32.mhdref32_advance.argtypes = [C.POINTER(Config), fp, fp, fp, fp, fp, fp, C.c_int, C.c_double, C.c_double,
+                                            C.POINTER(C.c_ulonglong), C.c_int]
+        _lib32.mhdref32_dt.argtypes = [C.POINTER(Config), fp, fp, C.c_int, C.c_int, C.c_double, C.c_double, dp, dp]
+    return _lib32
 
 
 def _p(a):
@@ -92,6 +121,36 @@ def advance(cfg: Config, U_in, B_in, dt, dh, want_planes=True, force_ghost_ok=Fa
     if rc != 0:
         raise ValueError(f"mhdref_advance failed rc={rc}")
     return dict(U=U_out, B=B_out, flux=flux, emf=emf, stats=tuple(int(s) for s in stats))
+
+
+def _p32(a):
+    return a.ctypes.data_as(C.POINTER(C.c_float)) if a is not None else None
+
+
+def advance32(cfg: Config, U_in, B_in, dt, dh, want_planes=True):
+    """The oracle in single precision (every operation rounded to float): float32 in, float32 out."""
+    U_in = np.ascontiguousarray(U_in, dtype=np.float32); B_in = np.ascontiguousarray(B_in, dtype=np.float32)
+    G = U_in.shape[0]
+    N = cfg.ps2
+    f32 = np.float32
+    U_out = np.empty((G, 5 * N ** 3), f32); B_out = np.empty((G, 3 * N * N * (N + 1)), f32)
+    flux = np.empty((G, 9 * 5 * N * N), f32) if want_planes else None
+    emf = np.empty((G, 9 * 2 * (N + 1) * N), f32) if want_planes else None
+    stats = (C.c_ulonglong * 3)(0, 0, 0)
+    rc = lib32().mhdref32_advance(C.byref(cfg), _p32(U_in), _p32(B_in), _p32(U_out), _p32(B_out), _p32(flux), _p32(emf), G,
+                                  float(dt), float(dh), stats, 0)
+    if rc != 0:
+        raise ValueError(f"mhdref32_advance failed rc={rc}")
+    return dict(U=U_out, B=B_out, flux=flux, emf=emf, stats=tuple(int(s) for s in stats))
+
+
+def dt_reduce32(cfg: Config, U, B, ng, dh, cfl):
+    U = np.ascontiguousarray(U, dtype=np.float32); B = np.ascontiguousarray(B, dtype=np.float32)
+    dt = C.c_double(0); sm = C.c_double(0)
+    rc = lib32().mhdref32_dt(C.byref(cfg), _p32(U), _p32(B), U.shape[0], ng, float(dh), float(cfl), C.byref(dt), C.byref(sm))
+    if rc != 0:
+        raise ValueError("mhdref32_dt failed")
+    return dt.value, sm.value
 
 
 def dt_reduce(cfg: Config, U, B, ng, dh, cfl):
@@ -138,6 +197,16 @@ def eig_roe(WL, WR, Bn, gamma=5.0 / 3.0):
     lam = np.empty(7); R = np.empty((7, 7)); L = np.empty((7, 7)); avg = np.empty(9)
     rc = lib().mhdref_eig_roe(_p(WL), _p(WR), float(Bn), float(gamma), _p(lam), _p(R), _p(L), _p(avg))
     return rc, lam, R, L, avg
+
+
+def emf_up(m, rm, rp, qm, qp, tie):
+    """R10a: the CT upwind switch; tie = emf_tie * dh / dt"""
+    return lib().mhdref_emf_up(float(m), float(rm), float(rp), float(qm), float(qp), float(tie))
+
+
+def edge_emf(Eface, mface, ec, rho, tie):
+    """SURVEY C6 for one edge: Eface/mface = (a-face lo, a-face hi, b-face lo, b-face hi), ec/rho = cells (a-1,b-1), (a,b-1), (a-1,b), (a,b)"""
+    return lib().mhdref_edge_emf(_p(_c(Eface)), _p(_c(mface)), _p(_c(ec)), _p(_c(rho)), float(tie))
 
 
 def mc(a, b):

@@ -31,10 +31,10 @@ def nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
-def stale() -> bool:
-    if not os.path.exists(LIB):
+def stale(lib: str = LIB) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
 
 
@@ -46,5 +46,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+LIB_IEEE32 = os.path.join(HERE, "libmhd_ieee32.so")
+
+
+def build_ieee32(force: bool = False) -> str:
+    """Control build for tests/fp32_controls.py only (never loaded by the product path unless MHD_LIBPATH points at it):
+    the same sources with -DMHD_IEEE32, i.e. IEEE-rounded FP32 division / square root instead of the SFU approximations."""
+    if force or stale(LIB_IEEE32):
+        cmd = [nvcc()] + NVCC_FLAGS + ["-DMHD_IEEE32"] + [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB_IEEE32]
+        subprocess.check_call(cmd)
+    return LIB_IEEE32
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--ieee32" in sys.argv:
+        print(build_ieee32(force="--force" in sys.argv))

@@ -49,8 +49,14 @@ enum : int { kPLM = 0, kPPM = 1, kPPMNoTrace = 2 };   // kPPMNoTrace: the PPM pa
 enum : int { kLimPrim = 0, kLimChar = 1 };   // kernels take LIM = limvar + 2 * limiter (limiter: 0 MC, 1 minmod, 2 van Leer)
 
 template <class R> struct Num;
+// -DMHD_IEEE32: control build (libmhd_ieee32.so, tests/fp32_controls.py): every FP32 division / square root IEEE-rounded
+// instead of the SFU approximations, to separate their error from the rounding inherent to single precision
 template <> struct Num<float> {
+#ifdef MHD_IEEE32
+  static __device__ __forceinline__ float sqrt(float x) { return __fsqrt_rn(x); }
+#else
   static __device__ __forceinline__ float sqrt(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+#endif
   static __device__ __forceinline__ float abs(float x) { return fabsf(x); }
   static __device__ __forceinline__ float min(float a, float b) { return fminf(a, b); }
   static __device__ __forceinline__ float max(float a, float b) { return fmaxf(a, b); }
@@ -69,14 +75,20 @@ template <class R> __device__ __forceinline__ R sqr(R x) { return x * x; }
 // (1e-4 after 10 steps) is four orders of magnitude above their error.
 __device__ __forceinline__ double frcp(double x) { return 1.0 / x; }
 __device__ __forceinline__ double fdiv(double a, double b) { return a / b; }
+#ifdef MHD_IEEE32
+__device__ __forceinline__ float frcp(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ float fdiv(float a, float b) { return __fdiv_rn(a, b); }
+__device__ __forceinline__ float frsqrt(float x) { return __frcp_rn(__fsqrt_rn(x)); }
+#else
 __device__ __forceinline__ float frcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float fdiv(float a, float b) { return a * frcp(b); }
 __device__ __forceinline__ float frsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+#endif
 __device__ __forceinline__ double frsqrt(double x) { return rsqrt(x); }
 // sqrt(x) and 1/sqrt(x): FP64 from one rsqrt (sqrt = x * rsqrt), FP32 from the two SFU approximations
 __device__ __forceinline__ void sqrt_and_inverse(double x, double& s, double& is) { is = rsqrt(x); s = x * is; }
 __device__ __forceinline__ void sqrt_and_inverse(float x, float& s, float& is) {
-  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(x));
+  s = Num<float>::sqrt(x);
   is = frcp(s);
 }
 // several reciprocals at once.  FP32: one SFU op each.  FP64: ONE division for the product and a few multiplications

@@ -261,6 +261,48 @@ def config2_batch(G, N=16, g=3, seed=3479, first=0, dtype=np.float64, gamma=GAMM
     return U_in, B_in, 1.0 / N
 
 
+def _hash_uniform(idx, seed):
+    """Counter-based uniform [0,1) from an integer array (splitmix64 finaliser): the value of a cell depends only on its
+    global index, so ghost cells of one group equal the interior cells of its neighbour without building the grid."""
+    with np.errstate(over="ignore"):
+        z = idx.astype(np.uint64) + np.uint64(seed) * np.uint64(0x9E3779B97F4A7C15) + np.uint64(0x632BE59BD9B4E019)
+        z = (z ^ (z >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)
+        z = (z ^ (z >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)
+        z = z ^ (z >> np.uint64(31))
+    return (z >> np.uint64(11)).astype(np.float64) * (1.0 / 9007199254740992.0)
+
+
+def abc_groups(n, first, G, N=16, g=3, seed=1805, p0=0.15, vamp=1e-2, dtype=np.float64, gamma=GAMMA):
+    """Config 5 (BASELINE.json): G consecutive patch groups (group order of pack_groups: gz outermost, gx fastest), starting
+    at group `first`, of the periodic n^3 ABC state of config 3 (rho = 1, p = p0, A=B=C=1, k = 2 pi, v_d ~ U(-vamp, vamp)),
+    generated group by group WITHOUT building the grid (1024^3 does not fit): the face field is the discrete curl of the
+    analytic edge potential on the ghost-zoned tile, the velocity of a cell a counter-based hash of its global index."""
+    dh = 1.0 / n
+    m = n // N
+    T = N + 2 * g
+    k = 2.0 * np.pi
+    U_in = np.empty((G, 5, T, T, T), dtype=dtype)
+    B_in = np.empty((G, 3 * T * T * (T + 1)), dtype=dtype)
+    bxo, byo, bzo = split_B(B_in, T)
+    for q in range(G):
+        gi = first + q
+        gx, gy, gz = gi % m, (gi // m) % m, gi // (m * m)
+        ci = [np.arange(-g, N + g) + o * N for o in (gx, gy, gz)]            # global (unwrapped) cell indices per axis
+        c = [(a + 0.5) * dh for a in ci]
+        f = [np.arange(-g, N + g + 1) * dh + o * N * dh for o in (gx, gy, gz)]
+        Z, Y, X = np.meshgrid(f[2], f[1], c[0], indexing="ij"); Ax = (np.sin(k * Z) + np.cos(k * Y) + 0 * X) / k
+        Z, Y, X = np.meshgrid(f[2], c[1], f[0], indexing="ij"); Ay = (np.sin(k * X) + np.cos(k * Z) + 0 * Y) / k
+        Z, Y, X = np.meshgrid(c[2], f[1], f[0], indexing="ij"); Az = (np.sin(k * Y) + np.cos(k * X) + 0 * Z) / k
+        bx, by, bz = faces_from_potential(Ax, Ay, Az, dh)
+        K, J, I = np.meshgrid(ci[2] % n, ci[1] % n, ci[0] % n, indexing="ij")
+        lin = (K.astype(np.int64) * n + J) * n + I
+        v = [vamp * (2.0 * _hash_uniform(3 * lin + d, seed) - 1.0) for d in range(3)]
+        o = np.ones((T, T, T))
+        U_in[q] = conserved(o, v[0], v[1], v[2], p0 * o, bx, by, bz, gamma)
+        bxo[q], byo[q], bzo[q] = bx, by, bz
+    return U_in.reshape(G, -1), B_in, dh
+
+
 # ----------------------------------------------------------------------------------------
 # SURVEY 8(f) NEXT-4 second workload: the paper's 1-D Riemann problems (PAPER.md:266-292, Table 1)
 # ----------------------------------------------------------------------------------------

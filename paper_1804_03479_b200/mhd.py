@@ -10,7 +10,8 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBPATH = os.path.join(_HERE, "libmhd.so")
+# MHD_LIBPATH: another build of the same library (the IEEE-division control build of tests/fp32_controls.py)
+_LIBPATH = os.environ.get("MHD_LIBPATH") or os.path.join(_HERE, "libmhd.so")
 
 FP32, FP64 = 0, 1
 VL, CTU = 0, 1

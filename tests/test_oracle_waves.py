@@ -49,12 +49,14 @@ def _run_axis(oracle, scheme, recon, g, riemann, mode, axis, N):
 @pytest.mark.parametrize("name,scheme,recon,g,riemann", CASES)
 @pytest.mark.parametrize("mode", ["fast", "alfven", "slow"])
 def test_p5_axis_waves_converge_at_second_order(oracle, name, scheme, recon, g, riemann, mode):
+    """N = 16, 32, 64 (BASELINE.json north_star; Fig. 4: L1 error proportional to N^-2); bounds of SURVEY P5:
+    observed order >= 1.5 for 16 -> 32 and >= 1.7 for 32 -> 64 (a first-order bug shows as ~1.0)"""
     axis = {"fast": 0, "alfven": 1, "slow": 2}[mode]
-    e16 = _run_axis(oracle, scheme, recon, g, riemann, mode, axis, 16)[0]
-    e32 = _run_axis(oracle, scheme, recon, g, riemann, mode, axis, 32)[0]
-    order = np.log2(e16 / e32)
-    assert order > 1.5, (e16, e32, order)
-    assert e32 < 6e-8           # amplitude 1e-6: a first-order scheme leaves ~2e-7 at N = 32
+    e16, e32, e64 = (_run_axis(oracle, scheme, recon, g, riemann, mode, axis, N)[0] for N in (16, 32, 64))
+    o1, o2 = np.log2(e16 / e32), np.log2(e32 / e64)
+    print(f"P5 axis {name} {mode}: errors {e16:.3e} {e32:.3e} {e64:.3e}, orders {o1:.2f} {o2:.2f}")
+    assert o1 > 1.5 and o2 > 1.7, (e16, e32, e64, o1, o2)
+    assert e32 < 6e-8 and e64 < 1.6e-8      # amplitude 1e-6: a first-order scheme leaves ~2e-7 at N = 32
 
 
 def test_p5_axes_are_equivalent(oracle):
@@ -62,15 +64,28 @@ def test_p5_axes_are_equivalent(oracle):
     assert max(e) - min(e) < 1e-7 * max(e) + 1e-15
 
 
+def _run_diagonal(oracle, scheme, recon, g, riemann, mode, N):
+    U, bx, by, bz, dh, spd, lam = waves.diagonal_wave(N, mode)
+    assert H.rel_divb(bx, by, bz, dh) < 1e-13
+    cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon, riemann=riemann)
+    adv = lambda Ui, Bi, dt, dh_: oracle.advance(cfg, Ui, Bi, dt, dh_)
+    dt_fn = lambda U_, a, b, c, dh_, cfl: cfl * dh_ / 2.0
+    return waves.run_period(adv, dt_fn, U, bx, by, bz, dh, lam / spd, N, g)[0]
+
+
+# body diagonal of [0,1)^3 (the paper's set-up): every wave family for the two schemes of the configs at
+# N = 16, 32; the 32 -> 64 step for the fast wave (a 64^3 period of the slow wave costs minutes of oracle time)
+DIAG = [("vl_plm", 0, 0, 3, 1, "fast", (16, 32, 64)), ("vl_plm", 0, 0, 3, 1, "alfven", (16, 32)), ("vl_plm", 0, 0, 3, 1, "slow", (16, 32)),
+        ("ctu_ppm", 1, 1, 4, 1, "fast", (16, 32, 64)), ("ctu_ppm", 1, 1, 4, 1, "alfven", (16, 32)), ("ctu_ppm", 1, 1, 4, 1, "slow", (16, 32)),
+        ("vl_plm_roe", 0, 0, 3, 2, "fast", (16, 32)), ("ctu_plm", 1, 0, 3, 1, "fast", (16, 32)), ("ctu_ppm_roe", 1, 1, 4, 2, "fast", (16, 32))]
+
+
 @pytest.mark.slow
-@pytest.mark.parametrize("name,scheme,recon,g,riemann", [CASES[0], CASES[3]])
-def test_p5_diagonal_fast_wave(oracle, name, scheme, recon, g, riemann):
-    errs = []
-    for N in (16, 32):
-        U, bx, by, bz, dh, spd, lam = waves.diagonal_wave(N, "fast")
-        assert H.rel_divb(bx, by, bz, dh) < 1e-13
-        cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon, riemann=riemann)
-        adv = lambda Ui, Bi, dt, dh_: oracle.advance(cfg, Ui, Bi, dt, dh_)
-        dt_fn = lambda U_, a, b, c, dh_, cfl: cfl * dh_ / 2.0
-        errs.append(waves.run_period(adv, dt_fn, U, bx, by, bz, dh, lam / spd, N, g)[0])
-    assert np.log2(errs[0] / errs[1]) > 1.5, errs
+@pytest.mark.parametrize("name,scheme,recon,g,riemann,mode,Ns", DIAG)
+def test_p5_diagonal_waves(oracle, name, scheme, recon, g, riemann, mode, Ns):
+    errs = [_run_diagonal(oracle, scheme, recon, g, riemann, mode, N) for N in Ns]
+    orders = [float(np.log2(errs[i] / errs[i + 1])) for i in range(len(errs) - 1)]
+    print(f"P5 diagonal {name} {mode}: errors {errs}, orders {orders}")
+    assert orders[0] > 1.5, (errs, orders)
+    if len(orders) > 1:
+        assert orders[1] > 1.7, (errs, orders)
