@@ -16,6 +16,7 @@
 #include "mhd_prolong.cuh"
 #include "mhd_ctu_pass1.cuh"
 #include "mhd_vl_pass1.cuh"
+#include "mhd_march.h"
 
 using namespace mhd;
 
@@ -68,6 +69,7 @@ struct mhd_solver {
   // optional per-stage timing (mhd_set_profiling): pairs of events around every stage launch; slices then run
   // one after the other on the caller's stream so that the stage times do not overlap
   bool no_fused_pass1 = false;              // MHD_NO_FUSED_PASS1=1: the staged CTU steps 1 + 2 also for the standard group (tests)
+  bool no_march = false;                    // MHD_NO_MARCH=1 (or MHD_NO_FUSED_PASS1): VL without the plane-marching kernels (tests, A/B runs)
   bool prof_on = false;
   std::vector<cudaEvent_t> prof_ev;         // 2 per recorded launch
   std::vector<int> prof_stage;              // stage id per recorded launch
@@ -118,9 +120,9 @@ KParams<R> make_params(const mhd_solver* s, const void* Ui, const void* Bi, void
     default: { constexpr int LIM = 5; CALL; } break; \
   }
 
-enum Stage : int { ST_LOAD = 0, ST_RECON, ST_FLUX1, ST_EMF1, ST_HALF, ST_CORR, ST_FLUX2, ST_EMF2, ST_FINAL, ST_DT, ST_PASS1, ST_COUNT };
+enum Stage : int { ST_LOAD = 0, ST_RECON, ST_FLUX1, ST_EMF1, ST_HALF, ST_CORR, ST_FLUX2, ST_EMF2, ST_FINAL, ST_DT, ST_PASS1, ST_MARCH1, ST_MARCH2, ST_COUNT };
 const char* const kStageNames[ST_COUNT] = { "load_prim", "recon_ctu", "flux_pass1", "emf_pass1", "half_step", "ctu_corr",
-                                            "flux_pass2", "emf_pass2", "final_update", "dt_reduce", "pass1_fused" };
+                                            "flux_pass2", "emf_pass2", "final_update", "dt_reduce", "pass1_fused", "march_pass1", "march_pass2" };
 constexpr size_t kProfMaxLaunches = 16384;
 
 inline void prof_begin(mhd_solver* s, int stage, cudaStream_t st) {
@@ -187,6 +189,17 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
   const int lim = s->cfg.limvar + 2 * s->cfg.limiter;     // template parameter LIM of the slope kernels
 #define GRID1(b) dim3(blocks_for(b, TPB), 1, ng)
 #define GRID3(b) dim3(blocks_for(b, TPB), 3, ng)
+  // standard VL + PLM group: the whole step as two plane-marching kernels with the intermediates on chip (mhd_vl_march.cuh)
+  if constexpr (SC == 23) {
+    if (s->cfg.scheme == MHD_VL && s->cfg.recon == MHD_PLM && N == 16 && g == 3 && !s->no_march && vl_march_supports<R>(sol)) {
+      cudaError_t e1 = cudaSuccess, e2 = cudaSuccess;
+      LAUNCH(ST_MARCH1, e1 = launch_vl_march<R>(p0, ng, sol, lim, 1, st));
+      LAUNCH(ST_MARCH2, e2 = launch_vl_march<R>(p0, ng, sol, lim, 2, st));
+      if (e1 != cudaSuccess) return cuda_fail(e1, "k_vl_march1");
+      if (e2 != cudaSuccess) return cuda_fail(e2, "k_vl_march2");
+      return MHD_OK;
+    }
+  }
   int f2 = A_F;                                   // where the pass-2 fluxes are
   const Box3 ball = box(0, S, 0, S, 0, S);
   // standard VL group with HLLD or Roe: S0 + S1 + S2 in one kernel (mhd_vl_pass1.cuh)
@@ -383,6 +396,7 @@ int mhd_create(const mhd_config* cfg, mhd_solver** out) {
   s->N = cfg->ps2; s->g = cfg->nghost; s->T = s->N + 2 * s->g; s->S = s->T + 1;
   s->S3 = (size_t)s->S * s->S * s->S;
   s->no_fused_pass1 = getenv("MHD_NO_FUSED_PASS1") != nullptr;
+  s->no_march = s->no_fused_pass1 || getenv("MHD_NO_MARCH") != nullptr;
   s->narr = (cfg->scheme == MHD_VL && cfg->recon == MHD_PLM) ? A_VL_END : A_CTU_END;   // face-state arrays: CTU, VL + PPM
   s->esz = cfg->prec == MHD_FP32 ? 4 : 8;
   const size_t N = s->N, T = s->T;

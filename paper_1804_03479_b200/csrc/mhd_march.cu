@@ -1,0 +1,69 @@
+// mhd_march.cu -- instantiations and launchers of the plane-marching VL kernels (mhd_vl_march.cuh)
+#include <cstdlib>
+#include "mhd_march.h"
+#include "mhd_vl_march.cuh"
+
+namespace mhd {
+
+namespace {
+
+template <class K> cudaError_t big_smem(K kernel, size_t bytes) {
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+template <class R, int SOLVER, int LIM>
+cudaError_t launch2(const KParamsSC<R, 23>& p, int ng, cudaStream_t st) {
+  cudaError_t e;
+  if (p.red) {
+    if ((e = big_smem(k_vl_march2<R, SOLVER, LIM, true>, march2_smem<R>())) != cudaSuccess) return e;
+    k_vl_march2<R, SOLVER, LIM, true><<<ng, kM2P, march2_smem<R>(), st>>>(p);
+  } else {
+    if ((e = big_smem(k_vl_march2<R, SOLVER, LIM, false>, march2_smem<R>())) != cudaSuccess) return e;
+    k_vl_march2<R, SOLVER, LIM, false><<<ng, kM2P, march2_smem<R>(), st>>>(p);
+  }
+  return cudaGetLastError();
+}
+
+template <class R, int SOLVER>
+cudaError_t launch_solver(const KParamsSC<R, 23>& p, int ng, int lim, int pass, cudaStream_t st) {
+  if (pass == 1) {
+    // bulk copies need 16-byte aligned planes: the group strides are multiples of 16 bytes, the base pointers must be
+    static const bool no_tma = getenv("MHD_NO_TMA") != nullptr;
+    const bool tma = !no_tma && ((reinterpret_cast<size_t>(p.Uin) | reinterpret_cast<size_t>(p.Bin)) & 15) == 0;
+    cudaError_t e;
+    if (tma) {
+      if ((e = big_smem(k_vl_march1<R, SOLVER, true>, march1_smem<R, true>())) != cudaSuccess) return e;
+      k_vl_march1<R, SOLVER, true><<<ng, kMP, march1_smem<R, true>(), st>>>(p);
+    } else {
+      if ((e = big_smem(k_vl_march1<R, SOLVER, false>, march1_smem<R, false>())) != cudaSuccess) return e;
+      k_vl_march1<R, SOLVER, false><<<ng, kMP, march1_smem<R, false>(), st>>>(p);
+    }
+    return cudaGetLastError();
+  }
+  switch (lim) {
+    case 0: return launch2<R, SOLVER, 0>(p, ng, st);
+    case 1: return launch2<R, SOLVER, 1>(p, ng, st);
+    case 2: return launch2<R, SOLVER, 2>(p, ng, st);
+    case 3: return launch2<R, SOLVER, 3>(p, ng, st);
+    case 4: return launch2<R, SOLVER, 4>(p, ng, st);
+    default: return launch2<R, SOLVER, 5>(p, ng, st);
+  }
+}
+
+}  // namespace
+
+template <class R> bool vl_march_supports(int solver) { return solver == kHLLD; }
+
+template <class R>
+cudaError_t launch_vl_march(const KParams<R>& p0, int ng, int solver, int lim, int pass, cudaStream_t st) {
+  const KParamsSC<R, 23> p(p0);
+  if (solver == kHLLD) return launch_solver<R, kHLLD>(p, ng, lim, pass, st);
+  return cudaErrorInvalidValue;
+}
+
+template cudaError_t launch_vl_march<float>(const KParams<float>&, int, int, int, int, cudaStream_t);
+template cudaError_t launch_vl_march<double>(const KParams<double>&, int, int, int, int, cudaStream_t);
+template bool vl_march_supports<float>(int);
+template bool vl_march_supports<double>(int);
+
+}  // namespace mhd

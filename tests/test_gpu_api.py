@@ -8,6 +8,7 @@ import pytest
 from paper_1804_03479_b200 import inputs
 import harness as H
 import gpu_util as GU
+import parity_cases as PC
 
 pytestmark = pytest.mark.gpu
 
@@ -308,13 +309,58 @@ def test_configs_3_4_full_size_256_cubed_on_sampled_groups(oracle, which, prec):
     ref = oracle.advance(cfg, Ui[sample].astype(np.float64), Bi[sample].astype(np.float64), dt, dh)
     errs = GU.field_errors({k: out[k][sample] for k in out}, ref, N)
     if prec == 0:
-        # |M|, the mass flux and the EMF (~ v B) are 1e-2 of the momentum-flux scale on this config
-        for k in ("Mx", "My", "Mz", "flux_rho", "emf"):
-            assert errs.pop(k) <= 1e-3
-    assert max(errs.values()) <= (1e-12 if prec == 1 else 1e-4), errs
+        # R14b: |M|, the mass flux and the EMF (~ v B) are 1e-2 of the momentum-flux scale on this
+        # config, so the plain algorithm in IEEE single precision (the FP32 oracle) is itself up to 7.6e-4 (emf) away from
+        # the FP64 oracle after ONE step.  Gate per field: max(1e-4, 2 x that); measured GPU / gate <= 0.42
+        # (profiles/r02_fp32_controls.md)
+        r32 = oracle.advance32(cfg, Ui[sample], Bi[sample], dt, dh)
+        gate = PC.fp32_gate(GU.field_errors(r32, ref, N))
+        for k in ("rho", "e", "Bx", "By", "Bz", "flux_Mx", "flux_My", "flux_Mz"):
+            assert gate[k] == 1e-4, (k, gate[k])
+        bad = {k: (v, gate[k]) for k, v in errs.items() if not v <= gate[k]}
+        assert not bad, (bad, errs)
+    else:
+        assert max(errs.values()) <= 1e-12, errs
     Un, bxn, byn, bzn, mism = inputs.unpack_groups(out["U"], out["B"], n, N)
     assert mism == 0.0
     assert H.rel_divb(bxn.astype(np.float64), byn.astype(np.float64), bzn.astype(np.float64), dh) < (1e-13 if prec == 1 else 2e-5)
     t0, t1 = H.totals(U), H.totals(Un)
     tol = 1e-13 if prec == 1 else 2e-6
     assert abs(t1[0] - t0[0]) / t0[0] < tol and abs(t1[4] - t0[4]) / t0[4] < tol
+
+
+@pytest.mark.parametrize("scheme,recon,g", [(0, 0, 3), (1, 1, 4)])
+@pytest.mark.parametrize("nstreams", [3, 4])
+def test_config5_first_batch_through_the_host_path(oracle, scheme, recon, g, nstreams):
+    """BASELINE.json configs[4]: the first 512-group batch of the 1024^3 ABC state (dh = 1/1024, generated group by group:
+    inputs.abc_groups), FP32, VL+PLM and CTU+PPM, through mhd_advance_host_dt in 32-group chunks on 3 / 4 streams (a ragged
+    last chunk with 3: 512 = 15 x 32 + 32 on lanes 0, 1, 2, 0, ...; and a ragged batch of 500 groups).  16 sampled groups
+    against the FP64 oracle at the gate of R14b (max(1e-4, 2 x the FP32 oracle's error)); div B of every group at
+    round-off; the returned dt equals the CFL reduction of the output."""
+    import torch
+    N, G = 16, 512 if nstreams == 4 else 500
+    dtp = np.float32
+    Ui, Bi, dh = inputs.abc_groups(1024, 0, G, N, g, dtype=dtp)
+    sample = list(range(3, G, 32))
+    cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon, emf_tie=1e-5)
+    dt, _ = oracle.dt_reduce(cfg, Ui.astype(np.float64), Bi.astype(np.float64), g, dh, 0.3)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=scheme, recon=recon, prec=0, max_groups=G)
+    s = gpu.solver
+    hU, hB = torch.from_numpy(Ui).pin_memory(), torch.from_numpy(Bi).pin_memory()
+    ho = {k: torch.empty((G, n), dtype=torch.float32).pin_memory() for k, n in
+          (("U", s.n_U_out), ("B", s.n_B_out), ("flux", s.n_flux), ("emf", s.n_emf))}
+    dt_next, smax = s.advance_host_dt(hU, hB, ho["U"], ho["B"], ho["flux"], ho["emf"], G, dt, dh, 32, nstreams, 0.3)
+    out = {k: v.numpy() for k, v in ho.items()}
+    ref = oracle.advance(cfg, Ui[sample].astype(np.float64), Bi[sample].astype(np.float64), dt, dh)
+    r32 = oracle.advance32(cfg, Ui[sample], Bi[sample], dt, dh)
+    gate = PC.fp32_gate(GU.field_errors(r32, ref, N))
+    errs = GU.field_errors({k: out[k][sample] for k in out}, ref, N)
+    bad = {k: (v, gate[k]) for k, v in errs.items() if not v <= gate[k]}
+    assert not bad, (bad, errs)
+    for k in ("rho", "e", "Bx", "By", "Bz", "flux_Mx", "flux_My", "flux_Mz"):
+        assert gate[k] == 1e-4 and errs[k] <= 1e-4
+    bx, by, bz = inputs.split_B(out["B"].astype(np.float64), N)
+    assert H.rel_divb(bx, by, bz, dh) < 2e-5 * 64            # FP32 round-off of b ~ 1 over dh = 1/1024 against the 16^3 boxes' 1/16
+    dt_ref, _ = oracle.dt_reduce(cfg, out["U"].astype(np.float64), out["B"].astype(np.float64), 0, dh, 0.3)
+    assert abs(dt_next - dt_ref) <= 1e-6 * dt_ref
+    assert gpu.stats() == (0, 0, 0)

@@ -8,6 +8,7 @@ import pytest
 from paper_1804_03479_b200 import inputs
 import harness as H
 import gpu_util as GU
+import parity_cases as PC
 
 pytestmark = pytest.mark.gpu
 
@@ -16,7 +17,7 @@ TOL_ONE_STEP = {1: 2e-13, 0: 1e-4}
 SCHEMES = [("vl_plm", 0, 0, 3), ("ctu_plm", 1, 0, 3), ("ctu_ppm", 1, 1, 4)]
 
 
-EMF_TIE = {1: 1e-12, 0: 1e-5}   # DESIGN.md R10a: the tie width is part of the method and follows the working precision
+EMF_TIE = PC.EMF_TIE   # DESIGN.md R10a: the tie width is part of the method and follows the working precision
 
 
 def oracle_fn(oracle, N, g, scheme, recon, riemann, limvar, prec=1):
@@ -101,37 +102,37 @@ def test_config1_abc32_vl_plm_fp64_10_steps(oracle):
 # ---------------------------------------------------------------------------------------------------------------
 # config 2: batch of independent 16^3 boxes (each its own periodic domain), VL+PLM+CT, FP64 and FP32, 10 steps
 # ---------------------------------------------------------------------------------------------------------------
+def _fp32_reference(oracle, cfg):
+    """the oracle instantiated in single precision (oracle/mhd_oracle_f32.cpp): its distance from the FP64 oracle is the
+    error inherent to the plain algorithm in IEEE single precision and sets the FP32 gate (R14b)"""
+    return lambda Ui, Bi, dt, dh: oracle.advance32(cfg, Ui, Bi, dt, dh)
+
+
 @pytest.mark.parametrize("prec", [1, 0])
 def test_config2_batch_vl_plm_10_steps(oracle, prec):
     N, g, G = 16, 3, 24
     dtp = GU.np_dtype(prec)
-    boxes0 = []
-    for q in range(G):
-        U, bx, by, bz, dh = inputs.random_group_grid(N, 3479 + q)
-        # FP32 runs start from the FP32-rounded state on both sides (R14)
-        boxes0.append(tuple(a.astype(dtp).astype(np.float64) for a in (U, bx, by, bz)))
+    boxes0, dh = PC.config2_boxes(G, N, prec)
     cfg, adv = oracle_fn(oracle, N, g, 0, 0, 1, 0, prec)
+    dts, ref_boxes, ref_out, _ = PC.run_boxes_oracle(oracle, cfg, boxes0, dh, N, g)
     gpu = GU.GpuRunner(N=N, g=g, scheme=0, recon=0, riemann=1, prec=prec, max_groups=G)
-    ref_boxes, gpu_boxes = boxes0, [tuple(a.astype(dtp) for a in b) for b in boxes0]
-    ref_out = gpu_out = None
-    for step in range(10):
-        Ui, Bi = H.pack_boxes(ref_boxes, N, g)
-        dt, _ = oracle.dt_reduce(cfg, Ui, Bi, g, dh, 0.3)
-        ref_boxes, ref_out = H.step_boxes(adv, ref_boxes, dt, dh, N, g)
-        gpu_boxes, gpu_out = H.step_boxes(gpu, gpu_boxes, dt, dh, N, g, dtype=dtp)
-    # DESIGN.md R14a: in a group whose pressure floor fires, P = (gamma-1)(e - KE - ME) is the difference of numbers 1e5+
-    # times larger, i.e. rounding noise in FP32; the time-centred plane fluxes of such a group are held to
-    # 5e-4 of the batch maximum, everything else (all fields of all groups, planes of the other groups) to 1e-4
-    floored = np.array([oracle.advance(cfg, Ui[q:q + 1], Bi[q:q + 1], dt, dh)["stats"][1] > 0 for q in range(G)])
-    sel = lambda out, m: {k: (np.asarray(v)[m] if v is not None else None) for k, v in out.items() if k in ("U", "B", "flux", "emf")}
-    if prec == 0 and floored.any():
-        clean = ~floored
-        assert_fields(GU.field_errors(sel(gpu_out, clean), sel(ref_out, clean), N), TOL[prec], "config 2 FP32, groups without floor events")
-        e_all = GU.field_errors(gpu_out, ref_out, N)
-        assert_fields({k: v for k, v in e_all.items() if not k.startswith(("flux", "emf"))}, TOL[prec], "config 2 FP32, fields of all groups")
-        assert_fields({k: v for k, v in e_all.items() if k.startswith(("flux", "emf"))}, 5e-4, "config 2 FP32, planes of floored groups")
+    gpu_boxes, gpu_out = PC.run_boxes(gpu, boxes0, dts, dh, N, g, dtp)
+    errs = PC.boxes_errors(gpu_boxes, ref_boxes)
+    errs.update({k: v for k, v in GU.field_errors(gpu_out, ref_out, N).items() if k.startswith(("flux", "emf"))})
+    if prec == 1:
+        assert_fields(errs, TOL[1], "config 2 FP64, state and planes of step 10")
     else:
-        assert_fields(GU.field_errors(gpu_out, ref_out, N), TOL[prec], f"config 2 prec={prec} outputs of step 10")
+        # every field of every group -- also the planes of the groups whose pressure floor fires (floors fire in 7 of the
+        # 24 groups from step 6 on) -- at the north-star 1e-4, or 2 x the FP32 oracle's own error where that is larger
+        # (it is not on this config: measured <= 3.3e-5, profiles/r02_fp32_controls.md)
+        b32, o32 = PC.run_boxes(_fp32_reference(oracle, cfg), boxes0, dts, dh, N, g, np.float32)
+        e32 = PC.boxes_errors(b32, ref_boxes)
+        e32.update({k: v for k, v in GU.field_errors(o32, ref_out, N).items() if k.startswith(("flux", "emf"))})
+        gate = PC.fp32_gate(e32)
+        assert max(gate.values()) <= 1e-4 + 1e-12, gate       # the inherent FP32 error itself stays below 5e-5 here
+        bad = {k: (v, gate[k]) for k, v in errs.items() if not v <= gate[k]}
+        assert not bad, f"config 2 FP32 over the gate (R14b): {bad}; all {errs}; oracle-FP32 {e32}"
+        assert ref_out["stats"][1] > 0                       # the floors did fire: that path is inside the gate
     for q in range(G):
         bx, by, bz = (np.asarray(a, dtype=np.float64) for a in gpu_boxes[q][1:])
         assert H.rel_divb(bx, by, bz, dh) < (1e-13 if prec == 1 else 2e-5)
@@ -144,21 +145,28 @@ def test_config2_batch_vl_plm_10_steps(oracle, prec):
 def test_config3_abc_ctu_ppm_10_steps(oracle, prec):
     n, N, g = 64, 16, 4
     dtp = GU.np_dtype(prec)
-    U, bx, by, bz, dh = inputs.abc_grid(n, seed=1805, p0=0.15, vamp=1e-2)
-    U, bx, by, bz = (a.astype(dtp).astype(np.float64) for a in (U, bx, by, bz))
+    state0, dh = PC.config3_grid(n, prec)
     cfg, adv = oracle_fn(oracle, N, g, 1, 1, 1, 1, prec)
-    dts, ref, ref_out = oracle_dt_sequence(oracle, adv, U, bx, by, bz, dh, N, g, 10)
+    dts, ref, ref_out = PC.run_grid_oracle(oracle, adv, state0, dh, N, g)
     gpu = GU.GpuRunner(N=N, g=g, scheme=1, recon=1, riemann=1, limvar=1, prec=prec, max_groups=64)
-    res = run_grid(gpu, U.astype(dtp), bx.astype(dtp), by.astype(dtp), bz.astype(dtp), dts, dh, N, g, dtype=dtp)
-    errs = grid_errors(res, ref)
-    if prec == 0:
-        # |M| <= 1.2e-2 here while the momentum flux is O(pT) = 3.2: the FP32 rounding of the flux differences alone
-        # is ~3e-7 per step = 3e-5 max|M| (measured, every variant), and on this grid-scale-noisy velocity field the
-        # limiters let isolated cells drift to 1e-4..7e-4 max|M| within 10 steps.  Every other
-        # field meets the north-star 1e-4 with two orders of margin; momentum is held to 1e-3 max|M| = 1.2e-5 absolute.
-        for k in ("Mx", "My", "Mz"):
-            assert errs.pop(k) <= 1e-3
-    assert_fields(errs, TOL[prec], f"config 3 prec={prec}")
+    res, gpu_out = PC.run_grid(gpu, state0, dts, dh, N, g, dtype=dtp)
+    errs = PC.grid_errors(res, ref)
+    errs.update({k: v for k, v in GU.field_errors(gpu_out, ref_out, N).items() if k.startswith(("flux", "emf"))})
+    if prec == 1:
+        assert_fields(errs, TOL[1], "config 3 FP64")
+    else:
+        # R14b: |M| <= 1.2e-2 here while the momentum flux is O(pT) = 3.2, so the plain algorithm in
+        # IEEE single precision (the FP32 oracle) is itself 2.4e-4 .. 8.8e-4 of max|M| away from the FP64 oracle after 10
+        # steps, and 2.6e-4 / 1.9e-4 / 5.5e-4 in the mass flux, energy flux and EMF planes.  Gate per field:
+        # max(1e-4, 2 x that); measured GPU / gate <= 0.4 (profiles/r02_fp32_controls.md).  rho, e, B, momentum fluxes: 1e-4.
+        s32, o32 = PC.run_grid(_fp32_reference(oracle, cfg), state0, dts, dh, N, g, dtype=np.float32)
+        e32 = PC.grid_errors(s32, ref)
+        e32.update({k: v for k, v in GU.field_errors(o32, ref_out, N).items() if k.startswith(("flux", "emf"))})
+        gate = PC.fp32_gate(e32)
+        for k in ("rho", "e", "Bx", "By", "Bz", "flux_Mx", "flux_My", "flux_Mz"):
+            assert gate[k] == 1e-4, (k, gate[k])
+        bad = {k: (v, gate[k]) for k, v in errs.items() if not v <= gate[k]}
+        assert not bad, f"config 3 FP32 over the gate (R14b): {bad}; all {errs}; oracle-FP32 {e32}"
     assert H.rel_divb(*(np.asarray(a, dtype=np.float64) for a in res[1:4]), dh) < (1e-13 if prec == 1 else 2e-5)
     assert gpu.stats() == (0, 0, 0)
 
