@@ -29,18 +29,39 @@ sys.path.insert(0, ROOT)
 
 N_PS2, NGROUPS = 16, 512
 PAPER_P100 = {"f32": 1.2e8, "f64": 5.5e7}       # PAPER.md:12, :465-467 (Tesla P100, VL+PLM+Roe) -- context only
-# algorithmic work per Riemann solve and per group, DESIGN.md "Roofline arithmetic"
-# exact operation counts of the oracle instantiated with a counting scalar (oracle/count_ops.cpp; add/sub/mul/div/sqrt = 1)
+# Algorithmic work: exact operation counts of the oracle instantiated with a counting scalar
+# (oracle/count_ops.cpp; add / sub / mul / div / sqrt = 1 each), pinned to that tool's output by tests/test_op_counts.py.
 FLOP_PER_SOLVE = {"hlld": 381, "roe": 1107, "hlle": 361}
-FLOP_PER_CELL_UPDATE = {("vl", "hlld"): 6263.5, ("vl", "roe"): 15289.0, ("ctu", "hlld"): 26067.6, ("ctu", "roe"): 35160.4}   # whole step
-FLOP_PLM_PER_FACE = 140     # two MC-limited primitive slopes + the two face states (VL pass 2)
-# dram__bytes_read.sum + dram__bytes_write.sum of each stage's launches of one 512-group step (two slices of 256), VL+PLM+HLLD, from the
-# ncu --set full captures summarised in profiles/r01h_full_top_kernels.md and r01h_f64_full_top_kernels.md (MB)
-NCU_TRAFFIC_MB = {"f32": {"pass1_fused": 968.0, "emf_pass1": 351.3, "half_step": 856.6, "flux_pass2": 609.4,
-                          "emf_pass2": 229.2, "final_update": 418.6},
-                  "f64": {"pass1_fused": 1756.3, "emf_pass1": 691.7, "half_step": 1631.1, "flux_pass2": 1058.2,
-                          "emf_pass2": 438.1, "final_update": 831.7}}
+# whole step per interior cell-update: "max" = on the oracle's maximal index ranges, "min" = every stage only where the final update
+# needs it (mhdref_config.minimal_ranges; the device's ranges): the work the method itself requires
+FLOP_PER_CELL_UPDATE = {("vl", "hlld"): {"max": 6127.4, "min": 5586.4}, ("vl", "roe"): {"max": 15153.0, "min": 13924.0},
+                        ("ctu", "hlld"): {"max": 25945.8, "min": 18657.6}, ("ctu", "roe"): {"max": 35038.5, "min": 25627.7}}
+# flops per patch group of the seven steps of the update on the minimal ranges: con->prim, pass-1 fluxes (CTU: + reconstruction),
+# EMF-1, half step, pass-2 states + fluxes, EMF-2, full update
+FLOP_PER_GROUP_STEPS = {("vl", "hlld"): [276848, 11617452, 1230060, 654004, 8236384, 638118, 229122],
+                        ("vl", "roe"): [276848, 33754644, 1230060, 654004, 20249952, 638118, 229122],
+                        ("ctu", "hlld"): [359426, 64502472, 896730, 477254, 9318565, 638118, 229122],
+                        ("ctu", "roe"): [359426, 81055272, 896730, 477254, 21314989, 638118, 229122]}
+# which steps each profiled stage (mhd_set_profiling) covers; stages that share a step are timed together
+STAGE_STEPS = {"march_pass1": (1, 2, 3, 4), "march_pass2": (5, 6, 7), "emf_pass1": (3,), "half_step": (4,), "flux_pass2": (5,), "emf_pass2": (6,),
+               "final_update": (7,)}
 NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_dram_traffic.csv")
+E2E_CHUNK, E2E_STREAMS = 32, 4                  # measured best of chunk x streams on this box (PCIe-bound)
+
+
+def ncu_traffic():
+    """profiles/r02_dram_traffic.csv (written from ncu --set full captures, command in profiles/r02_dram_traffic.md):
+    {(scheme, riemann, prec): {stage: (launches per 512-group step, MB read + written per launch)}}; {} if the file is missing"""
+    out = {}
+    try:
+        import csv
+        for r in csv.DictReader(open(TRAFFIC_CSV)):
+            key = (r["scheme"], r["riemann"], r["prec"])
+            out.setdefault(key, {})[r["stage"]] = (float(r["launches_per_step"]), float(r["dram_read_MB"]) + float(r["dram_write_MB"]))
+    except Exception:
+        pass
+    return out
 
 
 def parse():
@@ -54,6 +75,8 @@ def parse():
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"], help="precision of the headline value")
     ap.add_argument("--groups", type=int, default=NGROUPS)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    ap.add_argument("--main-only", action="store_true", help="only the headline arm and its other precision (no ctu / roe / config5 sub-records)")
     ap.add_argument("--config5", type=int, default=0, metavar="POOL", help="instead of the batch: BASELINE config 5, 262144 "
                     "group-updates (= 1024^3 cells) in FP32 streamed from a pinned pool of POOL groups (a multiple of 512, e.g. 4096), "
                     "VL+PLM and CTU+PPM, with and without transfers")
@@ -132,27 +155,71 @@ def hbm_peak():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+_BATCH_CACHE = {}
+
+
 def make_batch(G, g, npdt):
-    """config-2 batch: a pool of 16 distinct seeded groups tiled to G (the kernels' work does not depend on values)."""
+    """config-2 batch (BASELINE.json configs[1]): G DISTINCT seeded patch groups (seed 3479 + group id): the branch pattern of
+    the Riemann solver, the floors and the upwind ramp depend on the values"""
     import numpy as np
     from paper_1804_03479_b200 import inputs
-    pool = min(G, 16)
-    U, B, dh = inputs.config2_batch(pool, N=N_PS2, g=g, dtype=npdt)
-    reps = (G + pool - 1) // pool
-    return np.tile(U, (reps, 1))[:G].copy(), np.tile(B, (reps, 1))[:G].copy(), dh
+    key = (G, g)
+    if key not in _BATCH_CACHE:
+        _BATCH_CACHE[key] = inputs.config2_batch(G, N=N_PS2, g=g, dtype=np.float64)
+    U, B, dh = _BATCH_CACHE[key]
+    return U.astype(npdt), B.astype(npdt), dh
 
 
-def measure(args, prec_name, rank, world, dist):
+def pcie_peaks(dev, nbytes=256 << 20):
+    """pinned host <-> device copy bandwidth of this box, measured in the same run: H2D alone, D2H alone, both at once (GB/s)"""
+    import torch
+    h1, h2 = torch.empty(nbytes, dtype=torch.uint8).pin_memory(), torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    d1, d2 = torch.empty(nbytes, dtype=torch.uint8, device=dev), torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    s1, s2 = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+
+    def run(h2d, d2h, reps=4):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            if h2d:
+                with torch.cuda.stream(s1):
+                    d1.copy_(h1, non_blocking=True)
+            if d2h:
+                with torch.cuda.stream(s2):
+                    h2.copy_(d2, non_blocking=True)
+        torch.cuda.synchronize()
+        return (int(h2d) + int(d2h)) * nbytes * reps / (time.perf_counter() - t0) / 1e9
+    run(True, True, 1)
+    return {"h2d_GBs": run(True, False), "d2h_GBs": run(False, True), "bidirectional_GBs": run(True, True)}
+
+
+def merge_stages(stages):
+    """profiled stages -> roofline units: the stages that share steps 1-2 of the update (tile staging / con->prim, reconstruction,
+    pass-1 Riemann solves) are timed together; returns {unit: {ms_per_step, launches_per_step, steps}}"""
+    out = {k: dict(v, steps=STAGE_STEPS.get(k)) for k, v in stages.items()}
+    parts = [k for k in ("load_prim", "recon_ctu", "flux_pass1", "pass1_fused") if k in out]
+    if parts:
+        ms = sum(out[k]["ms_per_step"] for k in parts)
+        nl = max(out[k]["launches_per_step"] for k in parts)
+        for k in parts:
+            del out[k]
+        out["+".join(parts)] = {"ms_per_step": ms, "launches_per_step": nl, "steps": (1, 2)}
+    return out
+
+
+def measure(args, prec_name, rank, world, dist, scheme=None, riemann=None, steps=None, e2e=True, pcie=None):
     """Time K steps of mhd_advance_dt on device-resident data, then the per-stage profile, then e2e."""
     import numpy as np
     import torch
     from paper_1804_03479_b200 import mhd, shard
-    sp = scheme_params(args)
+    a2 = argparse.Namespace(**{**vars(args), "scheme": scheme or args.scheme, "riemann": riemann or args.riemann})
+    sp = scheme_params(a2)
+    steps = steps or args.steps
     g, G = sp["g"], args.groups
     prec = mhd.FP32 if prec_name == "f32" else mhd.FP64
     npdt = np.float32 if prec_name == "f32" else np.float64
     esz = 4 if prec_name == "f32" else 8
-    riem = {"hlle": mhd.HLLE, "hlld": mhd.HLLD, "roe": mhd.ROE}[args.riemann]
+    riem = {"hlle": mhd.HLLE, "hlld": mhd.HLLD, "roe": mhd.ROE}[a2.riemann]
     dev = torch.device("cuda", torch.cuda.current_device())
     solver = mhd.Solver(mhd.make_config(N=N_PS2, g=g, scheme=sp["scheme"], recon=sp["recon"], riemann=riem, prec=prec,
                                         max_groups=G, device=dev.index))
@@ -181,7 +248,7 @@ def measure(args, prec_name, rank, world, dist):
     barrier()
     sampler.start()
     e0.record(stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     e1.record(stream)
     barrier()
@@ -189,113 +256,125 @@ def measure(args, prec_name, rank, world, dist):
     ms = e0.elapsed_time(e1)
     launches = solver.launch_count() - l0
     ms = shard.max_over_ranks(ms, dist, dev)          # job time = slowest rank's device time
-    cells = G * N_PS2 ** 3 * args.steps * world
-    res = dict(value=cells / (ms * 1e-3), ms_per_step=ms / args.steps, launches=launches, clocks=clocks)
+    cells = G * N_PS2 ** 3 * steps * world
+    res = dict(value=cells / (ms * 1e-3), ms_per_step=ms / steps, launches=launches, clocks=clocks, steps=steps,
+               variant="%s+%s" % (sp["name"], a2.riemann.upper()))
 
-    # per-stage device time over K more steps (events around every stage launch on the launching stream)
+    # per-stage device time over K more steps (events around every stage launch on the launching stream; the slices of a
+    # step then run one after the other, so the stage times add up to a little more than the overlapped step)
     solver.set_profiling(True)
     p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     p0.record(stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     p1.record(stream)
     torch.cuda.synchronize()
     prof = solver.get_profile()
     solver.set_profiling(False)
     prof_ms = p0.elapsed_time(p1)
-    stages = {k: {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps} for k, v in prof.items() if v[1]}
-    f1, f2 = faces_per_group(g, args.scheme)
-    fl = FLOP_PER_SOLVE[args.riemann]
-    top = max(stages, key=lambda k: stages[k]["ms_per_step"])
-    flops_stage = {"flux_pass1": fl * f1 * G, "flux_pass2": (fl + (FLOP_PLM_PER_FACE if args.scheme == "vl" else 0)) * f2 * G}
-    if args.scheme == "vl":
-        # S0-S2 in one kernel: the pass-1 Riemann solves + con->prim and the reference EMFs of the T^3 cells (27 + 9 flops each)
-        flops_stage["pass1_fused"] = (fl * f1 + 36 * (N_PS2 + 2 * g) ** 3) * G
+    stages = {k: {"ms_per_step": v[0] / steps, "launches_per_step": v[1] / steps} for k, v in prof.items() if v[1]}
+    key = (a2.scheme, a2.riemann)
+    units = merge_stages(stages)
     roof = None
-    if top in flops_stage:
-        n_launch = stages[top]["launches_per_step"]
-        dur = stages[top]["ms_per_step"] / n_launch * 1e-3            # average launch duration
-        ach = flops_stage[top] / n_launch / dur / 1e12
-        peak = NOMINAL_TFLOPS[prec_name]
-        roof = {"bound": "alu", "kernel": top, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                "peak_source": "nominal: 148 SMs x %d FMA lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if prec_name == "f32" else 64),
-                "peak_fma_measured": mhd.measure_fma_peak(dev.index, prec),
-                "traffic": (NCU_TRAFFIC_MB[prec_name][top] * 1e6 / n_launch if (args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS
-                                                                                   and top in NCU_TRAFFIC_MB[prec_name]) else None),
-                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum of the stage's launches of one step, "
-                                "profiles/r01h_*, / launches per step)",
-                "avg_launch_ms": dur * 1e3, "launches_per_step": n_launch,
-                "share_of_step": stages[top]["ms_per_step"] / (prof_ms / args.steps)}
+    step_flops = FLOP_PER_GROUP_STEPS.get(key)
+    traffic = ncu_traffic().get((a2.scheme, a2.riemann, prec_name), {}) if G == NGROUPS else {}
+    if step_flops:
+        top = max(units, key=lambda k: units[k]["ms_per_step"])
+        if units[top]["steps"]:
+            n_launch = units[top]["launches_per_step"]
+            dur = units[top]["ms_per_step"] / n_launch * 1e-3            # average launch duration
+            fl = sum(step_flops[i - 1] for i in units[top]["steps"]) * G   # algorithmic flops of the steps this kernel covers, per step
+            ach = fl / n_launch / dur / 1e12
+            peak = NOMINAL_TFLOPS[prec_name]
+            trs = [traffic[k] for k in top.split("+") if k in traffic]
+            tr = (n_launch, sum(a * b for a, b in trs) / n_launch) if len(trs) == len(top.split("+")) else None
+            roof = {"bound": "alu", "kernel": top, "steps_covered": list(units[top]["steps"]), "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                    "frac": ach / peak, "flops_per_launch": fl / n_launch,
+                    "peak_source": "nominal: 148 SMs x %d FMA lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if prec_name == "f32" else 64),
+                    "peak_fma_measured": mhd.measure_fma_peak(dev.index, prec),
+                    "traffic": (tr[1] * 1e6 if tr else None),
+                    "traffic_unit": "bytes per launch: ncu dram__bytes_read.sum + dram__bytes_write.sum, read at run time from "
+                                    "profiles/r02_dram_traffic.csv (a %d-group launch)" % int(round(G / max(n_launch, 1))),
+                    "avg_launch_ms": dur * 1e3, "launches_per_step": n_launch,
+                    "share_of_step": units[top]["ms_per_step"] / (prof_ms / steps)}
     # HBM view of the whole step: algorithmic bytes = read the ghost-zoned tile once, write the results once (the CFL
     # reduction is fused into the final update: no second read of the new state)
     sz = solver.sizes()
     bytes_step = (sz["n_U_in"] + sz["n_B_in"] + sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]) * esz * G
-    if args.scheme == "vl" and args.riemann == "hlld" and G == NGROUPS and set(stages) == set(NCU_TRAFFIC_MB[prec_name]):
-        tot = sum(NCU_TRAFFIC_MB[prec_name].values()) * 1e6
-        res["dram_traffic"] = {"bytes_per_step_ncu": tot, "GBs": tot / 1e9 / (res["ms_per_step"] * 1e-3),
+    if traffic and all(k in traffic for k in stages):
+        tot = sum(traffic[k][0] * traffic[k][1] for k in stages) * 1e6
+        res["dram_traffic"] = {"bytes_per_step_ncu": tot, "over_algorithmic": tot / bytes_step, "GBs": tot / 1e9 / (res["ms_per_step"] * 1e-3),
                                "frac_of_hbm_peak": tot / 1e9 / (res["ms_per_step"] * 1e-3) / hbm_peak()[0],
-                               "note": "all stage kernels of one step; the intermediates between stages go through HBM"}
-    fpc = FLOP_PER_CELL_UPDATE.get((args.scheme, args.riemann))
+                               "source": "profiles/r02_dram_traffic.csv, all stage kernels of one 512-group step"}
+    fpc = FLOP_PER_CELL_UPDATE.get(key)
     if fpc:
-        tf = fpc * res["value"] / world / 1e12
-        res["alu_whole_step"] = {"flops_per_cell_update": fpc, "achieved_TFLOPs": tf, "frac_of_nominal_peak": tf / NOMINAL_TFLOPS[prec_name],
-                                 "note": "oracle's exact operation count on its maximal index ranges (oracle/count_ops.cpp) x measured cell-updates/s"}
-    res.update(stages=stages, roofline=roof, profiled_ms_per_step=prof_ms / args.steps,
+        tf = {k: v * res["value"] / world / 1e12 for k, v in fpc.items()}
+        res["alu_whole_step"] = {"flops_per_cell_update_minimal_ranges": fpc["min"], "flops_per_cell_update_oracle_ranges": fpc["max"],
+                                 "achieved_TFLOPs": tf["min"], "frac_of_nominal_peak": tf["min"] / NOMINAL_TFLOPS[prec_name],
+                                 "achieved_TFLOPs_oracle_ranges": tf["max"],
+                                 "note": "exact operation count of the oracle (oracle/count_ops.cpp) on the minimal index ranges (the work the "
+                                         "method requires = the device's ranges) x measured cell-updates/s; the maximal-range count beside it"}
+    res.update(stages=stages, roofline=roof, profiled_ms_per_step=prof_ms / steps,
                hbm={"algorithmic_GB_per_step": bytes_step / 1e9, "achieved_GBs": bytes_step / 1e9 / (res["ms_per_step"] * 1e-3),
                     "peak_GBs": hbm_peak()[0], "peak_source": hbm_peak()[1],
                     "frac": bytes_step / 1e9 / (res["ms_per_step"] * 1e-3) / hbm_peak()[0]})
-
-    # end to end through mhd_advance_host_dt (the same step S0-S9 as the device-resident line): pinned host buffers, H2D + kernels + D2H inside the timed region
-    pin = lambda a: torch.from_numpy(a).pin_memory()
-    pU, pB = pin(hU), pin(hB)
-    hout = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
-    chunk, nstr = max(1, min(G, 32)), 4          # measured best of chunk x streams on this box: PCIe-bound (69 GB/s H2D+D2H)
-    for _ in range(2):
-        solver.advance_host_dt(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], G, dt0, dh, chunk, nstr, 0.3)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        solver.advance_host_dt(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], G, dt0, dh, chunk, nstr, 0.3)
-    torch.cuda.synchronize()
-    te = time.perf_counter() - t0
-    te = shard.max_over_ranks(te, dist, dev)
-    h2d = (sz["n_U_in"] + sz["n_B_in"]) * esz * G
-    d2h = (sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]) * esz * G
-    res["e2e"] = {"value": cells / te, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                  "api": "mhd_advance_host_dt(chunk_groups=%d, nstreams=%d): S0-S9 through pinned host memory" % (chunk, nstr),
-                  "h2d_plus_d2h_GBs": (h2d + d2h) * world / 1e9 / (te / args.steps)}
+    if e2e and not args.no_e2e:
+        # end to end through mhd_advance_host_dt (the same step S0-S9 as the device-resident line): pinned host buffers, H2D +
+        # kernels + D2H inside the timed region
+        pin = lambda a: torch.from_numpy(a).pin_memory()
+        pU, pB = pin(hU), pin(hB)
+        hout = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
+        chunk, nstr = max(1, min(G, E2E_CHUNK)), E2E_STREAMS
+        ksteps = max(3, steps // 4)
+        for _ in range(2):
+            solver.advance_host_dt(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], G, dt0, dh, chunk, nstr, 0.3)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ksteps):
+            solver.advance_host_dt(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], G, dt0, dh, chunk, nstr, 0.3)
+        torch.cuda.synchronize()
+        te = time.perf_counter() - t0
+        te = shard.max_over_ranks(te, dist, dev)
+        h2d = (sz["n_U_in"] + sz["n_B_in"]) * esz * G
+        d2h = (sz["n_U_out"] + sz["n_B_out"] + sz["n_flux"] + sz["n_emf"]) * esz * G
+        gbs = (h2d + d2h) / 1e9 / (te / ksteps)
+        res["e2e"] = {"value": G * N_PS2 ** 3 * ksteps * world / te, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                      "steps": ksteps, "api": "mhd_advance_host_dt(chunk_groups=%d, nstreams=%d): S0-S9 through pinned host memory" % (chunk, nstr),
+                      "h2d_plus_d2h_GBs": gbs}
+        if pcie:
+            # the copies of a step at the measured one-direction rates, overlapped perfectly: the PCIe-bound time of the step
+            t_pcie = max(h2d / pcie["h2d_GBs"], d2h / pcie["d2h_GBs"], (h2d + d2h) / pcie["bidirectional_GBs"]) / 1e9
+            res["e2e"].update(pcie_peak_GBs=pcie, pcie_bound_value=G * N_PS2 ** 3 / t_pcie, frac=(te / ksteps and t_pcie / (te / ksteps)))
     res["stats"] = solver.get_stats()
     solver.destroy()
     return res
 
 
-def measure_config5(args, scheme_name):
+def measure_config5(args, scheme_name, pool=None):
     """BASELINE config 5: 1024^3 cells = 262144 patch groups of the ABC state (config 3), FP32, one step, streamed as
     16^3 patch-group batches from a pinned host pool (the full set would be 91-118 GB in / 52 GB out):
-    the pool = the patch groups of a 256^3 ABC grid, cycled.  With transfers: mhd_advance_host (H2D, kernels and D2H of
+    the pool = the first POOL patch groups of the 1024^3 grid itself (inputs.abc_groups, dh = 1/1024), cycled.  With transfers: mhd_advance_host (H2D, kernels and D2H of
     successive chunks overlapped on CUDA streams), host wall clock.  Without: the same pool resident on
     the device, mhd_advance per 512-group batch, CUDA events."""
     import numpy as np
     import torch
     from paper_1804_03479_b200 import inputs, mhd
-    P, total, batch = args.config5, (1024 // N_PS2) ** 3, 512
+    P, total, batch = pool or args.config5, (1024 // N_PS2) ** 3, 512
     a2 = argparse.Namespace(**{**vars(args), "scheme": scheme_name})
     sp = scheme_params(a2)
     g = sp["g"]
     riem = {"hlle": mhd.HLLE, "hlld": mhd.HLLD, "roe": mhd.ROE}[args.riemann]
     solver = mhd.Solver(mhd.make_config(N=N_PS2, g=g, scheme=sp["scheme"], recon=sp["recon"], riemann=riem, prec=mhd.FP32, max_groups=P))
-    U, bx, by, bz, dh = inputs.abc_grid(256, seed=1805, p0=0.15, vamp=1e-2)
-    hU, hB = inputs.pack_groups(U, bx, by, bz, N_PS2, g, np.float32)
-    reps = (P + hU.shape[0] - 1) // hU.shape[0]
-    hU, hB = np.tile(hU, (reps, 1))[:P].copy(), np.tile(hB, (reps, 1))[:P].copy()
+    # the first P patch groups of the 1024^3 grid (dh = 1/1024), generated group by group
+    hU, hB, dh = inputs.abc_groups(1024, 0, P, N_PS2, g, dtype=np.float32)
     dt0 = 0.3 * dh / 6.0                                         # well below the CFL limit of the state (max speed ~ 2.5)
     pin = lambda a: torch.from_numpy(a).pin_memory()
     pU, pB = pin(hU), pin(hB)
     out = solver.alloc_outputs(P, planes=True)
     hout = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
     passes = total // P
-    chunk, nstr = 32, 4
+    chunk, nstr = E2E_CHUNK, E2E_STREAMS
     solver.advance_host(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], P, dt0, dh, chunk, nstr)
     sampler = ClockSampler(torch.cuda.current_device())
     torch.cuda.synchronize()
@@ -417,9 +496,20 @@ def measure_grid(args, prec_name):
     return res
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
 def cpu_baseline(args, groups, reps=None, target_seconds=12.0):
     """The oracle, as it stands, on the host cores: `reps` passes (default: as many as fill ~target_seconds of CPU
-    work) over `groups` groups of the workload, one pass = advance + dt; value from the mean pass time."""
+    work) over `groups` groups of the workload, one pass = advance + dt; value from the mean pass time.  Beside it the
+    same on ONE thread (a bounded sample of 8 groups, best of 3), SURVEY 8(d)."""
     import numpy as np
     from oracle import mhdref
     mhdref.build()
@@ -429,9 +519,9 @@ def cpu_baseline(args, groups, reps=None, target_seconds=12.0):
     cfg = mhdref.make_config(N=N_PS2, g=sp["g"], scheme=sp["scheme"], recon=sp["recon"], riemann=riem)
     dt, _ = mhdref.dt_reduce(cfg, U, B, sp["g"], dh, 0.3)
 
-    def one_pass():
+    def one_pass(Ux=U, Bx=B):
         t0 = time.perf_counter()
-        o = mhdref.advance(cfg, U, B, dt, dh)
+        o = mhdref.advance(cfg, Ux, Bx, dt, dh)
         mhdref.dt_reduce(cfg, o["U"], o["B"], 0, dh, 0.3)
         return time.perf_counter() - t0
 
@@ -440,10 +530,14 @@ def cpu_baseline(args, groups, reps=None, target_seconds=12.0):
         reps = max(1, min(200, int(round(target_seconds / max(first, 1e-3)))))
     times = [one_pass() for _ in range(reps)]
     mean = sum(times) / len(times)
+    # one thread: the OpenMP loop over groups with a single group per call has nothing to share out
+    n1 = min(groups, 8)
+    t1 = min(sum(one_pass(U[q:q + 1], B[q:q + 1]) for q in range(n1)) for _ in range(3))
     return {"value": groups * N_PS2 ** 3 / mean, "unit": "cell-updates/s", "cores": os.cpu_count(), "kind": "oracle",
             "sample": "%d of the workload's patch groups x %d passes (advance + dt each), mean pass time, FP64, OpenMP "
                       "over groups" % (groups, reps), "seconds": sum(times), "best_pass_value": groups * N_PS2 ** 3 / min(times),
-            "_one_pass": one_pass}
+            "one_thread": {"value": n1 * N_PS2 ** 3 / t1, "unit": "cell-updates/s", "sample": "%d groups, one group per call (one thread), best of 3" % n1},
+            "cpu_model": cpu_model(), "_one_pass": one_pass}
 
 
 def main():
@@ -453,8 +547,8 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     sp_name = "VL+PLM" if args.scheme == "vl" else "CTU+PPM"
     g = 3 if args.scheme == "vl" else 4
-    config = {"workload": "BASELINE.json configs[1]: batch of %d patch groups of 16^3 cells + %d ghost cells, %s+%s+CT, "
-                          "flux_out and emf_out requested; per rank" % (args.groups, g, sp_name, args.riemann.upper()),
+    config = {"workload": "BASELINE.json configs[1]: batch of %d DISTINCT seeded patch groups (seed 3479 + group id) of 16^3 cells + %d ghost "
+                          "cells, %s+%s+CT, flux_out and emf_out requested; per rank" % (args.groups, g, sp_name, args.riemann.upper()),
               "groups_per_rank": args.groups, "ps2": N_PS2, "nghost": g, "scheme": sp_name, "riemann": args.riemann,
               "step": "mhd_advance_dt: S0-S8 with the CFL reduction S9 fused into the final update", "l2": "inputs larger than L2 (no flush needed)",
               "parallelism": "independent batches per GPU (no collective)" if world > 1 else "single GPU"}
@@ -497,7 +591,7 @@ def main():
     if args.config5:
         r = [measure_config5(args, "vl"), measure_config5(args, "ctu")]
         config.update(workload="BASELINE.json configs[4]: 1024^3 cells = 262144 patch groups of 16^3 of the config-3 ABC state, FP32, one step, "
-                               "streamed from a pinned pool of %d groups (the patch groups of a 256^3 ABC grid, cycled)" % args.config5,
+                               "streamed from a pinned pool of %d groups (the first groups of the 1024^3 grid, dh = 1/1024, cycled)" % args.config5,
                       step="mhd_advance_host over the whole stream (with transfers) / mhd_advance per 512-group batch (without)",
                       groups_per_rank=262144, scheme="VL+PLM and CTU+PPM")
         print(json.dumps({"metric": "cell-updates/sec", "value": r[0]["without_transfers"]["value"], "unit": "cell-updates/s", "n_gpus": 1,
@@ -536,8 +630,21 @@ def main():
         return 0
     main_prec = args.prec
     other = "f64" if main_prec == "f32" else "f32"
-    r_main = measure(args, main_prec, rank, world, dist)
-    r_other = measure(args, other, rank, world, dist)
+    pcie = pcie_peaks(torch.device("cuda", local))
+    r_main = measure(args, main_prec, rank, world, dist, pcie=pcie)
+    r_other = measure(args, other, rank, world, dist, pcie=pcie)
+    extra = {}
+    if not args.main_only and world == 1:
+        # the other variants the paper names, in the driver's line (fewer steps each: they are sub-records, not the headline)
+        k2 = max(10, args.steps // 4)
+        if (args.scheme, args.riemann) != ("ctu", "hlld"):      # CTU+PPM+HLLD: BASELINE configs 3-5
+            extra["ctu_ppm_hlld"] = {pr: measure(args, pr, rank, world, dist, scheme="ctu", riemann="hlld", steps=k2, e2e=(pr == "f32"), pcie=pcie) for pr in ("f32", "f64")}
+        if (args.scheme, args.riemann) != ("vl", "roe"):        # VL+PLM+Roe: the combination of the paper's Fig. 18
+            extra["vl_plm_roe"] = {pr: measure(args, pr, rank, world, dist, scheme="vl", riemann="roe", steps=k2, e2e=False) for pr in ("f32", "f64")}
+        # BASELINE configs[4]: 1024^3 cells streamed as 16^3 patch-group batches, with and without transfers
+        extra["config5"] = {"workload": "BASELINE.json configs[4]: 262144 group-updates (= 1024^3 cells) of the 1024^3 ABC state, FP32, streamed from a "
+                                        "pinned pool of 1024 groups (the first groups of that grid, dh = 1/1024), HLLD",
+                            "vl_plm": measure_config5(args, "vl", pool=1024), "ctu_ppm": measure_config5(args, "ctu", pool=1024)}
     if rank == 0:
         cb = None
         if not args.no_cpu_baseline and world == 1:
@@ -545,20 +652,26 @@ def main():
             cb.pop("_one_pass")
 
         def sub(r, prec):
-            return {"value": r["value"], "unit": "cell-updates/s", "ms_per_step": r["ms_per_step"], "dtype": prec,
-                    "roofline": r["roofline"], "hbm": r["hbm"], "stages_ms_per_step": {k: round(v["ms_per_step"], 4) for k, v in r["stages"].items()},
-                    "profiled_ms_per_step": r["profiled_ms_per_step"], "e2e": r["e2e"], "clocks": r["clocks"],
-                    "stats": r["stats"], "paper_p100_context": PAPER_P100[prec]}
+            d = {"variant": r["variant"], "value": r["value"], "unit": "cell-updates/s", "ms_per_step": r["ms_per_step"], "steps": r["steps"], "dtype": prec,
+                 "roofline": r["roofline"], "alu_whole_step": r.get("alu_whole_step"), "dram_traffic": r.get("dram_traffic"), "hbm": r["hbm"],
+                 "stages_ms_per_step": {k: round(v["ms_per_step"], 4) for k, v in r["stages"].items()},
+                 "profiled_ms_per_step": r["profiled_ms_per_step"], "gpu_launches": r["launches"], "clocks": r["clocks"],
+                 "stats": r["stats"], "paper_p100_context": PAPER_P100[prec]}
+            if "e2e" in r:
+                d["e2e"] = r["e2e"]
+            return d
 
         line = {"metric": "cell-updates/sec", "value": r_main["value"], "unit": "cell-updates/s", "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": r_main["ms_per_step"], "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": main_prec, "data": "synthetic", "config": config,
-                "clocks": r_main["clocks"], "e2e": r_main["e2e"], "gpu_launches": r_main["launches"],
+                "clocks": r_main["clocks"], "e2e": r_main.get("e2e"), "gpu_launches": r_main["launches"],
                 "roofline": r_main["roofline"], "cpu_baseline": cb, "dram_traffic": r_main.get("dram_traffic"), "alu_whole_step": r_main.get("alu_whole_step"),
                 "hbm": r_main["hbm"], "stages_ms_per_step": {k: round(v["ms_per_step"], 4) for k, v in r_main["stages"].items()},
                 "profiled_ms_per_step": r_main["profiled_ms_per_step"],
                 "paper_p100_context": {"value": PAPER_P100[main_prec], "note": "Tesla P100, VL+PLM+Roe, PAPER.md:12,:465 -- context, not a target"},
                 {"f32": "fp32", "f64": "fp64"}[other]: sub(r_other, other)}
+        for name, recs in extra.items():
+            line[name] = recs if name == "config5" else {pr: sub(r, pr) for pr, r in recs.items()}
         print(json.dumps(line))
     if dist is not None:
         dist.barrier()

@@ -70,16 +70,22 @@ int main() {
     char buf[64]; std::snprintf(buf, sizeof buf, "per Riemann solve, %s", names[sol]);
     show(buf, diff(g_t, t0), 1.0);
   }
-  // whole patch group, smooth seeded state (no floors), per interior cell-update
+  // whole patch group, smooth seeded state (no floors), per interior cell-update; on the oracle's maximal index ranges and on the
+  // minimal ones (every stage only where the final update needs it: the work the method itself requires, mhdref_config.minimal_ranges),
+  // with the flops of each step (hook after every step of the group's update)
   struct V { const char* name; int scheme, recon, riemann, limvar, g; } vars[] = {
-    { "VL+PLM+HLLD (g=3), per cell-update", 0, 0, 1, 0, 3 }, { "VL+PLM+Roe (g=3), per cell-update", 0, 0, 2, 0, 3 },
-    { "CTU+PLM+HLLD char (g=3), per cell-update", 1, 0, 1, 1, 3 }, { "CTU+PPM+HLLD char (g=4), per cell-update", 1, 1, 1, 1, 4 },
-    { "CTU+PPM+Roe char (g=4), per cell-update", 1, 1, 2, 1, 4 } };
+    { "VL+PLM+HLLD (g=3)", 0, 0, 1, 0, 3 }, { "VL+PLM+Roe (g=3)", 0, 0, 2, 0, 3 },
+    { "CTU+PLM+HLLD char (g=3)", 1, 0, 1, 1, 3 }, { "CTU+PPM+HLLD char (g=4)", 1, 1, 1, 1, 4 },
+    { "CTU+PPM+Roe char (g=4)", 1, 1, 2, 1, 4 } };
   const int N = 16;
-  for (const V& v : vars) {
+  static Tally marks[8];
+  mhdref_stage_hook = [](int n) { if (n >= 0 && n < 8) marks[n] = g_t; };
+  const char* steps[8] = { "", "con->prim", "pass-1 fluxes (+ CTU reconstruction)", "EMF-1", "half step", "pass-2 states + fluxes", "EMF-2", "full update" };
+  for (const V& v : vars) for (int mn = 0; mn < 2; ++mn) {
     const int T = N + 2 * v.g;
     mhdref_config cfg; cfg.ps2 = N; cfg.nghost = v.g; cfg.gamma = Counted(gam); cfg.scheme = v.scheme; cfg.recon = v.recon;
     cfg.riemann = v.riemann; cfg.limvar = v.limvar; cfg.min_dens = Counted(1e-10); cfg.min_pres = Counted(1e-10); cfg.emf_tie = Counted(1e-12); cfg.limiter = 0;
+    cfg.minimal_ranges = mn;
     std::vector<Counted> U(5 * T * T * T), B(3 * T * T * (T + 1)), Uo(5 * N * N * N), Bo(3 * N * N * (N + 1)), fo(9 * 5 * N * N), eo(9 * 2 * (N + 1) * N);
     const real_t k = 2.0 * 3.14159265358979323846 / N;
     for (int kk = 0; kk < T; ++kk) for (int j = 0; j < T; ++j) for (int i = 0; i < T; ++i) {
@@ -93,7 +99,12 @@ int main() {
     unsigned long long st[3] = { 0, 0, 0 };
     Tally t0 = g_t;
     mhdref_advance(&cfg, U.data(), B.data(), Uo.data(), Bo.data(), fo.data(), eo.data(), 1, Counted(0.01), Counted(1.0 / N), st, 0);
-    show(v.name, diff(g_t, t0), (double)N * N * N);
+    char buf[96]; std::snprintf(buf, sizeof buf, "%s, %s ranges, per cell-update", v.name, mn ? "minimal" : "maximal");
+    show(buf, diff(g_t, t0), (double)N * N * N);
+    for (int n = 1; n < 8; ++n) {
+      const Tally d = diff(marks[n], marks[n - 1]);
+      std::printf("    step %d %-40s flops per group %12llu\n", n, steps[n], d.add + d.mul + d.div + d.sqrt);
+    }
   }
   return 0;
 }

@@ -41,7 +41,12 @@ typedef struct {
   double min_dens, min_pres;
   double emf_tie;  // reading R10a: width of the linear blend of the CT upwind switch, in units of (mean cell density) * dh/dt
   int limiter;     // NEXT-4 variants: 0 MC (reading R5, the default), 1 minmod, 2 van Leer
+  int minimal_ranges;  // 0: every stage on the maximal index range on which its inputs exist (the default); 1: every stage only
+                       // where the final update of the N^3 interior cells needs it.  Same arithmetic per
+                       // cell / face / edge; the outputs are bitwise the same (pinned), only the operation count differs
 } mhdref_config;
+// measurement hook (oracle/count_ops.cpp): called with the number of the step that just finished inside one group's update
+void (*mhdref_stage_hook)(int) = nullptr;
 }
 
 namespace {
@@ -405,6 +410,7 @@ struct Group {
     if (cfg.scheme == 1) { for (auto& wd : Wlo) for (auto& a : wd) mk(a); for (auto& wd : Wup) for (auto& a : wd) mk(a); }
   }
   inline int off(int d) const { return d == 0 ? 1 : (d == 1 ? t.S : t.S * t.S); }
+  static inline void stage(int n) { if (mhdref_stage_hook) mhdref_stage_hook(n); }
 
   void load(const double* Uin, const double* Bin) {
     int T = t.T;
@@ -560,7 +566,10 @@ struct Group {
   // ------------------------------------------------------------------------------
   void advance_vl() {
     int T = t.T;
+    const bool mn = c.minimal_ranges != 0;
+    const int g = t.g, N = t.N;
     con2prim(U, b, W, 0, T);                                           // time-n primitives
+    stage(1);
     // step 1: first-order fluxes, longitudinal B = face value
     for (int d = 0; d < 3; ++d) {
       int lo[3] = { 0, 0, 0 }; lo[d] = 1;
@@ -571,19 +580,24 @@ struct Group {
         solve_face(d, q, wl, wr, b[d][q]);
       }
     }
-    edge_emf(W, 1, T - 1, 0, T);                                       // step 2
+    stage(2);
+    edge_emf(W, 1, T - 1, mn ? 1 : 0, mn ? T - 1 : T);                 // step 2 (the half step reads edges along c only for c in [1, T-1))
+    stage(3);
     fv_update(Uh, 0.5 * dt, 1, T - 1);                                 // step 3 (dt/2)
     ct_update(b, bh, 0.5 * dt, 1, T - 1);
     con2prim(Uh, bh, Wh, 1, T - 1);
+    stage(4);
     for (auto& fd : F) for (auto& a : fd) a.assign(t.n3, NaN);           // pass-1 fluxes are dead from here on
     // step 4+5: PLM (or, NEXT-4 variant, the PPM parabola of C4) in primitive/characteristic variables at the half step,
     // no tracing (the half step supplies the time centring); Bn = bh(face).  Faces whose stencil lies inside the cells
     // that carry a half-step state: PLM cells i-2..i+1 -> faces 3..T-3; PPM cells i-3..i+2 -> faces 4..T-4
     const int r = c.recon == 0 ? 3 : 4;
+    // minimal: the faces of the interior cells and of their transverse neighbours (the edge EMFs of the interior faces need those)
+    const int tlo = mn ? g - 1 : 1, thi = mn ? g + N + 1 : T - 1, nlo = mn ? g : r, nhi = mn ? g + N : T - r;
     for (int d = 0; d < 3; ++d) {
       int t1, t2; cyc(d, t1, t2);
       int idx[3];
-      for (idx[t2] = 1; idx[t2] < T - 1; ++idx[t2]) for (idx[t1] = 1; idx[t1] < T - 1; ++idx[t1]) for (idx[d] = r; idx[d] <= T - r; ++idx[d]) {
+      for (idx[t2] = tlo; idx[t2] < thi; ++idx[t2]) for (idx[t1] = tlo; idx[t1] < thi; ++idx[t1]) for (idx[d] = nlo; idx[d] <= nhi; ++idx[d]) {
         size_t q = t.id(idx[0], idx[1], idx[2]), ql = q - off(d);
         double wl[7], wr[7];
         if (c.recon == 0) {
@@ -600,7 +614,9 @@ struct Group {
         solve_face(d, q, wl, wr, bh[d][q]);
       }
     }
-    edge_emf(Wh, r, T - r, 1, T - 1);                                  // step 6
+    stage(5);
+    if (mn) edge_emf(Wh, g, g + N, g, g + N); else edge_emf(Wh, r, T - r, 1, T - 1);   // step 6
+    stage(6);
   }
 
   // ------------------------------------------------------------------------------
@@ -610,11 +626,16 @@ struct Group {
     int T = t.T;
     int r = c.recon == 0 ? 1 : 2;
     double sig = dt / dh, hdt = 0.5 * dt;
+    const bool mn = c.minimal_ranges != 0;
+    // minimal: everything is derived from the cells whose half-step state the second pass needs, [lo, hi)^3 = interior + 1
+    const int lo_ = t.g - 1, hi_ = t.g + t.N + 1;
     con2prim(U, b, W, 0, T);
+    stage(1);
     // step 1: reconstruction + half-step tracing (matrix form, all waves) + primitive MHD source terms
     for (int d = 0; d < 3; ++d) {
       int t1, t2; cyc(d, t1, t2);
       int lo[3] = { 0, 0, 0 }, hi[3] = { T, T, T }; lo[d] = r; hi[d] = T - r;
+      if (mn) for (int a = 0; a < 3; ++a) { lo[a] = lo_ - 1; hi[a] = hi_ + 1; }        // face states one cell beyond [lo, hi)^3
       for (int k = lo[2]; k < hi[2]; ++k) for (int j = lo[1]; j < hi[1]; ++j) for (int i = lo[0]; i < hi[0]; ++i) {
         size_t q = t.id(i, j, k);
         int od = off(d);
@@ -648,6 +669,7 @@ struct Group {
     // step 2: F1 = Riemann(Wup(i-1), Wlo(i), b_n(face) at t^n)
     for (int d = 0; d < 3; ++d) {
       int lo[3] = { 0, 0, 0 }, hi[3] = { T, T, T }; lo[d] = r + 1; hi[d] = T - r;
+      if (mn) { for (int a = 0; a < 3; ++a) { lo[a] = lo_ - 1; hi[a] = hi_ + 1; } lo[d] = lo_; }   // faces n in [lo, hi], t in [lo-1, hi]
       for (int k = lo[2]; k < hi[2]; ++k) for (int j = lo[1]; j < hi[1]; ++j) for (int i = lo[0]; i < hi[0]; ++i) {
         size_t q = t.id(i, j, k), ql = q - off(d);
         double wl[7], wr[7];
@@ -655,10 +677,13 @@ struct Group {
         solve_face(d, q, wl, wr, b[d][q]);
       }
     }
-    edge_emf(W, r + 1, T - 1 - r, 0, T);                               // step 3
+    stage(2);
+    if (mn) edge_emf(W, lo_, hi_, lo_, hi_); else edge_emf(W, r + 1, T - 1 - r, 0, T);   // step 3
+    stage(3);
     fv_update(Uh, hdt, r + 1, T - 1 - r);                              // step 4
     ct_update(b, bh, hdt, r + 1, T - 1 - r);
     con2prim(Uh, bh, Wh, r + 1, T - 1 - r);
+    stage(4);
     // step 5: transverse flux-gradient correction + conservative MHD source terms (C3 step 5)
     double qh = hdt / dh;
     for (int d = 0; d < 3; ++d) {
@@ -666,6 +691,7 @@ struct Group {
       int od = off(d), o1 = off(t1), o2 = off(t2);
       int lo[3], hi[3];
       lo[t1] = lo[t2] = r + 1; hi[t1] = hi[t2] = T - 1 - r; lo[d] = r; hi[d] = T - r;
+      if (mn) { lo[d] = lo_; hi[d] = hi_; }                            // the two cells of every pass-2 face
       for (int k = lo[2]; k < hi[2]; ++k) for (int j = lo[1]; j < hi[1]; ++j) for (int i = lo[0]; i < hi[0]; ++i) {
         size_t q = t.id(i, j, k);
         int cn = (d == 0 ? i : (d == 1 ? j : k));
@@ -689,6 +715,7 @@ struct Group {
         for (int side = 0; side < 2; ++side) {     // 0: Wlo (lower face cn), 1: Wup (upper face cn+1)
           int face = cn + side;
           if (face < r + 1 || face > T - 1 - r) continue;              // bh exists only there
+          if (mn && (face < t.g || face > t.g + t.N)) continue;        // minimal: only the states of the interior faces
           size_t qf = q + (side ? od : 0);
           double w[7], u[7];
           for (int v = 0; v < 7; ++v) w[v] = side ? Wup[d][v][q] : Wlo[d][v][q];
@@ -717,6 +744,7 @@ struct Group {
         int t1, t2; cyc(d, t1, t2);
         int lo[3], hi[3];
         lo[t1] = lo[t2] = r + 1; hi[t1] = hi[t2] = T - 1 - r; lo[d] = r + 1; hi[d] = T - r;
+        if (mn) { lo[d] = t.g; hi[d] = t.g + t.N + 1; }
         for (int k = lo[2]; k < hi[2]; ++k) for (int j = lo[1]; j < hi[1]; ++j) for (int i = lo[0]; i < hi[0]; ++i) {
           size_t q = t.id(i, j, k), ql = q - off(d);
           double wl[7], wr[7], f[7];
@@ -728,11 +756,14 @@ struct Group {
       }
       for (int d = 0; d < 3; ++d) for (int v = 0; v < 7; ++v) F[d][v].swap(F2[d][v]);
     }
-    edge_emf(Wh, r + 2, T - 2 - r, r + 1, T - 1 - r);                  // step 7
+    stage(5);
+    if (mn) edge_emf(Wh, t.g, t.g + t.N, t.g, t.g + t.N); else edge_emf(Wh, r + 2, T - 2 - r, r + 1, T - 1 - r);   // step 7
+    stage(6);
   }
 
   void run(const double* Uin, const double* Bin, double* Uout, double* Bout, double* fout, double* eout) {
     load(Uin, Bin);
+    stage(0);
     if (c.scheme == 0) advance_vl(); else advance_ctu();
     // step 7 (VL) / 8 (CTU): full update with F2 and the second edge EMFs; outputs
     int N = t.N, g = t.g;
@@ -741,6 +772,7 @@ struct Group {
     for (auto& a : bn) a.assign(t.n3, NaN);
     fv_update(Un, dt, g, g + N);
     ct_update(b, bn, dt, g, g + N);
+    stage(7);
     for (int v = 0; v < 5; ++v) for (int k = 0; k < N; ++k) for (int j = 0; j < N; ++j) for (int i = 0; i < N; ++i)
       Uout[(((size_t)v * N + k) * N + j) * N + i] = Un[v][t.id(i + g, j + g, k + g)];
     double* ox = Bout; double* oy = ox + (size_t)N * N * (N + 1); double* oz = oy + (size_t)N * N * (N + 1);

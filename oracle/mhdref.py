@@ -28,7 +28,8 @@ MC, MINMOD, VANLEER = 0, 1, 2
 class Config(C.Structure):
     _fields_ = [("ps2", C.c_int), ("nghost", C.c_int), ("gamma", C.c_double), ("scheme", C.c_int),
                 ("recon", C.c_int), ("riemann", C.c_int), ("limvar", C.c_int),
-                ("min_dens", C.c_double), ("min_pres", C.c_double), ("emf_tie", C.c_double), ("limiter", C.c_int)]
+                ("min_dens", C.c_double), ("min_pres", C.c_double), ("emf_tie", C.c_double), ("limiter", C.c_int),
+                ("minimal_ranges", C.c_int)]
 
 
 def build(force: bool = False) -> str:
@@ -100,11 +101,11 @@ def _c(a):
 
 
 def make_config(N=16, g=3, gamma=5.0 / 3.0, scheme=VL, recon=PLM, riemann=HLLD, limvar=None,
-                min_dens=1e-10, min_pres=1e-10, emf_tie=1e-12, limiter=MC) -> Config:
+                min_dens=1e-10, min_pres=1e-10, emf_tie=1e-12, limiter=MC, minimal_ranges=0) -> Config:
     """emf_tie: reading R10a; 1e-12 is the FP64 value, the FP32 path is checked against the oracle run with 1e-5."""
     if limvar is None:
         limvar = LIM_PRIM if scheme == VL else LIM_CHAR
-    return Config(N, g, gamma, scheme, recon, riemann, limvar, min_dens, min_pres, emf_tie, limiter)
+    return Config(N, g, gamma, scheme, recon, riemann, limvar, min_dens, min_pres, emf_tie, limiter, minimal_ranges)
 
 
 def advance(cfg: Config, U_in, B_in, dt, dh, want_planes=True, force_ghost_ok=False):

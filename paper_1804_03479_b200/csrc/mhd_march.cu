@@ -13,14 +13,9 @@ template <class K> cudaError_t big_smem(K kernel, size_t bytes) {
 
 template <class R, int SOLVER, int LIM>
 cudaError_t launch2(const KParamsSC<R, 23>& p, int ng, cudaStream_t st) {
-  cudaError_t e;
-  if (p.red) {
-    if ((e = big_smem(k_vl_march2<R, SOLVER, LIM, true>, march2_smem<R>())) != cudaSuccess) return e;
-    k_vl_march2<R, SOLVER, LIM, true><<<ng, kM2P, march2_smem<R>(), st>>>(p);
-  } else {
-    if ((e = big_smem(k_vl_march2<R, SOLVER, LIM, false>, march2_smem<R>())) != cudaSuccess) return e;
-    k_vl_march2<R, SOLVER, LIM, false><<<ng, kM2P, march2_smem<R>(), st>>>(p);
-  }
+  cudaError_t e = big_smem(k_vl_march2<R, SOLVER, LIM>, march2_smem<R>());
+  if (e != cudaSuccess) return e;
+  k_vl_march2<R, SOLVER, LIM><<<ng, kM2P, march2_smem<R>(), st>>>(p);
   return cudaGetLastError();
 }
 

@@ -273,7 +273,9 @@ template <class R> constexpr size_t march2_smem() {
 #ifndef MHD_M2_MINB
 #define MHD_M2_MINB 2
 #endif
-template <class R, int SOLVER, int LIM, bool DT>
+// S9 (p.red set: mhd_advance_dt) is a run-time branch, not a template flag: the two instantiations compiled the energy flux of
+// the Riemann solve to different last bits in FP32, and mhd_advance_dt must equal mhd_advance + mhd_dt_reduce bit for bit
+template <class R, int SOLVER, int LIM>
 __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_march2(const KParamsSC<R, 23> p) {
   constexpr int T = kMT, PT = kMT * kMT, T3 = T * T * T, P = kM2P, W = kM2W, N = 16, M = N + 1, g = 3;
   extern __shared__ __align__(16) unsigned char march_smem[];
@@ -310,6 +312,7 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
   R Cx = R(0), Cy = R(0), bzlo = R(0);
   R pFx0 = R(0), pFx6 = R(0), pFy0 = R(0), pFy5 = R(0);
   R smax = R(0);
+  const bool DT = p.red != nullptr;
   // stage the 8 primitives of plane kp into its ring slot
   auto stage = [&](int kp, bool arm) {
     constexpr unsigned PB = PT * sizeof(R);
