@@ -62,7 +62,10 @@ typedef struct {
   int limiter;      /* mhd_limiter (0 = MC) */
 } mhd_config;
 
-enum { MHD_OK = 0, MHD_EINVAL = -1, MHD_ECUDA = -2, MHD_ENOMEM = -3 };
+/* MHD_ESTATE: a call that returns a time step (mhd_dt_reduce, mhd_advance_dt, mhd_advance_host_dt, mhd_grid_dt,
+ * mhd_grid_advance_dt) found no finite positive signal speed -- the state holds NaN or infinite values (a cell with a NaN
+ * input reports an infinite speed, so the maximum cannot drop it).  The arrays have been written; *dt_out is not usable. */
+enum { MHD_OK = 0, MHD_EINVAL = -1, MHD_ECUDA = -2, MHD_ENOMEM = -3, MHD_ESTATE = -4 };
 
 /* Create a solver.  Allocates the device workspace (for min(max_groups, what fits a 6 GB budget) groups: larger
  * batches are processed in equal slices).  Returns MHD_EINVAL for a bad configuration (incl. too small a ghost width), MHD_ECUDA /

@@ -62,7 +62,6 @@ struct mhd_solver {
   cudaEvent_t fork = nullptr;
   unsigned long long* d_stats = nullptr;    // 3 counters
   unsigned long long* d_red = nullptr;      // dt reduction cell
-  unsigned long long* red_now = nullptr;    // set by mhd_advance_dt around its launches: the final update also reduces the CFL speed
   unsigned long long launches = 0;
   HostLane lanes[kMaxStreams];
   int lane_groups = 0, lane_count = 0;
@@ -83,7 +82,7 @@ namespace {
 
 template <class R>
 KParams<R> make_params(const mhd_solver* s, const void* Ui, const void* Bi, void* Uo, void* Bo, void* fo, void* eo,
-                       void* ws, int first, double dt, double dh) {
+                       void* ws, int first, double dt, double dh, unsigned long long* red) {
   KParams<R> p;
   p.Uin = static_cast<const R*>(Ui) + (size_t)first * s->nUi;
   p.Bin = static_cast<const R*>(Bi) + (size_t)first * s->nBi;
@@ -93,7 +92,7 @@ KParams<R> make_params(const mhd_solver* s, const void* Ui, const void* Bi, void
   p.eout = eo ? static_cast<R*>(eo) + (size_t)first * s->nE : nullptr;
   p.ws = static_cast<R*>(ws);
   p.stats = s->d_stats;
-  p.red = s->red_now;
+  p.red = red;                       // non-null: the final update also reduces the CFL speed of the state it writes (S9)
   p.N = s->N; p.g = s->g; p.T = s->T; p.S = s->S; p.S2 = s->S * s->S; p.S3 = (int)s->S3; p.narr = s->narr;
   p.nUi = (long long)s->nUi; p.nBi = (long long)s->nBi; p.nUo = (long long)s->nUo; p.nBo = (long long)s->nBo;
   p.nF = (long long)s->nF; p.nE = (long long)s->nE;
@@ -304,8 +303,8 @@ int run_slice(mhd_solver* s, const KParams<R>& p, int ng, cudaStream_t st) {
 // kernels fill the SMs it leaves idle.  Measured (B200, 512 groups, VL+PLM+HLLD): 0.973 against 1.000 ms per step in
 // FP32, 1.876 against 1.917 ms in FP64; slices are bitwise independent of the cut (tests/test_gpu_api.py).
 constexpr int kMinSliceGroups = 128;
-inline int balanced_slice(const mhd_solver* s, int ngroups) {
-  int nslices = (ngroups + s->slice_groups - 1) / s->slice_groups;
+inline int balanced_slice(const mhd_solver* s, int ngroups, int cap) {
+  int nslices = (ngroups + cap - 1) / cap;
   if (nslices < s->nlanes && ngroups >= kMinSliceGroups * s->nlanes && !s->slice_fixed) nslices = s->nlanes;
   return (ngroups + nslices - 1) / nslices;
 }
@@ -313,11 +312,11 @@ inline int balanced_slice(const mhd_solver* s, int ngroups) {
 // slices of one batch on ONE stream with ONE workspace (host path, profiling)
 template <class R>
 int advance_serial(mhd_solver* s, const void* Ui, const void* Bi, void* Uo, void* Bo, void* fo, void* eo, void* ws,
-                   int ngroups, double dt, double dh, cudaStream_t st) {
-  const int per = balanced_slice(s, ngroups);
+                   int ngroups, double dt, double dh, cudaStream_t st, unsigned long long* red, int slice_cap) {
+  const int per = balanced_slice(s, ngroups, slice_cap);
   for (int first = 0; first < ngroups; first += per) {
     const int ng = std::min(per, ngroups - first);
-    KParams<R> p = make_params<R>(s, Ui, Bi, Uo, Bo, fo, eo, ws, first, dt, dh);
+    KParams<R> p = make_params<R>(s, Ui, Bi, Uo, Bo, fo, eo, ws, first, dt, dh, red);
     int rc = run_slice<R>(s, p, ng, st);
     if (rc != MHD_OK) return rc;
   }
@@ -327,26 +326,51 @@ int advance_serial(mhd_solver* s, const void* Ui, const void* Bi, void* Uo, void
 // slices round-robin over the internal lanes, forked from and joined back into the caller's stream
 template <class R>
 int advance_lanes(mhd_solver* s, const void* Ui, const void* Bi, void* Uo, void* Bo, void* fo, void* eo,
-                  int ngroups, double dt, double dh, cudaStream_t user) {
-  const int per = balanced_slice(s, ngroups);
+                  int ngroups, double dt, double dh, cudaStream_t user, unsigned long long* red) {
+  const int per = balanced_slice(s, ngroups, s->slice_groups);
   const int nslices = (ngroups + per - 1) / per;
   const int nl = std::min(s->nlanes, nslices);
-  if (s->prof_on || nl <= 1) return advance_serial<R>(s, Ui, Bi, Uo, Bo, fo, eo, s->dev[0].ws, ngroups, dt, dh, user);
+  if (s->prof_on || nl <= 1) return advance_serial<R>(s, Ui, Bi, Uo, Bo, fo, eo, s->dev[0].ws, ngroups, dt, dh, user, red, s->slice_groups);
   CU(cudaEventRecord(s->fork, user));
   for (int l = 0; l < nl; ++l) CU(cudaStreamWaitEvent(s->dev[l].stream, s->fork, 0));
-  int i = 0;
-  for (int first = 0; first < ngroups; first += per, ++i) {
+  int i = 0, rc = MHD_OK;
+  for (int first = 0; first < ngroups && rc == MHD_OK; first += per, ++i) {
     const int ng = std::min(per, ngroups - first);
     DevLane& L = s->dev[i % nl];
-    KParams<R> p = make_params<R>(s, Ui, Bi, Uo, Bo, fo, eo, L.ws, first, dt, dh);
-    int rc = run_slice<R>(s, p, ng, L.stream);
-    if (rc != MHD_OK) return rc;
+    KParams<R> p = make_params<R>(s, Ui, Bi, Uo, Bo, fo, eo, L.ws, first, dt, dh, red);
+    rc = run_slice<R>(s, p, ng, L.stream);
   }
+  // also on an error: what the lanes have been given is joined back into the caller's stream
   for (int l = 0; l < nl; ++l) {
-    CU(cudaEventRecord(s->dev[l].done, s->dev[l].stream));
-    CU(cudaStreamWaitEvent(user, s->dev[l].done, 0));
+    cudaError_t e = cudaEventRecord(s->dev[l].done, s->dev[l].stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(user, s->dev[l].done, 0);
+    if (e != cudaSuccess && rc == MHD_OK) rc = cuda_fail(e, "mhd_advance join");
   }
-  return MHD_OK;
+  return rc;
+}
+
+// largest signal speed from the bit pattern the kernels reduced; MHD_ESTATE if it is not finite and positive (a NaN or infinite
+// state: the kernels encode a NaN speed as +inf so that the maximum cannot drop it)
+inline int speed_to_dt(const mhd_solver* s, unsigned long long bits, double cfl, double dh, double* dt_out, double* maxspeed_out) {
+  double smax;
+  if (s->cfg.prec == MHD_FP32) { unsigned int b32 = (unsigned int)(bits & 0xffffffffu); float f; memcpy(&f, &b32, 4); smax = f; }
+  else memcpy(&smax, &bits, 8);
+  if (maxspeed_out) *maxspeed_out = smax;
+  *dt_out = cfl * dh / smax;
+  return (std::isfinite(smax) && smax > 0.0) ? MHD_OK : MHD_ESTATE;
+}
+
+int advance_impl(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out, void* flux_out, void* emf_out,
+                 int ngroups, double dt, double dh, void* cuda_stream, unsigned long long* red) {
+  if (!s || !U_in || !B_in || !U_out || !B_out) return MHD_EINVAL;
+  if (ngroups < 0 || ngroups > s->cfg.max_groups) return MHD_EINVAL;
+  if (!(dt > 0.0) || !(dh > 0.0) || !std::isfinite(dt) || !std::isfinite(dh)) return MHD_EINVAL;
+  if (ngroups == 0) return MHD_OK;
+  CU(cudaSetDevice(s->cfg.device));
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  return s->cfg.prec == MHD_FP32
+             ? advance_lanes<float>(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, st, red)
+             : advance_lanes<double>(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, st, red);
 }
 
 int check_config(const mhd_config* c) {
@@ -462,15 +486,7 @@ int mhd_sizes(const mhd_solver* s, size_t* a, size_t* b, size_t* c, size_t* d, s
 
 int mhd_advance(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out, void* flux_out,
                 void* emf_out, int ngroups, double dt, double dh, void* cuda_stream) {
-  if (!s || !U_in || !B_in || !U_out || !B_out) return MHD_EINVAL;
-  if (ngroups < 0 || ngroups > s->cfg.max_groups) return MHD_EINVAL;
-  if (!(dt > 0.0) || !(dh > 0.0) || !std::isfinite(dt) || !std::isfinite(dh)) return MHD_EINVAL;
-  if (ngroups == 0) return MHD_OK;
-  CU(cudaSetDevice(s->cfg.device));
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  return s->cfg.prec == MHD_FP32
-             ? advance_lanes<float>(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, st)
-             : advance_lanes<double>(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, st);
+  return advance_impl(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, cuda_stream, nullptr);
 }
 
 // mhd_advance with the CFL reduction (S9) of its own output fused into the final update (S8)
@@ -481,19 +497,12 @@ int mhd_advance_dt(mhd_solver* s, const void* U_in, const void* B_in, void* U_ou
   CU(cudaSetDevice(s->cfg.device));
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   CU(cudaMemsetAsync(s->d_red, 0, sizeof(unsigned long long), st));
-  s->red_now = s->d_red;
-  const int rc = mhd_advance(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, cuda_stream);
-  s->red_now = nullptr;
+  const int rc = advance_impl(s, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, cuda_stream, s->d_red);
   if (rc != MHD_OK) return rc;
   unsigned long long bits = 0;
   CU(cudaMemcpyAsync(&bits, s->d_red, sizeof bits, cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));
-  double smax;
-  if (s->cfg.prec == MHD_FP32) { unsigned int b32 = (unsigned int)(bits & 0xffffffffu); float f; memcpy(&f, &b32, 4); smax = f; }
-  else memcpy(&smax, &bits, 8);
-  if (maxspeed_out) *maxspeed_out = smax;
-  *dt_out = cfl * dh / smax;
-  return MHD_OK;
+  return speed_to_dt(s, bits, cfl, dh, dt_out, maxspeed_out);
 }
 
 }  // extern "C"

@@ -88,17 +88,15 @@ static int grid_advance_impl(mhd_solver* s, void* U, void* bx, void* by, void* b
   }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (red) CU(cudaMemsetAsync(red, 0, sizeof(unsigned long long), st));
-  s->red_now = red;
   if (s->cfg.prec == MHD_FP32) {
     rc = grid_pack_t<float>(s, U, bx, by, bz, d, s->g, s->gUi, s->gBi, st);
-    if (rc == MHD_OK) rc = advance_lanes<float>(s, s->gUi, s->gBi, s->gUo, s->gBo, nullptr, nullptr, G, dt, dh, st);
+    if (rc == MHD_OK) rc = advance_lanes<float>(s, s->gUi, s->gBi, s->gUo, s->gBo, nullptr, nullptr, G, dt, dh, st, red);
     if (rc == MHD_OK) rc = grid_unpack_t<float>(s, s->gUo, s->gBo, d, U, bx, by, bz, st);
   } else {
     rc = grid_pack_t<double>(s, U, bx, by, bz, d, s->g, s->gUi, s->gBi, st);
-    if (rc == MHD_OK) rc = advance_lanes<double>(s, s->gUi, s->gBi, s->gUo, s->gBo, nullptr, nullptr, G, dt, dh, st);
+    if (rc == MHD_OK) rc = advance_lanes<double>(s, s->gUi, s->gBi, s->gUo, s->gBo, nullptr, nullptr, G, dt, dh, st, red);
     if (rc == MHD_OK) rc = grid_unpack_t<double>(s, s->gUo, s->gBo, d, U, bx, by, bz, st);
   }
-  s->red_now = nullptr;
   return rc;
 }
 
@@ -118,12 +116,7 @@ int mhd_grid_advance_dt(mhd_solver* s, void* U, void* bx, void* by, void* bz, in
   unsigned long long bits = 0;
   CU(cudaMemcpyAsync(&bits, s->d_red, sizeof bits, cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));
-  double smax;
-  if (s->cfg.prec == MHD_FP32) { unsigned int b32 = (unsigned int)(bits & 0xffffffffu); float f; memcpy(&f, &b32, 4); smax = f; }
-  else memcpy(&smax, &bits, 8);
-  if (maxspeed_out) *maxspeed_out = smax;
-  *dt_out = cfl * dh / smax;
-  return MHD_OK;
+  return speed_to_dt(s, bits, cfl, dh, dt_out, maxspeed_out);
 }
 
 int mhd_grid_dt(mhd_solver* s, const void* U, const void* bx, const void* by, const void* bz, int nx, int ny, int nz, double dh,
@@ -148,12 +141,7 @@ int mhd_grid_dt(mhd_solver* s, const void* U, const void* bx, const void* by, co
   unsigned long long bits = 0;
   CU(cudaMemcpyAsync(&bits, s->d_red, sizeof bits, cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));
-  double smax;
-  if (s->cfg.prec == MHD_FP32) { unsigned int b32 = (unsigned int)(bits & 0xffffffffu); float f; memcpy(&f, &b32, 4); smax = f; }
-  else memcpy(&smax, &bits, 8);
-  if (maxspeed_out) *maxspeed_out = smax;
-  *dt_out = cfl * dh / smax;
-  return MHD_OK;
+  return speed_to_dt(s, bits, cfl, dh, dt_out, maxspeed_out);
 }
 
 }  // extern "C"

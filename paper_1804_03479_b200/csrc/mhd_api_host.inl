@@ -37,35 +37,35 @@ int advance_host_impl(mhd_solver* s, const void* U_in, const void* B_in, void* U
   char* hUo = static_cast<char*>(U_out); char* hBo = static_cast<char*>(B_out);
   char* hf = static_cast<char*>(flux_out); char* he = static_cast<char*>(emf_out);
   // the lane's slice size must not exceed its workspace
-  const int saved_slice = s->slice_groups;
-  s->slice_groups = std::min(saved_slice, chunk_groups);
+  const int slice_cap = std::min(s->slice_groups, chunk_groups);
   if (red) {
     CU(cudaMemsetAsync(red, 0, sizeof(unsigned long long), s->lanes[0].stream));
     CU(cudaEventRecord(s->fork, s->lanes[0].stream));
     for (int l = 1; l < nstreams; ++l) CU(cudaStreamWaitEvent(s->lanes[l].stream, s->fork, 0));
   }
-  s->red_now = red;
   int c = 0;
-  for (int first = 0; first < ngroups; first += chunk_groups, ++c) {
+  for (int first = 0; first < ngroups && rc == MHD_OK; first += chunk_groups, ++c) {
     const size_t ng = (size_t)std::min(chunk_groups, ngroups - first), f = (size_t)first;
     HostLane& L = s->lanes[c % nstreams];
     cudaError_t ce = cudaMemcpyAsync(L.Ui, hUi + f * s->nUi * e, ng * s->nUi * e, cudaMemcpyHostToDevice, L.stream);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(L.Bi, hBi + f * s->nBi * e, ng * s->nBi * e, cudaMemcpyHostToDevice, L.stream);
-    if (ce != cudaSuccess) { s->slice_groups = saved_slice; s->red_now = nullptr; return cuda_fail(ce, "mhd_advance_host H2D"); }
+    if (ce != cudaSuccess) { rc = cuda_fail(ce, "mhd_advance_host H2D"); break; }
     rc = s->cfg.prec == MHD_FP32
-             ? advance_serial<float>(s, L.Ui, L.Bi, L.Uo, L.Bo, hf ? L.fo : nullptr, he ? L.eo : nullptr, L.ws, (int)ng, dt, dh, L.stream)
-             : advance_serial<double>(s, L.Ui, L.Bi, L.Uo, L.Bo, hf ? L.fo : nullptr, he ? L.eo : nullptr, L.ws, (int)ng, dt, dh, L.stream);
-    if (rc != MHD_OK) { s->slice_groups = saved_slice; s->red_now = nullptr; return rc; }
+             ? advance_serial<float>(s, L.Ui, L.Bi, L.Uo, L.Bo, hf ? L.fo : nullptr, he ? L.eo : nullptr, L.ws, (int)ng, dt, dh, L.stream, red, slice_cap)
+             : advance_serial<double>(s, L.Ui, L.Bi, L.Uo, L.Bo, hf ? L.fo : nullptr, he ? L.eo : nullptr, L.ws, (int)ng, dt, dh, L.stream, red, slice_cap);
+    if (rc != MHD_OK) break;
     ce = cudaMemcpyAsync(hUo + f * s->nUo * e, L.Uo, ng * s->nUo * e, cudaMemcpyDeviceToHost, L.stream);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(hBo + f * s->nBo * e, L.Bo, ng * s->nBo * e, cudaMemcpyDeviceToHost, L.stream);
     if (ce == cudaSuccess && hf) ce = cudaMemcpyAsync(hf + f * s->nF * e, L.fo, ng * s->nF * e, cudaMemcpyDeviceToHost, L.stream);
     if (ce == cudaSuccess && he) ce = cudaMemcpyAsync(he + f * s->nE * e, L.eo, ng * s->nE * e, cudaMemcpyDeviceToHost, L.stream);
-    if (ce != cudaSuccess) { s->slice_groups = saved_slice; s->red_now = nullptr; return cuda_fail(ce, "mhd_advance_host D2H"); }
+    if (ce != cudaSuccess) rc = cuda_fail(ce, "mhd_advance_host D2H");
   }
-  s->slice_groups = saved_slice;
-  s->red_now = nullptr;
-  for (int l = 0; l < nstreams; ++l) CU(cudaStreamSynchronize(s->lanes[l].stream));
-  return MHD_OK;
+  // also on an error: no copy into the caller's host buffers is left in flight when this call returns
+  for (int l = 0; l < nstreams; ++l) {
+    const cudaError_t ce = cudaStreamSynchronize(s->lanes[l].stream);
+    if (ce != cudaSuccess && rc == MHD_OK) rc = cuda_fail(ce, "mhd_advance_host synchronize");
+  }
+  return rc;
 }
 
 }  // namespace
@@ -85,12 +85,7 @@ int mhd_advance_host_dt(mhd_solver* s, const void* U_in, const void* B_in, void*
   if (rc != MHD_OK) return rc;
   unsigned long long bits = 0;
   CU(cudaMemcpy(&bits, s->d_red, sizeof bits, cudaMemcpyDeviceToHost));      // every lane is synchronised
-  double smax;
-  if (s->cfg.prec == MHD_FP32) { unsigned int b32 = (unsigned int)(bits & 0xffffffffu); float f; memcpy(&f, &b32, 4); smax = f; }
-  else memcpy(&smax, &bits, 8);
-  if (maxspeed_out) *maxspeed_out = smax;
-  *dt_out = cfl * dh / smax;
-  return MHD_OK;
+  return speed_to_dt(s, bits, cfl, dh, dt_out, maxspeed_out);
 }
 
 int mhd_dt_reduce(mhd_solver* s, const void* U, const void* B, int ngroups, int nghost_of_arrays, double dh, double cfl,
@@ -114,12 +109,7 @@ int mhd_dt_reduce(mhd_solver* s, const void* U, const void* B, int ngroups, int 
   unsigned long long bits = 0;
   CU(cudaMemcpyAsync(&bits, s->d_red, sizeof bits, cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));
-  double smax;
-  if (s->cfg.prec == MHD_FP32) { unsigned int b32 = (unsigned int)(bits & 0xffffffffu); float f; memcpy(&f, &b32, 4); smax = f; }
-  else memcpy(&smax, &bits, 8);
-  if (maxspeed_out) *maxspeed_out = smax;
-  *dt_out = cfl * dh / smax;
-  return MHD_OK;
+  return speed_to_dt(s, bits, cfl, dh, dt_out, maxspeed_out);
 }
 
 int mhd_get_stats(mhd_solver* s, unsigned long long* fd, unsigned long long* fp, unsigned long long* fb) {
@@ -190,6 +180,7 @@ const char* mhd_strerror(int code) {
     case MHD_EINVAL: return "invalid argument or configuration";
     case MHD_ECUDA: return g_cuda_err.c_str();
     case MHD_ENOMEM: return "out of device memory";
+    case MHD_ESTATE: return "the state has no finite positive signal speed (NaN or infinite values): no time step";
     default: return "unknown error code";
   }
 }

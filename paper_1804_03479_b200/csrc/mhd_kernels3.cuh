@@ -49,7 +49,10 @@ __device__ __forceinline__ R cell_signal_speed(const R (&u)[5], const R (&bl)[3]
     const R bn2 = Bc[d] * Bc[d];
     smax = Num<R>::max(smax, Num<R>::abs(v[d]) + fast_speed(rho, P, bn2, b2 - bn2, gam));
   }
-  return smax;
+  // fmax drops a NaN operand, and a NaN density / energy is replaced by the floors above: a cell with any NaN input reports an
+  // infinite speed, which survives every maximum and makes the reducing call fail with MHD_ESTATE instead of returning a finite dt
+  const R chk = ((u[0] + u[1]) + (u[2] + u[3])) + (u[4] + b2);
+  return (chk == chk && smax == smax) ? smax : R(INFINITY);
 }
 // speeds are >= 0, so their IEEE bit patterns order like unsigned integers: one atomicMax per block
 template <class R> struct Bits;

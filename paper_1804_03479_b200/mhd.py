@@ -19,7 +19,7 @@ PLM, PPM = 0, 1
 HLLE, HLLD, ROE = 0, 1, 2
 LIM_PRIM, LIM_CHAR = 0, 1
 MC, MINMOD, VANLEER = 0, 1, 2
-OK, EINVAL, ECUDA, ENOMEM = 0, -1, -2, -3
+OK, EINVAL, ECUDA, ENOMEM, ESTATE = 0, -1, -2, -3, -4
 
 EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance_host", "mhd_advance_host_dt", "mhd_dt_reduce", "mhd_advance_dt",
            "mhd_get_stats", "mhd_launch_count", "mhd_grid_pack", "mhd_grid_unpack", "mhd_grid_advance", "mhd_grid_advance_dt", "mhd_grid_dt", "mhd_amr_restrict", "mhd_amr_fixup", "mhd_amr_prolong", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
@@ -108,6 +108,35 @@ def _ptr(t):
     return C.c_void_p(t.ctypes.data)
 
 
+def _np_name(prec):
+    return "float32" if prec == FP32 else "float64"
+
+
+def _checked(t, prec, numel, what, device=None):
+    """_ptr with the checks a raw pointer cannot carry: element type of the solver's precision, at least `numel` elements,
+    and (device calls) a CUDA tensor on the solver's device.  None passes (nullable arguments)."""
+    if t is None:
+        return None
+    want = _np_name(prec)
+    if hasattr(t, "data_ptr"):
+        if str(t.dtype).split(".")[-1] != want:
+            raise TypeError(f"{what}: dtype {t.dtype}, the solver computes in {want}")
+        n = t.numel()
+        if device is not None and not (t.is_cuda and t.device.index == device):
+            raise ValueError(f"{what}: expected a CUDA tensor on device {device}, got {t.device}")
+        if device is None and t.is_cuda:
+            raise ValueError(f"{what}: expected a host tensor, got {t.device}")
+    else:
+        if device is not None:
+            raise ValueError(f"{what}: expected a CUDA tensor, got a host array")
+        if str(t.dtype) != want:
+            raise TypeError(f"{what}: dtype {t.dtype}, the solver computes in {want}")
+        n = t.size
+    if n < numel:
+        raise ValueError(f"{what}: {n} elements, the call needs {numel}")
+    return _ptr(t)
+
+
 def _stream_ptr(stream):
     if stream is None:
         import torch
@@ -163,33 +192,45 @@ class Solver:
         out["emf"] = torch.empty((G, self.n_emf), dtype=dt, device=dev) if planes else None
         return out
 
+    def _args(self, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, device):
+        G, pr = max(int(ngroups), 0), self.cfg.prec
+        if G > self.cfg.max_groups:
+            G = 0                      # the library rejects the call (MHD_EINVAL); no size to check against
+        return (_checked(U_in, pr, G * self.n_U_in, "U_in", device), _checked(B_in, pr, G * self.n_B_in, "B_in", device),
+                _checked(U_out, pr, G * self.n_U_out, "U_out", device), _checked(B_out, pr, G * self.n_B_out, "B_out", device),
+                _checked(flux_out, pr, G * self.n_flux, "flux_out", device), _checked(emf_out, pr, G * self.n_emf, "emf_out", device))
+
     def advance(self, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, stream=None):
         """mhd_advance: DEVICE tensors, asynchronous on `stream` (default: torch's current stream)."""
-        _check(lib().mhd_advance(self._h, _ptr(U_in), _ptr(B_in), _ptr(U_out), _ptr(B_out), _ptr(flux_out),
-                                 _ptr(emf_out), int(ngroups), float(dt), float(dh), _stream_ptr(stream)))
+        a = self._args(U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, self.cfg.device)
+        _check(lib().mhd_advance(self._h, *a, int(ngroups), float(dt), float(dh), _stream_ptr(stream)))
 
     def advance_host(self, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, chunk_groups, nstreams=3):
         """mhd_advance_host: HOST arrays (pinned torch tensors or numpy); blocking."""
-        _check(lib().mhd_advance_host(self._h, _ptr(U_in), _ptr(B_in), _ptr(U_out), _ptr(B_out), _ptr(flux_out),
-                                      _ptr(emf_out), int(ngroups), float(dt), float(dh), int(chunk_groups),
-                                      int(nstreams)))
+        a = self._args(U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, None)
+        _check(lib().mhd_advance_host(self._h, *a, int(ngroups), float(dt), float(dh), int(chunk_groups), int(nstreams)))
 
     def advance_host_dt(self, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, chunk_groups, nstreams, cfl):
         """mhd_advance_host_dt: HOST arrays; blocking; returns (dt_next, maxspeed)."""
         dtn, sm = C.c_double(), C.c_double()
-        _check(lib().mhd_advance_host_dt(self._h, _ptr(U_in), _ptr(B_in), _ptr(U_out), _ptr(B_out), _ptr(flux_out),
-                                         _ptr(emf_out), int(ngroups), float(dt), float(dh), int(chunk_groups),
+        a = self._args(U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, None)
+        _check(lib().mhd_advance_host_dt(self._h, *a, int(ngroups), float(dt), float(dh), int(chunk_groups),
                                          int(nstreams), float(cfl), C.byref(dtn), C.byref(sm)))
         return dtn.value, sm.value
 
     def advance_dt(self, U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, dt, dh, cfl, stream=None):
         dtn, sm = C.c_double(), C.c_double()
-        _check(lib().mhd_advance_dt(self._h, _ptr(U_in), _ptr(B_in), _ptr(U_out), _ptr(B_out), _ptr(flux_out), _ptr(emf_out),
-                                    int(ngroups), float(dt), float(dh), float(cfl), C.byref(dtn), C.byref(sm), _stream_ptr(stream)))
+        a = self._args(U_in, B_in, U_out, B_out, flux_out, emf_out, ngroups, self.cfg.device)
+        _check(lib().mhd_advance_dt(self._h, *a, int(ngroups), float(dt), float(dh), float(cfl), C.byref(dtn), C.byref(sm),
+                                    _stream_ptr(stream)))
         return dtn.value, sm.value
 
     def dt_reduce(self, U, B, ngroups, nghost_of_arrays, dh, cfl, stream=None):
         dt, sm = C.c_double(), C.c_double()
+        T = self.cfg.ps2 + 2 * int(nghost_of_arrays)
+        G = max(int(ngroups), 0)
+        _checked(U, self.cfg.prec, G * 5 * T ** 3, "U", self.cfg.device)
+        _checked(B, self.cfg.prec, G * 3 * T * T * (T + 1), "B", self.cfg.device)
         _check(lib().mhd_dt_reduce(self._h, _ptr(U), _ptr(B), int(ngroups), int(nghost_of_arrays), float(dh),
                                    float(cfl), C.byref(dt), C.byref(sm), _stream_ptr(stream)))
         return dt.value, sm.value

@@ -364,3 +364,49 @@ def test_config5_first_batch_through_the_host_path(oracle, scheme, recon, g, nst
     dt_ref, _ = oracle.dt_reduce(cfg, out["U"].astype(np.float64), out["B"].astype(np.float64), 0, dh, 0.3)
     assert abs(dt_next - dt_ref) <= 1e-6 * dt_ref
     assert gpu.stats() == (0, 0, 0)
+
+
+def test_nan_state_is_reported_not_turned_into_a_finite_dt():
+    """A blown-up state must not come back as MHD_OK with a usable dt (the maximum of the CFL reduction would drop a NaN
+    speed, and the floors of R9 would hide a NaN density): every dt-returning call fails with MHD_ESTATE."""
+    import torch
+    from paper_1804_03479_b200 import mhd
+    for prec, scheme, recon, g in ((0, 0, 0, 3), (1, 0, 0, 3), (0, 1, 1, 4)):
+        dtp = GU.np_dtype(prec)
+        U, B, dh = small_batch(3, g=g, dtype=dtp)
+        gpu = GU.GpuRunner(N=16, g=g, scheme=scheme, recon=recon, prec=prec, max_groups=3)
+        T = 16 + 2 * g
+        bad = U.copy().reshape(3, 5, T, T, T)
+        bad[1, 0, T // 2, T // 2, T // 2] = np.nan            # density of one interior cell of group 1
+        bad = bad.reshape(3, -1)
+        dU, dB = torch.from_numpy(bad).cuda(), torch.from_numpy(B).cuda()
+        with pytest.raises(mhd.MHDError) as ei:
+            gpu.solver.dt_reduce(dU, dB, 3, g, dh, 0.3)
+        assert ei.value.code == mhd.ESTATE
+        out = gpu.solver.alloc_outputs(3)
+        with pytest.raises(mhd.MHDError) as ei:
+            gpu.solver.advance_dt(dU, dB, out["U"], out["B"], out["flux"], out["emf"], 3, 1e-3, dh, 0.3)
+        assert ei.value.code == mhd.ESTATE
+        # the clean batch still works on the same solver afterwards
+        dt, smax = gpu.solver.dt_reduce(torch.from_numpy(U).cuda(), dB, 3, g, dh, 0.3)
+        assert np.isfinite(dt) and dt > 0 and np.isfinite(smax)
+
+
+def test_binding_rejects_wrong_dtype_size_and_device():
+    import torch
+    from paper_1804_03479_b200 import mhd
+    U, B, dh = small_batch(2, dtype=np.float64)
+    s = mhd.Solver(mhd.make_config(prec=mhd.FP64, max_groups=2))
+    dU, dB = torch.from_numpy(U).cuda(), torch.from_numpy(B).cuda()
+    out = s.alloc_outputs(2)
+    with pytest.raises(TypeError):
+        s.advance(dU.float(), dB, out["U"], out["B"], None, None, 2, 1e-3, dh)
+    with pytest.raises(ValueError):
+        s.advance(dU[:1], dB, out["U"], out["B"], None, None, 2, 1e-3, dh)          # too few elements for 2 groups
+    with pytest.raises(ValueError):
+        s.advance(torch.from_numpy(U), dB, out["U"], out["B"], None, None, 2, 1e-3, dh)   # host tensor handed to the device call
+    with pytest.raises(ValueError):
+        s.advance_host(dU, B, np.empty((2, s.n_U_out)), np.empty((2, s.n_B_out)), None, None, 2, 1e-3, dh, 1, 2)   # device tensor to the host call
+    s.advance(dU, dB, out["U"], out["B"], None, None, 2, 1e-3, dh)
+    torch.cuda.synchronize()
+    s.destroy()

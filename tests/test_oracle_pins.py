@@ -14,8 +14,14 @@ G = 5.0 / 3.0
 SCHEMES = [("vl_plm", 0, 0, 3), ("ctu_plm", 1, 0, 3), ("ctu_ppm", 1, 1, 4)]
 
 
-def mk(oracle, scheme, recon, g, N=16, riemann=1, limvar=None):
-    cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon, riemann=riemann, limvar=limvar)
+# reading R10a: the pins hold at the tie width of the FP64 path AND at the one of the FP32 path (the FP32
+# comparisons run the oracle with emf_tie = 1e-5); an inverted ramp weight, a wrong m0 scale or swapped candidates inside the
+# ramp break the uniform state (P2), div B / the shared faces (P4), the symmetries (P8) or the decomposition (P9) at 1e-5
+TIES = [1e-12, 1e-5]
+
+
+def mk(oracle, scheme, recon, g, N=16, riemann=1, limvar=None, tie=1e-12):
+    cfg = oracle.make_config(N=N, g=g, scheme=scheme, recon=recon, riemann=riemann, limvar=limvar, emf_tie=tie)
     return cfg, (lambda Ui, Bi, dt, dh: oracle.advance(cfg, Ui, Bi, dt, dh))
 
 
@@ -23,14 +29,14 @@ def mk(oracle, scheme, recon, g, N=16, riemann=1, limvar=None):
 # P2 uniform state: nothing changes, bitwise, for every scheme and solver
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name,scheme,recon,g", SCHEMES)
-@pytest.mark.parametrize("riemann", [0, 1, 2])
-def test_p2_uniform_state_is_a_fixed_point(oracle, name, scheme, recon, g, riemann):
+@pytest.mark.parametrize("riemann,tie", [(0, 1e-12), (1, 1e-12), (2, 1e-12), (1, 1e-5)])
+def test_p2_uniform_state_is_a_fixed_point(oracle, name, scheme, recon, g, riemann, tie):
     n = 16
     rho, v, p, B = 1.3, (0.4, -0.7, 0.2), 0.8, (0.5, -0.3, 0.9)
     bx = np.full((n, n, n + 1), B[0]); by = np.full((n, n + 1, n), B[1]); bz = np.full((n + 1, n, n), B[2])
     o = np.ones((n, n, n))
     U = inputs.conserved(rho * o, v[0] * o, v[1] * o, v[2] * o, p * o, bx, by, bz, G)
-    cfg, adv = mk(oracle, scheme, recon, g, riemann=riemann)
+    cfg, adv = mk(oracle, scheme, recon, g, riemann=riemann, tie=tie)
     Un, bxn, byn, bzn, out, _ = H.step_grid(adv, U, bx, by, bz, 0.01, 1.0 / n, 16, g)
     # rho and B are reproduced bitwise (their fluxes/EMFs are exact products of the uniform values);
     # M and e to round-off of the flux differences
@@ -43,10 +49,11 @@ def test_p2_uniform_state_is_a_fixed_point(oracle, name, scheme, recon, g, riema
 # P3 conservation + P4 div B + shared faces bitwise, 10 steps on a generic periodic state cut into 8 groups
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name,scheme,recon,g", SCHEMES)
-def test_p3_p4_conservation_and_divb(oracle, name, scheme, recon, g):
+@pytest.mark.parametrize("tie", TIES)
+def test_p3_p4_conservation_and_divb(oracle, name, scheme, recon, g, tie):
     n = 32
     U, bx, by, bz, dh = inputs.random_group_grid(n, 77)
-    cfg, adv = mk(oracle, scheme, recon, g)
+    cfg, adv = mk(oracle, scheme, recon, g, tie=tie)
     t0 = H.totals(U)
     assert H.rel_divb(bx, by, bz, dh) < 1e-13
     mean_b0 = [bx.mean(), by.mean(), bz.mean()]
@@ -69,18 +76,19 @@ def test_p3_p4_conservation_and_divb(oracle, name, scheme, recon, g):
 # P9 decomposition: monolithic 32^3 vs 8 groups of 16^3 with g ghosts: bitwise; one ghost fewer: not
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name,scheme,recon,g", SCHEMES)
-def test_p9_decomposition_is_bitwise_and_ghost_width_is_minimal(oracle, name, scheme, recon, g):
+@pytest.mark.parametrize("tie", TIES)
+def test_p9_decomposition_is_bitwise_and_ghost_width_is_minimal(oracle, name, scheme, recon, g, tie):
     n = 32
     U, bx, by, bz, dh = inputs.random_group_grid(n, 5)
     dt = 0.2 * dh
-    cfgM, advM = mk(oracle, scheme, recon, g, N=32)
-    cfgD, advD = mk(oracle, scheme, recon, g, N=16)
+    cfgM, advM = mk(oracle, scheme, recon, g, N=32, tie=tie)
+    cfgD, advD = mk(oracle, scheme, recon, g, N=16, tie=tie)
     a = H.step_grid(advM, U, bx, by, bz, dt, dh, 32, g)
     b = H.step_grid(advD, U, bx, by, bz, dt, dh, 16, g)
     for x, y in zip(a[:4], b[:4]):
         assert np.array_equal(x, y)
     # extra garbage layer beyond g must not matter: g+1 ghosts, outermost layer overwritten with junk
-    cfgE = oracle.make_config(N=16, g=g + 1, scheme=scheme, recon=recon)
+    cfgE = oracle.make_config(N=16, g=g + 1, scheme=scheme, recon=recon, emf_tie=tie)
     Ui, Bi = inputs.pack_groups(U, bx, by, bz, 16, g + 1)
     out0 = oracle.advance(cfgE, Ui, Bi, dt, dh)
     T = 16 + 2 * (g + 1)
@@ -90,7 +98,7 @@ def test_p9_decomposition_is_bitwise_and_ghost_width_is_minimal(oracle, name, sc
     out1 = oracle.advance(cfgE, Uj.reshape(Ui.shape), Bi, dt, dh)
     assert np.array_equal(out0["U"], out1["U"]) and np.array_equal(out0["B"], out1["B"])
     # one ghost cell fewer than required changes the answer (forced past the config check)
-    cfgS = oracle.make_config(N=16, g=g - 1, scheme=scheme, recon=recon)
+    cfgS = oracle.make_config(N=16, g=g - 1, scheme=scheme, recon=recon, emf_tie=tie)
     Ui, Bi = inputs.pack_groups(U, bx, by, bz, 16, g - 1)
     outS = oracle.advance(cfgS, Ui, Bi, dt, dh, force_ghost_ok=True)
     Us, bxs, bys, bzs, _ = inputs.unpack_groups(outS["U"], outS["B"], n, 16)
@@ -119,12 +127,12 @@ def _mirror_x(U, bx, by, bz):
 
 
 @pytest.mark.parametrize("name,scheme,recon,g", [SCHEMES[0], SCHEMES[2]])
-@pytest.mark.parametrize("riemann", [1, 2])
-def test_p8_axis_permutation_and_mirror(oracle, name, scheme, recon, g, riemann):
+@pytest.mark.parametrize("riemann,tie", [(1, 1e-12), (2, 1e-12), (1, 1e-5)])
+def test_p8_axis_permutation_and_mirror(oracle, name, scheme, recon, g, riemann, tie):
     n = 16
     U, bx, by, bz, dh = inputs.random_group_grid(n, 11)
     dt = 0.25 * dh
-    cfg, adv = mk(oracle, scheme, recon, g, riemann=riemann)
+    cfg, adv = mk(oracle, scheme, recon, g, riemann=riemann, tie=tie)
     ref = H.step_grid(adv, U, bx, by, bz, dt, dh, 16, g)[:4]
     for tf in (_permute, _mirror_x):
         got = H.step_grid(adv, *tf(U, bx, by, bz), dt, dh, 16, g)[:4]
@@ -138,10 +146,13 @@ def test_p8_axis_permutation_and_mirror(oracle, name, scheme, recon, g, riemann)
 # ------------------------------------------------------------------------------------------------
 # P6 ABC force-free equilibrium with uniform pressure: the residual of one step converges at 2nd order
 # ------------------------------------------------------------------------------------------------
+@pytest.mark.slow
 @pytest.mark.parametrize("name,scheme,recon,g", [SCHEMES[0], SCHEMES[2]])
 def test_p6_abc_equilibrium_residual_converges(oracle, name, scheme, recon, g):
+    """N = 16, 32, 64: the change of M and b over one step at CFL 0.3 shrinks >= 3.5x per doubling of N in the max
+    norm (the limiter clips the extrema: O(h^2)), and the rate of change in the mean norm by more than 3x"""
     res = []
-    for n in (16, 32):
+    for n in (16, 32, 64):
         U, bx, by, bz, dh = inputs.abc_grid(n, 0, p0=1.0, vamp=0.0)
         cfg, adv = mk(oracle, scheme, recon, g, N=n)
         c0 = oracle.make_config(N=n, g=3)
@@ -149,18 +160,22 @@ def test_p6_abc_equilibrium_residual_converges(oracle, name, scheme, recon, g):
         dt, _ = oracle.dt_reduce(c0, Ui, Bi, 0, dh, 0.3)
         Un, bxn, byn, bzn, _, _ = H.step_grid(adv, U, bx, by, bz, dt, dh, n, g)
         # rate of change (divide by dt: dt itself halves with dh)
-        res.append((np.abs(Un[1:4] - U[1:4]).mean() / dt, np.abs(bxn - bx).mean() / dt, np.abs(Un[0] - U[0]).max()))
-    assert res[0][0] / res[1][0] > 3.0 and res[0][1] / res[1][1] > 3.0, res
-    assert res[0][0] < 1.0      # a mis-signed tension/pressure term would leave a force ~ k B^2 ~ 12
-    assert res[1][2] < 3e-3 and res[1][2] < res[0][2]
+        res.append(dict(dM_rate=np.abs(Un[1:4] - U[1:4]).mean() / dt, db_rate=np.abs(bxn - bx).mean() / dt, drho=np.abs(Un[0] - U[0]).max(),
+                        dM_max=np.abs(Un[1:4] - U[1:4]).max(), db_max=max(np.abs(bxn - bx).max(), np.abs(byn - by).max(), np.abs(bzn - bz).max())))
+    print("P6", name, res)
+    for a, b in ((res[0], res[1]), (res[1], res[2])):
+        assert a["dM_rate"] / b["dM_rate"] > 3.0 and a["db_rate"] / b["db_rate"] > 3.0, res
+        assert a["dM_max"] / b["dM_max"] >= 3.5, res
+    assert res[0]["dM_rate"] < 1.0      # a mis-signed tension/pressure term would leave a force ~ k B^2 ~ 12
+    assert res[1]["drho"] < 3e-3 and res[2]["drho"] < res[1]["drho"] < res[0]["drho"]
 
 
 # ------------------------------------------------------------------------------------------------
 # P7 field loop: the out-of-plane field of an advected in-plane loop stays at round-off (CTU source terms)
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("name,scheme,recon,g", SCHEMES)
-@pytest.mark.parametrize("cdir", [2, 0])
-def test_p7_field_loop_out_of_plane_field(oracle, name, scheme, recon, g, cdir):
+@pytest.mark.parametrize("cdir,tie", [(2, 1e-12), (0, 1e-12), (2, 1e-5)])
+def test_p7_field_loop_out_of_plane_field(oracle, name, scheme, recon, g, cdir, tie):
     n, nc = 32, 16
     a, b = (cdir + 1) % 3, (cdir + 2) % 3
     shape_xyz = [n, n, n]; shape_xyz[cdir] = nc
@@ -180,7 +195,7 @@ def test_p7_field_loop_out_of_plane_field(oracle, name, scheme, recon, g, cdir):
     v = [0.0, 0.0, 0.0]; v[a] = 1.0; v[b] = 0.5; v[cdir] = 1.0
     o = np.ones((nz, ny, nx))
     U = inputs.conserved(o, v[0] * o, v[1] * o, v[2] * o, o, bx, by, bz, G)
-    cfg, adv = mk(oracle, scheme, recon, g)
+    cfg, adv = mk(oracle, scheme, recon, g, tie=tie)
     dt = 0.3 * dh / (1.0 + np.sqrt(G))
     for _ in range(10):
         U, bx, by, bz, _, _ = H.step_grid(adv, U, bx, by, bz, dt, dh, 16, g)
