@@ -1,4 +1,5 @@
 // mhd_march.cu -- instantiations and launchers of the plane-marching VL kernels (mhd_vl_march.cuh)
+#include <algorithm>
 #include <cstdlib>
 #include "mhd_march.h"
 #include "mhd_vl_march.cuh"
@@ -6,6 +7,11 @@
 namespace mhd {
 
 namespace {
+
+// block slots of the marching kernels on one B200 (two resident blocks on each of 148 SMs); MHD_MARCH_SLOTS overrides (tests: 1 = never
+// chunk, a large value = always the finest chunks)
+inline int march_slots() { const char* e = getenv("MHD_MARCH_SLOTS"); const int v = e ? atoi(e) : 0; return v > 0 ? v : 296; }
+#define kMarchSlots march_slots()
 
 template <class K> cudaError_t big_smem(K kernel, size_t bytes) {
   return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
@@ -15,7 +21,9 @@ template <class R, int SOLVER, int LIM>
 cudaError_t launch2(const KParamsSC<R, 23>& p, int ng, cudaStream_t st) {
   cudaError_t e = big_smem(k_vl_march2<R, SOLVER, LIM>, march2_smem<R>());
   if (e != cudaSuccess) return e;
-  k_vl_march2<R, SOLVER, LIM><<<ng, kM2P, march2_smem<R>(), st>>>(p);
+  // chunks of the 16 interior planes: as many as keep the grid within one wave of the 2 x 148 block slots (see k_vl_march1)
+  const int chunks = std::max(1, std::min(8, kMarchSlots / ng)), per = (16 + chunks - 1) / chunks;
+  k_vl_march2<R, SOLVER, LIM><<<dim3(ng, (16 + per - 1) / per), kM2P, march2_smem<R>(), st>>>(p, per);
   return cudaGetLastError();
 }
 
@@ -25,13 +33,14 @@ cudaError_t launch_solver(const KParamsSC<R, 23>& p, int ng, int lim, int pass, 
     // bulk copies need 16-byte aligned planes: the group strides are multiples of 16 bytes, the base pointers must be
     static const bool no_tma = getenv("MHD_NO_TMA") != nullptr;
     const bool tma = !no_tma && ((reinterpret_cast<size_t>(p.Uin) | reinterpret_cast<size_t>(p.Bin)) & 15) == 0;
+    const int chunks = std::max(1, std::min(10, kMarchSlots / ng)), per = (20 + chunks - 1) / chunks;   // 20 half-step planes
     cudaError_t e;
     if (tma) {
       if ((e = big_smem(k_vl_march1<R, SOLVER, true>, march1_smem<R, true>())) != cudaSuccess) return e;
-      k_vl_march1<R, SOLVER, true><<<ng, kMP, march1_smem<R, true>(), st>>>(p);
+      k_vl_march1<R, SOLVER, true><<<dim3(ng, (20 + per - 1) / per), kMP, march1_smem<R, true>(), st>>>(p, per);
     } else {
       if ((e = big_smem(k_vl_march1<R, SOLVER, false>, march1_smem<R, false>())) != cudaSuccess) return e;
-      k_vl_march1<R, SOLVER, false><<<ng, kMP, march1_smem<R, false>(), st>>>(p);
+      k_vl_march1<R, SOLVER, false><<<dim3(ng, (20 + per - 1) / per), kMP, march1_smem<R, false>(), st>>>(p, per);
     }
     return cudaGetLastError();
   }

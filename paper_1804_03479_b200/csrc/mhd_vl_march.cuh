@@ -113,8 +113,12 @@ template <class R, bool TMA> constexpr size_t march1_smem() {
   return (size_t)((2 * 11 + 21 + 3 + 2) * kMP + (TMA ? 7 * kMP + 2 * kMXP : 0)) * sizeof(R) + (TMA ? 16 : 0);
 }
 
+// grid = (groups, chunks): a small batch is cut along z into `chunks` blocks per group so that it still fills the GPU.  A chunk that
+// owns the half-step planes [k0, k1) marches over the planes k0-1 .. k1: the first plane only sets up what the others carry (its
+// primitives and x / y face data), so every chunk repeats two planes of solves; the values it produces are those of the whole march,
+// bit for bit (same operations on the same operands), whatever the number of chunks.
 template <class R, int SOLVER, bool TMA>
-__global__ void __launch_bounds__(kMP, sizeof(R) == 4 ? 2 : 1) k_vl_march1(const KParamsSC<R, 23> p) {
+__global__ void __launch_bounds__(kMP, sizeof(R) == 4 ? 2 : 1) k_vl_march1(const KParamsSC<R, 23> p, const int per) {
   constexpr int T = kMT, P = kMP, T3 = T * T * T, XP = T * (T + 1);
   extern __shared__ __align__(16) unsigned char march_smem[];
   R* sW = reinterpret_cast<R*>(march_smem);     // [2][11][P]: primitives (8) and reference EMFs (3) of planes k, k-1
@@ -136,33 +140,34 @@ __global__ void __launch_bounds__(kMP, sizeof(R) == 4 ? 2 : 1) k_vl_march1(const
   const bool cell = i >= 1 && i < T - 1 && j >= 1 && j < T - 1;       // half-step cells of the plane
   const bool corner = i >= 1 && j >= 1;                                // edges through the lowest corner exist
   const bool fx = corner && j < T - 1, fy = corner && i < T - 1;       // lower x / y faces of half-step cells (and their upper rim)
+  const int k0 = 1 + (int)blockIdx.y * per, k1 = min(T - 1, k0 + per), kb = k0 - 1;   // this block's half-step planes [k0, k1), first plane of the march
   // stage plane kn: U, Bx, By of plane kn and Bz of level kn+1 (the prologue also brings level 0).  A face plane of
   // 22 x 23 floats starts on an 8-byte boundary for odd kn: the copy starts at the 16-byte boundary below it
   auto stage = [&](int kn) {
     constexpr unsigned PB = P * sizeof(R);
     const unsigned mis = (unsigned)((size_t)kn * XP * sizeof(R)) & 15u;
     const unsigned XB = (unsigned)(XP * sizeof(R) + mis + 15u) & ~15u;
-    mbar_expect_tx(bar, (kn == 0 ? 7u : 6u) * PB + 2u * XB);
+    mbar_expect_tx(bar, (kn == kb ? 7u : 6u) * PB + 2u * XB);
 #pragma unroll
     for (int v = 0; v < 5; ++v) bulk_load(sU + v * P, U + v * T3 + kn * P, PB, bar);
     bulk_load(sBx, reinterpret_cast<const char*>(Bx + kn * XP) - mis, XB, bar);
     bulk_load(sBy, reinterpret_cast<const char*>(By + kn * XP) - mis, XB, bar);
-    if (kn == 0) bulk_load(sBz, Bz, PB, bar);
+    if (kn == kb) bulk_load(sBz + (kn & 1) * P, Bz + kn * P, PB, bar);
     bulk_load(sBz + ((kn + 1) & 1) * P, Bz + (kn + 1) * P, PB, bar);
   };
   if (TMA) {
-    if (t == 0) { mbar_init(bar, 1); stage(0); }
+    if (t == 0) { mbar_init(bar, 1); stage(kb); }
     __syncthreads();
   }
   R A[5] = { R(0), R(0), R(0), R(0), R(0) };                           // (x, y flux differences) - (lower z flux) of cell k
   R Cx = R(0), Cy = R(0), bzlo = R(0);                                 // open CT sums of the lower x / y faces; finished lower z face
   R pFx0 = R(0), pFx6 = R(0), pFy0 = R(0), pFy5 = R(0);                // x / y face data of the plane below
-  for (int k = 0; k < T; ++k) {
+  for (int k = kb; k <= k1; ++k) {
     R* Wc = sW + (k & 1) * 11 * P;
     const R* Wp = sW + ((k & 1) ^ 1) * 11 * P;
     R bl[3], W[8];
     if (TMA) {
-      mbar_wait(bar, k & 1);
+      mbar_wait(bar, (unsigned)(k - kb) & 1u);
       const int sh = (int)((((size_t)k * XP * sizeof(R)) & 15u) / sizeof(R));
       R u[5], bu[3];
 #pragma unroll
@@ -182,7 +187,7 @@ __global__ void __launch_bounds__(kMP, sizeof(R) == 4 ? 2 : 1) k_vl_march1(const
     Wc[9 * P + t] = W[1] * W[7] - W[3] * W[5];
     Wc[10 * P + t] = W[2] * W[5] - W[1] * W[6];
     __syncthreads();
-    if (TMA && t == 0 && k + 1 < T) stage(k + 1);          // every thread has taken plane k out of the staging buffers
+    if (TMA && t == 0 && k + 1 <= k1) stage(k + 1);        // every thread has taken plane k out of the staging buffers
     {
       R wl[7], wr[7], F[7];
       if (i >= 1) {
@@ -197,7 +202,7 @@ __global__ void __launch_bounds__(kMP, sizeof(R) == 4 ? 2 : 1) k_vl_march1(const
 #pragma unroll
         for (int v = 0; v < 7; ++v) sF[(7 + v) * P + t] = F[v];
       }
-      if (k >= 1) {
+      if (k > kb) {
         gen_from_smem<R, 2>(Wp, t, wl); gen_from_prim<R, 2>(W, wr);
         if (riemann<R, SOLVER>(wl, wr, bl[2], p.gam, p.gm1inv, F)) count_event(p.stats + 2);
 #pragma unroll
@@ -207,7 +212,7 @@ __global__ void __launch_bounds__(kMP, sizeof(R) == 4 ? 2 : 1) k_vl_march1(const
     __syncthreads();
     // time-n data of cell (i, j, k-1) and its lower x / y faces, read a second time (L2): asked for here, used below
     R Uo[5] = { R(0), R(0), R(0), R(0), R(0) }, bxo = R(0), byo = R(0);
-    if (k >= 2) {
+    if (k >= kb + 2) {
       const int cq = ((k - 1) * T + j) * T + i;
       if (cell) {
 #pragma unroll
@@ -219,13 +224,13 @@ __global__ void __launch_bounds__(kMP, sizeof(R) == 4 ? 2 : 1) k_vl_march1(const
     // ---- edge EMFs: E_z of this plane, E_x / E_y of the level k-1/2 ----
     R Ex = R(0), Ey = R(0), Ez = R(0);
     if (corner) {
-      march_emfs<R, P>(sF, Wc + 8 * P, Wp + 8 * P, Wc, Wp, t, 1, T, pFx0, pFx6, pFy0, pFy5, ht, k >= 1, Ex, Ey, Ez);
+      march_emfs<R, P>(sF, Wc + 8 * P, Wp + 8 * P, Wc, Wp, t, 1, T, pFx0, pFx6, pFy0, pFy5, ht, k > kb, Ex, Ey, Ez);
       pFx0 = sF[t]; pFx6 = sF[6 * P + t]; pFy0 = sF[7 * P + t]; pFy5 = sF[12 * P + t];
     }
     sE[t] = Ex; sE[P + t] = Ey; sE[2 * P + t] = Ez;
     // ---- CT (Eq. 13 with dt/2) of the lower x / y faces of plane k-1: their open sums close with E_y / E_x of this level ----
     R bxh = R(0), byh = R(0);
-    if (k >= 2) {
+    if (k >= kb + 2) {
       if (fx) { bxh = bxo - qh * (Cx - Ey); ws[(size_t)(M_BH + 0) * T3 + (k - 1) * P + t] = bxh; }
       if (fy) { byh = byo - qh * (Ex + Cy); ws[(size_t)(M_BH + 1) * T3 + (k - 1) * P + t] = byh; }
     }
@@ -241,13 +246,13 @@ __global__ void __launch_bounds__(kMP, sizeof(R) == 4 ? 2 : 1) k_vl_march1(const
     __syncthreads();
     // ---- the lower z face of level k-1/2 is complete; open the sums of the lower x / y faces of plane k; cell (i, j, k-1) ----
     R bzh = R(0);
-    if (cell && k >= 1) {
+    if (cell && k > kb) {
       bzh = bl[2] - qh * ((sE[P + t + 1] - Ey) - (sE[t + T] - Ex));
       ws[(size_t)(M_BH + 2) * T3 + k * P + t] = bzh;
     }
     if (fx) Cx = (sE[2 * P + t + T] - Ez) + Ey;
     if (fy) Cy = -Ex - (sE[2 * P + t + 1] - Ez);
-    if (cell && k >= 2) {
+    if (cell && k >= kb + 2) {
       // the upper x / y faces of a cell are the lower faces of its neighbours
       const R blh[3] = { bxh, byh, bzlo }, buh[3] = { sX[t + 1], sX[P + t + T], bzh };
       R Wh[8];
@@ -276,7 +281,7 @@ template <class R> constexpr size_t march2_smem() {
 // S9 (p.red set: mhd_advance_dt) is a run-time branch, not a template flag: the two instantiations compiled the energy flux of
 // the Riemann solve to different last bits in FP32, and mhd_advance_dt must equal mhd_advance + mhd_dt_reduce bit for bit
 template <class R, int SOLVER, int LIM>
-__global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_march2(const KParamsSC<R, 23> p) {
+__global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_march2(const KParamsSC<R, 23> p, const int per) {
   constexpr int T = kMT, PT = kMT * kMT, T3 = T * T * T, P = kM2P, W = kM2W, N = 16, M = N + 1, g = 3;
   extern __shared__ __align__(16) unsigned char march_smem[];
   R* sR = reinterpret_cast<R*>(march_smem);     // [3][8][PT]: half-step primitives of planes k-1, k, k+1 (plane kp in slot kp % 3)
@@ -313,6 +318,7 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
   R pFx0 = R(0), pFx6 = R(0), pFy0 = R(0), pFy5 = R(0);
   R smax = R(0);
   const bool DT = p.red != nullptr;
+  const int k0 = g + (int)blockIdx.y * per, k1 = min(g + N, k0 + per), kb = k0 - 1;     // this block's interior planes [k0, k1) (see k_vl_march1)
   // stage the 8 primitives of plane kp into its ring slot
   auto stage = [&](int kp, bool arm) {
     constexpr unsigned PB = PT * sizeof(R);
@@ -323,12 +329,12 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
   if (t == 0) {
     mbar_init(bar, 1);
     mbar_expect_tx(bar, 3u * 8u * PT * sizeof(R));
-    stage(g - 2, false); stage(g - 1, false); stage(g, false);
+    stage(kb - 1, false); stage(kb, false); stage(kb + 1, false);
   }
   __syncthreads();
   mbar_wait(bar, 0);
-  R bhn[3] = { bh[(g - 1) * PT + c], bh[T3 + (g - 1) * PT + c], bh[2 * T3 + (g - 1) * PT + c] };   // normal fields of the lower faces of plane k
-  for (int k = g - 1; k <= g + N; ++k) {
+  R bhn[3] = { bh[kb * PT + c], bh[T3 + kb * PT + c], bh[2 * T3 + kb * PT + c] };   // normal fields of the lower faces of plane k
+  for (int k = kb; k <= k1; ++k) {
     R* Cc = sC + (k & 1) * 4 * P;
     const R* Cp = sC + ((k & 1) ^ 1) * 4 * P;
     const R* Rk = sR + (k % 3) * 8 * PT;
@@ -370,10 +376,10 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
       // z face between planes k-1 and k: the upper state of the cell below was left in sZ one plane ago
       {
         R wp[7];
-        if (k > g - 1) mbar_wait(bar, (unsigned)(k - (g - 1)) & 1u);        // plane k+1 has landed (planes <= g with the prologue)
+        if (k > kb) mbar_wait(bar, (unsigned)(k - kb) & 1u);                 // plane k+1 has landed (the first three with the prologue)
         load_gen<R, 2>(sR + ((k + 2) % 3) * 8 * PT, PT, c, wm); gen_from_prim<R, 2>(W0, w0); load_gen<R, 2>(sR + ((k + 1) % 3) * 8 * PT, PT, c, wp);
         slope3<R, LIM>(wm, w0, wp, W0[7], p.gam, sr);
-        if (k >= g) {
+        if (k > kb) {
 #pragma unroll
           for (int v = 0; v < 7; ++v) { wl[v] = sZ[v * P + t]; wr[v] = w0[v] - R(0.5) * sr[v]; }
           apply_floors(p, wl); apply_floors(p, wr);
@@ -386,10 +392,10 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
       }
     }
     __syncthreads();
-    if (t == 0 && k + 2 <= g + N + 1) stage(k + 2, true);                 // into the slot of plane k-1: nobody reads it any more
+    if (t == 0 && k + 2 <= k1 + 1) stage(k + 2, true);                    // into the slot of plane k-1: nobody reads it any more
     // time-n data of cell (i, j, k-1), its lower x / y faces and the lower z face of level k-1/2: asked for here, used below
     R Ut[5] = { R(0), R(0), R(0), R(0), R(0) }, bxo = R(0), byo = R(0), bzo = R(0);
-    if (k >= g + 1) {
+    if (k >= kb + 2) {
       const int cq = ((k - 1) * T + j) * T + i;
       if (in) {
 #pragma unroll
@@ -398,8 +404,8 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
       if (fx) bxo = Bx[((k - 1) * T + j) * (T + 1) + i];
       if (fy) byo = By[((k - 1) * (T + 1) + j) * T + i];
     }
-    if (in && k >= g) bzo = Bz[(k * T + j) * T + i];
-    if (k < g + N) {
+    if (in && k > kb) bzo = Bz[(k * T + j) * T + i];
+    if (k < k1) {
       const int qn = (k + 1) * PT + c;
       bhn[0] = bh[qn]; bhn[1] = bh[T3 + qn]; bhn[2] = bh[2 * T3 + qn];
     }
@@ -408,7 +414,7 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
     if (in) {
       R dxy[5], fz[5];
       march_fluxdiv<R, P>(sF, t, 1, W, dxy, fz);
-      if (k >= g + 1) {
+      if (k >= kb + 2) {
         const int oq = ((kk - 1) * N + jj) * N + ii;
 #pragma unroll
         for (int v = 0; v < 5; ++v) { Un[v] = Ut[v] - q * (A[v] + fz[v]); Uo[v * N * N * N + oq] = Un[v]; }
@@ -427,7 +433,7 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
         R* f = fo + (size_t)(3 + sy) * 5 * NN + ii * N + kk;
         f[0] = sF[7 * P + t]; f[2 * NN] = sF[8 * P + t]; f[3 * NN] = sF[9 * P + t]; f[NN] = sF[10 * P + t]; f[4 * NN] = sF[11 * P + t];
       }
-      if (in && (kk == 0 || kk == N / 2 || kk == N)) {                   // z planes: [y][x], z faces carry (rho, Mz, Mx, My, e)
+      if (in && k > kb && (kk == 0 || kk == N / 2 || kk == N)) {         // z planes: [y][x], z faces carry (rho, Mz, Mx, My, e)
         R* f = fo + (size_t)(6 + (kk == 0 ? 0 : (kk == N ? 2 : 1))) * 5 * NN + jj * N + ii;
         f[0] = sF[14 * P + t]; f[3 * NN] = sF[15 * P + t]; f[NN] = sF[16 * P + t]; f[2 * NN] = sF[17 * P + t]; f[4 * NN] = sF[18 * P + t];
       }
@@ -435,13 +441,13 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
     // ---- edge EMFs ----
     R Ex = R(0), Ey = R(0), Ez = R(0);
     if (corner) {
-      march_emfs<R, P>(sF, Cc, Cp, Cc + 3 * P, Cp + 3 * P, t, 1, W, pFx0, pFx6, pFy0, pFy5, ht, k >= g, Ex, Ey, Ez);
+      march_emfs<R, P>(sF, Cc, Cp, Cc + 3 * P, Cp + 3 * P, t, 1, W, pFx0, pFx6, pFy0, pFy5, ht, k > kb, Ex, Ey, Ez);
       pFx0 = sF[t]; pFx6 = sF[6 * P + t]; pFy0 = sF[7 * P + t]; pFy5 = sF[12 * P + t];
     }
     sE[t] = Ex; sE[P + t] = Ey; sE[2 * P + t] = Ez;
     if (eo && corner) {
       const int MN = M * N;
-      const bool kf = kk >= 0 && kk <= N, kc = kk >= 0 && kk < N;         // kf: the level k-1/2 is an interior face level; kc: plane k is interior
+      const bool kf = k > kb, kc = kk >= 0 && kk < N;                      // kf: the EMFs of the level k-1/2 exist (an interior face level); kc: plane k is interior
       if (sx >= 0) {                                                     // x planes: E_y [z: N+1][y: N], E_z [z: N][y: N+1]
         R* e = eo + (size_t)(0 + sx) * 2 * MN;
         if (kf && jj < N) e[kk * N + jj] = Ey;
@@ -452,7 +458,7 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
         if (kc) e[ii * N + kk] = Ez;
         if (kf && ii < N) e[MN + ii * M + kk] = Ex;
       }
-      if (kk == 0 || kk == N / 2 || kk == N) {                           // z planes: E_x [y: N+1][x: N], E_y [y: N][x: N+1]
+      if (kf && (kk == 0 || kk == N / 2 || kk == N)) {                   // z planes: E_x [y: N+1][x: N], E_y [y: N][x: N+1]
         R* e = eo + (size_t)(6 + (kk == 0 ? 0 : (kk == N ? 2 : 1))) * 2 * MN;
         if (ii < N) e[jj * N + ii] = Ex;
         if (jj < N) e[MN + jj * M + ii] = Ey;
@@ -461,25 +467,25 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
     __syncthreads();
     // ---- CT (Eq. 13): lower z face of level k-1/2; lower x / y faces of plane k-1 ----
     R bzn = R(0), bxn = R(0), byn = R(0);
-    if (in && k >= g) {
+    if (in && k > kb) {
       bzn = bzo - q * ((sE[P + t + 1] - Ey) - (sE[t + W] - Ex));
       Bzo[(kk * N + jj) * N + ii] = bzn;
     }
     if (fx) {
-      if (k >= g + 1) {
+      if (k >= kb + 2) {
         bxn = bxo - q * (Cx - Ey);
         Bxo[((kk - 1) * N + jj) * (N + 1) + ii] = bxn;
       }
       Cx = (sE[2 * P + t + W] - Ez) + Ey;
     }
     if (fy) {
-      if (k >= g + 1) {
+      if (k >= kb + 2) {
         byn = byo - q * (Ex + Cy);
         Byo[((kk - 1) * (N + 1) + jj) * N + ii] = byn;
       }
       Cy = -Ex - (sE[2 * P + t + 1] - Ez);
     }
-    if (DT && k >= g + 1) {
+    if (DT && k >= kb + 2) {
       // S9 on the new state of cell (i, j, k-1): its upper x / y faces are the lower faces of the neighbours
       sX[t] = bxn; sX[P + t] = byn;
       __syncthreads();

@@ -410,3 +410,62 @@ def test_binding_rejects_wrong_dtype_size_and_device():
     s.advance(dU, dB, out["U"], out["B"], None, None, 2, 1e-3, dh)
     torch.cuda.synchronize()
     s.destroy()
+
+
+@pytest.mark.parametrize("prec,scheme,recon,g", [(0, 0, 0, 3), (1, 0, 0, 3), (0, 1, 1, 4), (1, 1, 1, 4)])
+def test_guard_bands_and_run_to_run_determinism(prec, scheme, recon, g):
+    """Stand-in for compute-sanitizer memcheck / racecheck, which is closed on this GPU pool (profiles/r02_sanitizers.md):
+    (a) every output array sits between guard bands of a sentinel value that must survive the call (an out-of-bounds store of
+    the epilogues lands there); the inputs sit at the very end of their allocation with a NaN band in front (an
+    out-of-bounds load below the array would poison the result); (b) ten repeated calls give bitwise the same outputs and the
+    same dt (an unsynchronised shared-memory hand-off in the plane-marching / pencil kernels shows up as run-to-run noise)."""
+    import torch
+    from paper_1804_03479_b200 import mhd
+    dtp = GU.np_dtype(prec)
+    G, PAD = 9, 4096
+    U, B, dh = small_batch(G, g=g, dtype=dtp)
+    s = mhd.Solver(mhd.make_config(N=16, g=g, scheme=scheme, recon=recon, prec=prec, max_groups=G))
+    tdt = torch.float32 if prec == 0 else torch.float64
+
+    def banded(n, fill):
+        t = torch.full((PAD + n + PAD,), fill, dtype=tdt, device="cuda")
+        return t, t[PAD:PAD + n]
+    inU_all = torch.full((PAD + U.size,), float("nan"), dtype=tdt, device="cuda"); inU = inU_all[PAD:]; inU.copy_(torch.from_numpy(U.ravel()))
+    inB_all = torch.full((PAD + B.size,), float("nan"), dtype=tdt, device="cuda"); inB = inB_all[PAD:]; inB.copy_(torch.from_numpy(B.ravel()))
+    SENT = 12345.0
+    bufs = {k: banded(G * n, SENT) for k, n in (("U", s.n_U_out), ("B", s.n_B_out), ("flux", s.n_flux), ("emf", s.n_emf))}
+    ref = None
+    for rep in range(10):
+        for _, v in bufs.values():
+            v.fill_(-1.0)
+        dt, sm = s.advance_dt(inU, inB, bufs["U"][1], bufs["B"][1], bufs["flux"][1], bufs["emf"][1], G, 2e-3, dh, 0.3)
+        got = {k: v[1].cpu().numpy().copy() for k, v in bufs.items()}
+        got["dt"] = np.array([dt, sm])
+        for k, (full, view) in bufs.items():
+            assert bool((full[:PAD] == SENT).all()) and bool((full[-PAD:] == SENT).all()), (k, "guard band overwritten")
+            assert np.isfinite(got[k]).all() and not (got[k] == -1.0).all(), k
+        if ref is None:
+            ref = got
+        for k in ref:
+            assert np.array_equal(ref[k], got[k]), (rep, k)
+    s.destroy()
+
+
+@pytest.mark.parametrize("prec", [1, 0])
+def test_march_chunks_give_the_same_bits(prec, monkeypatch):
+    """A small batch of the standard VL group is cut along z into several blocks per group (csrc/mhd_vl_march.cuh) so that it
+    still fills the GPU; every chunking gives bitwise the outputs and the CFL speed of the whole-column march."""
+    dtp = GU.np_dtype(prec)
+    G = 5
+    U, B, dh = small_batch(G, g=3, dtype=dtp)
+    res = []
+    for slots in ("1", "12", "25", "100000"):            # 1, 2, 5 and 10 / 8 chunks per group
+        monkeypatch.setenv("MHD_MARCH_SLOTS", slots)
+        gpu = GU.GpuRunner(N=16, g=3, scheme=0, recon=0, prec=prec, max_groups=G)
+        out, dt, sm = gpu.advance_dt(U, B, 2e-3, dh, 0.3)
+        out["dt"] = np.array([dt, sm])
+        res.append(out)
+    monkeypatch.delenv("MHD_MARCH_SLOTS")
+    for r in res[1:]:
+        for k in ("U", "B", "flux", "emf", "dt"):
+            assert np.array_equal(res[0][k], r[k]), k
