@@ -85,7 +85,7 @@ int main() {
     const int T = N + 2 * v.g;
     mhdref_config cfg; cfg.ps2 = N; cfg.nghost = v.g; cfg.gamma = Counted(gam); cfg.scheme = v.scheme; cfg.recon = v.recon;
     cfg.riemann = v.riemann; cfg.limvar = v.limvar; cfg.min_dens = Counted(1e-10); cfg.min_pres = Counted(1e-10); cfg.emf_tie = Counted(1e-12); cfg.limiter = 0;
-    cfg.minimal_ranges = mn;
+    cfg.minimal_ranges = mn; cfg.hcorr = 0;
     std::vector<Counted> U(5 * T * T * T), B(3 * T * T * (T + 1)), Uo(5 * N * N * N), Bo(3 * N * N * (N + 1)), fo(9 * 5 * N * N), eo(9 * 2 * (N + 1) * N);
     const real_t k = 2.0 * 3.14159265358979323846 / N;
     for (int kk = 0; kk < T; ++kk) for (int j = 0; j < T; ++j) for (int i = 0; i < T; ++i) {

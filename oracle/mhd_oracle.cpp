@@ -44,6 +44,8 @@ typedef struct {
   int minimal_ranges;  // 0: every stage on the maximal index range on which its inputs exist (the default); 1: every stage only
                        // where the final update of the N^3 interior cells needs it.  Same arithmetic per
                        // cell / face / edge; the outputs are bitwise the same (pinned), only the operation count differs
+  int hcorr;           // NEXT-4 variant (reading R19): H-correction of the Roe solver (multidimensional entropy fix);
+                       // needs riemann = Roe and one ghost cell more than the scheme alone; evaluated on the maximal ranges
 } mhdref_config;
 // measurement hook (oracle/count_ops.cpp): called with the number of the step that just finished inside one group's update
 void (*mhdref_stage_hook)(int) = nullptr;
@@ -312,7 +314,8 @@ void hlld(const double WL[7], const double WR[7], double Bn, double gam, double 
 
 // Roe (reading R7/R11): 1/2(FL+FR) - 1/2 sum |lam_k| (L_k.dU) R_k, HLLE fallback
 // returns 1 if it fell back to HLLE
-int roe(const double WL[7], const double WR[7], double Bn, double gam, double F[7]) {
+// etah (reading R19, H-correction): every wave speed of the dissipation term is |lam_k| -> max(|lam_k|, etah); etah = 0: plain Roe
+int roe(const double WL[7], const double WR[7], double Bn, double gam, double F[7], double etah = 0.0) {
   double UL[7], UR[7], FL[7], FR[7];
   prim2cons(WL, Bn, gam, UL); prim2cons(WR, Bn, gam, UR);
   physflux(WL, Bn, UL, FL); physflux(WR, Bn, UR, FR);
@@ -336,16 +339,21 @@ int roe(const double WL[7], const double WR[7], double Bn, double gam, double F[
   }
   for (int c = 0; c < 7; ++c) {
     double d = 0.0;
-    for (int k = 0; k < 7; ++k) d += std::fabs(lam[k]) * a[k] * R[k][c];
+    for (int k = 0; k < 7; ++k) d += std::max(std::fabs(lam[k]), etah) * a[k] * R[k][c];
     F[c] = 0.5 * (FL[c] + FR[c]) - 0.5 * d;
   }
   return 0;
 }
 
-int riemann(int solver, const double WL[7], const double WR[7], double Bn, double gam, double F[7]) {
+int riemann(int solver, const double WL[7], const double WR[7], double Bn, double gam, double F[7], double etah = 0.0) {
   if (solver == 0) { hlle(WL, WR, Bn, gam, F); return 0; }
   if (solver == 1) { hlld(WL, WR, Bn, gam, F); return 0; }
-  return roe(WL, WR, Bn, gam, F);
+  return roe(WL, WR, Bn, gam, F, etah);
+}
+// reading R19: eta of a face = half the largest jump of the two fast characteristic speeds v_n -+ c_f between its L and R states
+double eta_face(const double WL[7], const double WR[7], double Bn, double gam) {
+  double cl = fastspeed(WL, Bn, gam), cr = fastspeed(WR, Bn, gam);
+  return 0.5 * std::max(std::fabs((WR[1] + cr) - (WL[1] + cl)), std::fabs((WR[1] - cr) - (WL[1] - cl)));
 }
 
 // ---------------------------------------------------------------------------------
@@ -400,6 +408,12 @@ struct Group {
   Arr E[3];                 // edge EMF: E[0]=Ex at (i, j-1/2, k-1/2) etc.
   Arr Uh[5], bh[3], Wh[8];  // half-step data
   Arr Wlo[3][7], Wup[3][7]; // CTU: states at the lower / upper d-face of every cell (generic order)
+  // H-correction (R19), in the pass whose fluxes update the solution (VL step 5, CTU step 6); the predictor pass keeps the plain
+  // solver.  The pass over the faces runs twice, first recording eta of every face it visits, then solving with
+  // eta^H = the largest eta among the face itself and the eight transverse faces of its two cells that were visited
+  int hphase = 0;           // 0: no H-correction; 1: record eta; 2: solve with eta^H
+  Arr eta[3];
+  std::vector<char> etaok[3];
 
   Group(const mhdref_config& cfg, double dt_, double dh_, Stats* s) : c(cfg), gam(cfg.gamma), dt(dt_), dh(dh_), st(s) {
     t.N = cfg.ps2; t.g = cfg.nghost; t.T = t.N + 2 * t.g; t.S = t.T + 1; t.n3 = (size_t)t.S * t.S * t.S;
@@ -408,6 +422,25 @@ struct Group {
     for (auto& fd : F) for (auto& a : fd) mk(a);
     for (auto& a : E) mk(a); for (auto& a : Uh) mk(a); for (auto& a : bh) mk(a); for (auto& a : Wh) mk(a);
     if (cfg.scheme == 1) { for (auto& wd : Wlo) for (auto& a : wd) mk(a); for (auto& wd : Wup) for (auto& a : wd) mk(a); }
+    if (cfg.hcorr) for (int d = 0; d < 3; ++d) { mk(eta[d]); etaok[d].assign(t.n3, 0); }
+  }
+  double etaH(int d, size_t q) const {
+    int t1, t2; cyc(d, t1, t2);
+    double e = eta[d][q];
+    const int tt[2] = { t1, t2 };
+    for (int s = 0; s < 2; ++s) {
+      const int tdir = tt[s];
+      const size_t ql = q - off(d), x[4] = { ql, ql + (size_t)off(tdir), q, q + (size_t)off(tdir) };   // lower / upper t-faces of the two cells
+      for (int n = 0; n < 4; ++n) if (etaok[tdir][x[n]]) e = std::max(e, eta[tdir][x[n]]);
+    }
+    return e;
+  }
+  template <class Fn> void face_pass(Fn&& loops) {
+    if (!c.hcorr) { loops(); return; }
+    for (int d = 0; d < 3; ++d) { eta[d].assign(t.n3, NaN); etaok[d].assign(t.n3, 0); }
+    hphase = 1; loops();
+    hphase = 2; loops();
+    hphase = 0;
   }
   inline int off(int d) const { return d == 0 ? 1 : (d == 1 ? t.S : t.S * t.S); }
   static inline void stage(int n) { if (mhdref_stage_hook) mhdref_stage_hook(n); }
@@ -445,8 +478,9 @@ struct Group {
     w[4] = Wc[4][q]; w[5] = Wc[5 + t1][q]; w[6] = Wc[5 + t2][q];
   }
   void floors(double w[7]) {
-    if (w[0] < c.min_dens) { w[0] = c.min_dens; if (st) st->fd++; }
-    if (w[4] < c.min_pres) { w[4] = c.min_pres; if (st) st->fp++; }
+    const bool count = st && hphase != 1;           // the eta-recording sweep of a pass repeats the states of the solving sweep
+    if (w[0] < c.min_dens) { w[0] = c.min_dens; if (count) st->fd++; }
+    if (w[4] < c.min_pres) { w[4] = c.min_pres; if (count) st->fp++; }
   }
 
   // reading R10: edge EMFs from the face fluxes F, cell-centred reference field from Wc (v, Bc).
@@ -511,11 +545,13 @@ struct Group {
       for (int v = 0; v < 5; ++v) Uo[v][q] = U[v][q] - qh * dU[v];
     }
   }
-  void solve_face(int d, size_t q, const double wl[7], const double wr[7], double bn) {
+  void solve_face(int d, size_t q, const double wl[7], const double wr[7], double bn, Arr (*Fout)[7] = nullptr) {
+    if (hphase == 1) { eta[d][q] = eta_face(wl, wr, bn, gam); etaok[d][q] = 1; return; }
     double f[7];
-    int fb = riemann(c.riemann, wl, wr, bn, gam, f);
+    int fb = hphase == 2 ? riemann(c.riemann, wl, wr, bn, gam, f, etaH(d, q)) : riemann(c.riemann, wl, wr, bn, gam, f);
     if (fb && st) st->fb++;
-    for (int v = 0; v < 7; ++v) F[d][v][q] = f[v];
+    Arr (*Fo)[7] = Fout ? Fout : F;
+    for (int v = 0; v < 7; ++v) Fo[d][v][q] = f[v];
   }
 
   // the slope limiter selected by the configuration (R5: MC; NEXT-4 variants: minmod, van Leer)
@@ -566,11 +602,11 @@ struct Group {
   // ------------------------------------------------------------------------------
   void advance_vl() {
     int T = t.T;
-    const bool mn = c.minimal_ranges != 0;
+    const bool mn = c.minimal_ranges != 0 && !c.hcorr;
     const int g = t.g, N = t.N;
     con2prim(U, b, W, 0, T);                                           // time-n primitives
     stage(1);
-    // step 1: first-order fluxes, longitudinal B = face value
+    // step 1: first-order fluxes, longitudinal B = face value; R19: the predictor pass uses the plain solver
     for (int d = 0; d < 3; ++d) {
       int lo[3] = { 0, 0, 0 }; lo[d] = 1;
       for (int k = lo[2]; k < T; ++k) for (int j = lo[1]; j < T; ++j) for (int i = lo[0]; i < T; ++i) {
@@ -594,6 +630,7 @@ struct Group {
     const int r = c.recon == 0 ? 3 : 4;
     // minimal: the faces of the interior cells and of their transverse neighbours (the edge EMFs of the interior faces need those)
     const int tlo = mn ? g - 1 : 1, thi = mn ? g + N + 1 : T - 1, nlo = mn ? g : r, nhi = mn ? g + N : T - r;
+    face_pass([&]() {
     for (int d = 0; d < 3; ++d) {
       int t1, t2; cyc(d, t1, t2);
       int idx[3];
@@ -614,6 +651,7 @@ struct Group {
         solve_face(d, q, wl, wr, bh[d][q]);
       }
     }
+    });
     stage(5);
     if (mn) edge_emf(Wh, g, g + N, g, g + N); else edge_emf(Wh, r, T - r, 1, T - 1);   // step 6
     stage(6);
@@ -626,7 +664,7 @@ struct Group {
     int T = t.T;
     int r = c.recon == 0 ? 1 : 2;
     double sig = dt / dh, hdt = 0.5 * dt;
-    const bool mn = c.minimal_ranges != 0;
+    const bool mn = c.minimal_ranges != 0 && !c.hcorr;
     // minimal: everything is derived from the cells whose half-step state the second pass needs, [lo, hi)^3 = interior + 1
     const int lo_ = t.g - 1, hi_ = t.g + t.N + 1;
     con2prim(U, b, W, 0, T);
@@ -666,7 +704,7 @@ struct Group {
         for (int v = 0; v < 7; ++v) { Wlo[d][v][q] = wlo[v]; Wup[d][v][q] = wup[v]; }
       }
     }
-    // step 2: F1 = Riemann(Wup(i-1), Wlo(i), b_n(face) at t^n)
+    // step 2: F1 = Riemann(Wup(i-1), Wlo(i), b_n(face) at t^n); R19: the predictor pass uses the plain solver
     for (int d = 0; d < 3; ++d) {
       int lo[3] = { 0, 0, 0 }, hi[3] = { T, T, T }; lo[d] = r + 1; hi[d] = T - r;
       if (mn) { for (int a = 0; a < 3; ++a) { lo[a] = lo_ - 1; hi[a] = hi_ + 1; } lo[d] = lo_; }   // faces n in [lo, hi], t in [lo-1, hi]
@@ -740,6 +778,7 @@ struct Group {
     {
       Arr F2[3][7];
       for (int d = 0; d < 3; ++d) for (int v = 0; v < 7; ++v) F2[d][v].assign(t.n3, NaN);
+      face_pass([&]() {
       for (int d = 0; d < 3; ++d) {
         int t1, t2; cyc(d, t1, t2);
         int lo[3], hi[3];
@@ -747,13 +786,12 @@ struct Group {
         if (mn) { lo[d] = t.g; hi[d] = t.g + t.N + 1; }
         for (int k = lo[2]; k < hi[2]; ++k) for (int j = lo[1]; j < hi[1]; ++j) for (int i = lo[0]; i < hi[0]; ++i) {
           size_t q = t.id(i, j, k), ql = q - off(d);
-          double wl[7], wr[7], f[7];
+          double wl[7], wr[7];
           for (int v = 0; v < 7; ++v) { wl[v] = Wup[d][v][ql]; wr[v] = Wlo[d][v][q]; }
-          int fb = riemann(c.riemann, wl, wr, bh[d][q], gam, f);
-          if (fb && st) st->fb++;
-          for (int v = 0; v < 7; ++v) F2[d][v][q] = f[v];
+          solve_face(d, q, wl, wr, bh[d][q], F2);
         }
       }
+      });
       for (int d = 0; d < 3; ++d) for (int v = 0; v < 7; ++v) F[d][v].swap(F2[d][v]);
     }
     stage(5);
@@ -811,6 +849,8 @@ int check_cfg(const mhdref_config* c) {
   if (!c) return -1;
   if (c->ps2 < 2 || c->scheme < 0 || c->scheme > 1 || c->recon < 0 || c->recon > 1 || c->riemann < 0 || c->riemann > 2 || c->limvar < 0 || c->limvar > 1 || c->limiter < 0 || c->limiter > 2) return -1;
   int need = c->recon == 1 ? 4 : 3;                        // reading R8
+  if (c->hcorr < 0 || c->hcorr > 1 || (c->hcorr && c->riemann != 2)) return -1;
+  if (c->hcorr) need += 1;                                 // reading R19: eta of the transverse faces one cell further out
   if (c->nghost < need) return -1;
   if (!(c->gamma > 1.0)) return -1;
   if (!(c->emf_tie >= 0.0)) return -1;
@@ -875,6 +915,9 @@ int mhdref_dt(const mhdref_config* cfg, const double* U, const double* B, int ng
 
 // ---- unit entry points for the pins (tests only) ----
 int mhdref_riemann(int solver, const double* WL, const double* WR, double Bn, double gamma, double* F) { return riemann(solver, WL, WR, Bn, gamma, F); }
+// Roe flux with every dissipation speed raised to at least etah (R19), and the eta of a face
+int mhdref_roe_eta(const double* WL, const double* WR, double Bn, double gamma, double etah, double* F) { return roe(WL, WR, Bn, gamma, F, etah); }
+double mhdref_eta_face(const double* WL, const double* WR, double Bn, double gamma) { return eta_face(WL, WR, Bn, gamma); }
 void mhdref_prim2cons(const double* W, double Bn, double gamma, double* U) { prim2cons(W, Bn, gamma, U); }
 void mhdref_physflux(const double* W, double Bn, double gamma, double* F) { double U[7]; prim2cons(W, Bn, gamma, U); physflux(W, Bn, U, F); }
 double mhdref_fastspeed(const double* W, double Bn, double gamma) { return fastspeed(W, Bn, gamma); }

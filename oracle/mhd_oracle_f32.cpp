@@ -52,13 +52,13 @@ template <> struct numeric_limits<F32> { static F32 quiet_NaN() { return F32(num
 // plain-C entry points (float arrays, double scalars) so that the binding does not depend on how F32 is passed by value
 extern "C" {
 typedef struct {
-  int ps2, nghost; double gamma; int scheme, recon, riemann, limvar; double min_dens, min_pres, emf_tie; int limiter, minimal_ranges;
+  int ps2, nghost; double gamma; int scheme, recon, riemann, limvar; double min_dens, min_pres, emf_tie; int limiter, minimal_ranges, hcorr;
 } mhdref32_config;
 
 static mhdref_config to_f32_cfg(const mhdref32_config* c) {
   mhdref_config k;
   k.ps2 = c->ps2; k.nghost = c->nghost; k.gamma = F32(c->gamma); k.scheme = c->scheme; k.recon = c->recon; k.riemann = c->riemann;
-  k.limvar = c->limvar; k.min_dens = F32(c->min_dens); k.min_pres = F32(c->min_pres); k.emf_tie = F32(c->emf_tie); k.limiter = c->limiter; k.minimal_ranges = c->minimal_ranges;
+  k.limvar = c->limvar; k.min_dens = F32(c->min_dens); k.min_pres = F32(c->min_pres); k.emf_tie = F32(c->emf_tie); k.limiter = c->limiter; k.minimal_ranges = c->minimal_ranges; k.hcorr = c->hcorr;
   return k;
 }
 int mhdref32_advance(const mhdref32_config* cfg, const float* U_in, const float* B_in, float* U_out, float* B_out, float* flux_out,

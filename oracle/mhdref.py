@@ -29,7 +29,7 @@ class Config(C.Structure):
     _fields_ = [("ps2", C.c_int), ("nghost", C.c_int), ("gamma", C.c_double), ("scheme", C.c_int),
                 ("recon", C.c_int), ("riemann", C.c_int), ("limvar", C.c_int),
                 ("min_dens", C.c_double), ("min_pres", C.c_double), ("emf_tie", C.c_double), ("limiter", C.c_int),
-                ("minimal_ranges", C.c_int)]
+                ("minimal_ranges", C.c_int), ("hcorr", C.c_int)]
 
 
 def build(force: bool = False) -> str:
@@ -70,6 +70,9 @@ def lib():
         _lib.mhdref_mc.restype = C.c_double
         _lib.mhdref_limiter.argtypes = [C.c_int, C.c_double, C.c_double]
         _lib.mhdref_limiter.restype = C.c_double
+        _lib.mhdref_roe_eta.argtypes = [dp, dp, C.c_double, C.c_double, C.c_double, dp]
+        _lib.mhdref_eta_face.argtypes = [dp, dp, C.c_double, C.c_double]
+        _lib.mhdref_eta_face.restype = C.c_double
         _lib.mhdref_emf_up.argtypes = [C.c_double] * 6
         _lib.mhdref_emf_up.restype = C.c_double
         _lib.mhdref_edge_emf.argtypes = [dp, dp, dp, dp, C.c_double]
@@ -101,11 +104,11 @@ def _c(a):
 
 
 def make_config(N=16, g=3, gamma=5.0 / 3.0, scheme=VL, recon=PLM, riemann=HLLD, limvar=None,
-                min_dens=1e-10, min_pres=1e-10, emf_tie=1e-12, limiter=MC, minimal_ranges=0) -> Config:
+                min_dens=1e-10, min_pres=1e-10, emf_tie=1e-12, limiter=MC, minimal_ranges=0, hcorr=0) -> Config:
     """emf_tie: reading R10a; 1e-12 is the FP64 value, the FP32 path is checked against the oracle run with 1e-5."""
     if limvar is None:
         limvar = LIM_PRIM if scheme == VL else LIM_CHAR
-    return Config(N, g, gamma, scheme, recon, riemann, limvar, min_dens, min_pres, emf_tie, limiter, minimal_ranges)
+    return Config(N, g, gamma, scheme, recon, riemann, limvar, min_dens, min_pres, emf_tie, limiter, minimal_ranges, hcorr)
 
 
 def advance(cfg: Config, U_in, B_in, dt, dh, want_planes=True, force_ghost_ok=False):
@@ -198,6 +201,17 @@ def eig_roe(WL, WR, Bn, gamma=5.0 / 3.0):
     lam = np.empty(7); R = np.empty((7, 7)); L = np.empty((7, 7)); avg = np.empty(9)
     rc = lib().mhdref_eig_roe(_p(WL), _p(WR), float(Bn), float(gamma), _p(lam), _p(R), _p(L), _p(avg))
     return rc, lam, R, L, avg
+
+
+def roe_eta(WL, WR, Bn, etah, gamma=5.0 / 3.0):
+    """Roe flux with every dissipation speed raised to at least etah (reading R19); returns (F, fell back to HLLE)"""
+    WL = _c(WL); WR = _c(WR); F = np.empty(7)
+    fb = lib().mhdref_roe_eta(_p(WL), _p(WR), float(Bn), float(gamma), float(etah), _p(F))
+    return F, fb
+
+
+def eta_face(WL, WR, Bn, gamma=5.0 / 3.0):
+    return lib().mhdref_eta_face(_p(_c(WL)), _p(_c(WR)), float(Bn), float(gamma))
 
 
 def emf_up(m, rm, rp, qm, qp, tie):

@@ -14,7 +14,7 @@ int main() {
       const int N = 8, g = recon ? 4 : 3, T = N + 2 * g, G = 2;
       mhdref_config cfg; cfg.ps2 = N; cfg.nghost = g; cfg.gamma = gam; cfg.scheme = scheme; cfg.recon = recon; cfg.riemann = riemann;
       cfg.limvar = limvar; cfg.min_dens = 1e-10; cfg.min_pres = 1e-10; cfg.emf_tie = (riemann == 1 ? 1e-5 : 1e-12); cfg.limiter = (riemann + recon) % 3;
-      cfg.minimal_ranges = mn;
+      cfg.minimal_ranges = mn; cfg.hcorr = 0;
       const size_t T3 = (size_t)T * T * T, nf = (size_t)T * T * (T + 1);
       std::vector<double> U(G * 5 * T3), B(G * 3 * nf), Uo(G * 5 * N * N * N), Bo(G * 3 * N * N * (N + 1)), fo(G * 9 * 5 * N * N), eo(G * 9 * 2 * (N + 1) * N);
       const double k = 2.0 * 3.14159265358979323846 / N;
