@@ -323,8 +323,10 @@ int roe(const double WL[7], const double WR[7], double Bn, double gam, double F[
   if (!(r.a2 > 0.0)) { hlle(WL, WR, Bn, gam, F); return 1; }
   double lam[7], R[7][7], L[7][7], a[7], dU[7];
   eig_cons(r, Bn, gam, lam, R, L);
-  if (lam[0] >= 0.0) { for (int c = 0; c < 7; ++c) F[c] = FL[c]; return 0; }
-  if (lam[6] <= 0.0) { for (int c = 0; c < 7; ++c) F[c] = FR[c]; return 0; }
+  // supersonic shortcuts; with the H-correction only where every wave is faster than etah, so that the flux stays a continuous
+  // function of the states (for lam_min >= etah the dissipation formula below gives F_L exactly, as it does for plain Roe at lam_min >= 0)
+  if (lam[0] >= etah) { for (int c = 0; c < 7; ++c) F[c] = FL[c]; return 0; }
+  if (lam[6] <= -etah) { for (int c = 0; c < 7; ++c) F[c] = FR[c]; return 0; }
   for (int c = 0; c < 7; ++c) dU[c] = UR[c] - UL[c];
   for (int k = 0; k < 7; ++k) { a[k] = 0.0; for (int c = 0; c < 7; ++c) a[k] += L[k][c] * dU[c]; }
   // intermediate states U_L + sum_{k<=m} a_k R_k, m = 0..5, tested only where lam_{m+1} > lam_m

@@ -221,7 +221,12 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
     if (!fusedv) LAUNCH(ST_FLUX1, SOLVER_SWITCH(sol, (k_flux1_vl<R, SOLVER, SC><<<GRID3(bf1), blk, 0, st>>>(p, bf1))));          // step 1
     LAUNCH(ST_EMF1, (k_emf<R, A_F, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 2
     LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh, 1)));                                         // step 3
-    if (s->cfg.recon == MHD_PLM) {
+    if (s->cfg.recon == MHD_PLM && s->cfg.hcorr) {
+      // R19: eta of the pass-2 faces and of the transverse faces around them (one face further along the normal), then Roe with eta^H
+      const Box3x3 bet = dir_boxes(g - 1, g + N + 2, g - 1, g + N + 1);
+      LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_eta2_vl<R, LIM, SC><<<GRID3(bet), blk, 0, st>>>(p, bet))));
+      LIM_SWITCH(lim, LAUNCH(ST_FLUX2, (k_flux2_vl<R, kROE, LIM, SC, true><<<GRID3(bf2), blk, 0, st>>>(p, bf2))));
+    } else if (s->cfg.recon == MHD_PLM) {
       LIM_SWITCH(lim, LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_vl<R, SOLVER, LIM, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2)))));   // steps 4+5
     } else {
       // VL + PPM (NEXT-4): limited slopes of the half-step primitives (parked in the dead pass-1 flux arrays), the
@@ -382,7 +387,12 @@ int check_config(const mhd_config* c) {
   if (c->limvar != MHD_LIM_PRIM && c->limvar != MHD_LIM_CHAR) return MHD_EINVAL;
   if (c->prec != MHD_FP32 && c->prec != MHD_FP64) return MHD_EINVAL;
   if (c->limiter < MHD_LIMITER_MC || c->limiter > MHD_LIMITER_VANLEER) return MHD_EINVAL;
-  const int need = c->recon == MHD_PPM ? 4 : 3;     // DESIGN.md R8
+  int need = c->recon == MHD_PPM ? 4 : 3;           // DESIGN.md R8
+  if (c->hcorr != 0 && c->hcorr != 1) return MHD_EINVAL;
+  if (c->hcorr) {                                   // DESIGN.md R19: Roe only, one more ghost cell; device path for VL + PLM
+    if (c->riemann != MHD_ROE || c->scheme != MHD_VL || c->recon != MHD_PLM) return MHD_EINVAL;
+    need += 1;
+  }
   if (c->nghost < need || c->nghost > 8) return MHD_EINVAL;
   if (!(c->gamma > 1.0) || !std::isfinite(c->gamma)) return MHD_EINVAL;
   if (!(c->min_dens >= 0.0) || !(c->min_pres >= 0.0)) return MHD_EINVAL;

@@ -90,7 +90,8 @@ __device__ __forceinline__ void riemann_hlle(const R (&wl)[7], const R (&wr)[7],
 // Roe: F = 1/2 (F_L + F_R) - 1/2 sum_k |lambda_k| (L_k . dU) R_k on the conserved eigen-system of the Roe average;
 // HLLE where a~^2 <= 0 or an intermediate state has rho <= 0 or P <= 0.  Returns true if it fell back.
 template <class R>
-__device__ __forceinline__ bool riemann_roe(const R (&wl)[7], const R (&wr)[7], R bn, R gam, R gm1inv, R (&F)[7]) {
+// etah (R19, H-correction): every wave speed of the dissipation term is max(|lam_k|, etah); 0: the plain solver
+__device__ __forceinline__ bool riemann_roe(const R (&wl)[7], const R (&wr)[7], R bn, R gam, R gm1inv, R (&F)[7], R etah = R(0)) {
   const R bn2 = bn * bn;
   Side<R> L, Rr;
   side_setup(wl, bn, bn2, gm1inv, gam, L);
@@ -157,7 +158,7 @@ __device__ __forceinline__ bool riemann_roe(const R (&wl)[7], const R (&wr)[7], 
     R ak = R(0);
 #pragma unroll
     for (int c = 0; c < 7; ++c) ak += Lk[c] * dU[c];
-    const R wk = Num<R>::abs(lam[k]) * ak;
+    const R wk = Num<R>::max(Num<R>::abs(lam[k]), etah) * ak;
 #pragma unroll
     for (int c = 0; c < 7; ++c) { diss[c] += wk * Rk[c]; Ui[c] += ak * Rk[c]; }
     if (k < 6) {
@@ -170,7 +171,7 @@ __device__ __forceinline__ bool riemann_roe(const R (&wl)[7], const R (&wr)[7], 
   }
   R Fh[7];
   hlle_flux(wl, wr, L, Rr, a2ok, r.vn, w.cf, Fh);
-  const bool superL = lam[0] >= R(0), superR = lam[6] <= R(0);
+  const bool superL = lam[0] >= etah, superR = lam[6] <= -etah;     // R19: the shortcuts only where every wave is faster than etah
   const bool fallback = !a2ok || (!superL && !superR && bad);
 #pragma unroll
   for (int c = 0; c < 7; ++c) {
@@ -181,10 +182,17 @@ __device__ __forceinline__ bool riemann_roe(const R (&wl)[7], const R (&wr)[7], 
 }
 
 template <class R, int SOLVER>
-__device__ __forceinline__ bool riemann(const R (&wl)[7], const R (&wr)[7], R bn, R gam, R gm1inv, R (&F)[7]) {
+__device__ __forceinline__ bool riemann(const R (&wl)[7], const R (&wr)[7], R bn, R gam, R gm1inv, R (&F)[7], R etah = R(0)) {
   if (SOLVER == kHLLE) { riemann_hlle(wl, wr, bn, gam, gm1inv, F); return false; }
   else if (SOLVER == kHLLD) { riemann_hlld(wl, wr, bn, gam, gm1inv, F); return false; }
-  else return riemann_roe(wl, wr, bn, gam, gm1inv, F);
+  else return riemann_roe(wl, wr, bn, gam, gm1inv, F, etah);
+}
+// R19: eta of a face = half the largest jump of the fast characteristic speeds v_n -+ c_f between its L and R states
+template <class R>
+__device__ __forceinline__ R eta_face(const R (&wl)[7], const R (&wr)[7], R bn, R gam) {
+  const R bn2 = bn * bn;
+  const R cl = fast_speed(wl[0], wl[4], bn2, wl[5] * wl[5] + wl[6] * wl[6], gam), cr = fast_speed(wr[0], wr[4], bn2, wr[5] * wr[5] + wr[6] * wr[6], gam);
+  return R(0.5) * Num<R>::max(Num<R>::abs((wr[1] + cr) - (wl[1] + cl)), Num<R>::abs((wr[1] - cr) - (wl[1] - cl)));
 }
 
 }  // namespace mhd

@@ -25,6 +25,7 @@ enum : int {
   A_E = 32,     // 3
   A_BH = 35,    // 3: face field at t^{n+1/2}
   A_WH = 38,    // 8: half-step primitives
+  A_ETA = 1,    // 3: H-correction (R19): eta of the pass-2 faces of VL, in the arrays of the time-n velocities (dead after the half step)
   A_EC = 46,    // 3: cell-centred reference EMF
   A_VL_END = 49,
   A_LO = 49,    // 21: CTU state at the lower d-face of each cell, [d][v]
@@ -100,10 +101,10 @@ __device__ __forceinline__ void load_gen(const R* Wb, int S3, int q, R (&w)[7]) 
   w[5] = Wb[(size_t)(5 + T1) * S3 + q]; w[6] = Wb[(size_t)(5 + T2) * S3 + q];
 }
 
-template <class R, class KP>
+template <bool COUNT = true, class R, class KP>
 __device__ __forceinline__ void apply_floors(const KP& p, R (&w)[7]) {
-  if (w[0] < p.min_dens) { w[0] = p.min_dens; count_event(p.stats + 0); }
-  if (w[4] < p.min_pres) { w[4] = p.min_pres; count_event(p.stats + 1); }
+  if (w[0] < p.min_dens) { w[0] = p.min_dens; if (COUNT) count_event(p.stats + 0); }
+  if (w[4] < p.min_pres) { w[4] = p.min_pres; if (COUNT) count_event(p.stats + 1); }
 }
 
 // conserved cell data + the six face fields of the cell -> primitives (Eq. 5; floors R9)

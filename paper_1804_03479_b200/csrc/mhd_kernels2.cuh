@@ -5,10 +5,9 @@
 namespace mhd {
 
 // ---- VL steps 4+5: PLM at the half step + Riemann solve, normal B = half-step face value --------
-template <class R, int SOLVER, int LIMVAR, int D, class KP>
-__device__ __forceinline__ void flux2_vl_dir(const KP& p, const Box3& box) {
-  Ctx<R, KP> c(p, box);
-  if (!c.ok) return;
+// PLM states of a D face from the half-step primitives (shared by the flux kernel and the eta kernel of the H-correction)
+template <class R, int LIMVAR, int D, bool COUNT, class KP>
+__device__ __forceinline__ void plm_states_vl(const Ctx<R, KP>& c, const KP& p, R (&wl)[7], R (&wr)[7]) {
   const int o = c.off(D), q = c.q;
   const R* Wh = c.arr(A_WH);
   R wmm[7], wm[7], w0[7], wp[7], sl[7], sr[7];
@@ -18,21 +17,55 @@ __device__ __forceinline__ void flux2_vl_dir(const KP& p, const Box3& box) {
   load_gen<R, D>(Wh, p.S3, q + o, wp);
   slope3<R, LIMVAR>(wmm, wm, w0, Wh[(size_t)(5 + D) * p.S3 + q - o], p.gam, sl);
   slope3<R, LIMVAR>(wm, w0, wp, Wh[(size_t)(5 + D) * p.S3 + q], p.gam, sr);
-  R wl[7], wr[7], F[7];
 #pragma unroll
   for (int v = 0; v < 7; ++v) { wl[v] = wm[v] + R(0.5) * sl[v]; wr[v] = w0[v] - R(0.5) * sr[v]; }
-  apply_floors(p, wl); apply_floors(p, wr);
-  const bool fb = riemann<R, SOLVER>(wl, wr, c.arr(A_BH + D)[q], p.gam, p.gm1inv, F);
+  apply_floors<COUNT>(p, wl); apply_floors<COUNT>(p, wr);
+}
+template <class R, int SOLVER, int LIMVAR, int D, bool HC, class KP>
+__device__ __forceinline__ void flux2_vl_dir(const KP& p, const Box3& box) {
+  constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
+  Ctx<R, KP> c(p, box);
+  if (!c.ok) return;
+  const int o = c.off(D), q = c.q;
+  R wl[7], wr[7], F[7];
+  plm_states_vl<R, LIMVAR, D, true>(c, p, wl, wr);
+  R etah = R(0);
+  if (HC) {
+    // eta^H: this face and the lower / upper T1 and T2 faces of its two cells (k_eta2_vl wrote them on a box one face wider)
+    etah = c.arr(A_ETA + D)[q];
+    const R* e1 = c.arr(A_ETA + T1); const R* e2 = c.arr(A_ETA + T2);
+    const int o1 = c.off(T1), o2 = c.off(T2), ql = q - o;
+    etah = Num<R>::max(etah, Num<R>::max(Num<R>::max(e1[ql], e1[ql + o1]), Num<R>::max(e1[q], e1[q + o1])));
+    etah = Num<R>::max(etah, Num<R>::max(Num<R>::max(e2[ql], e2[ql + o2]), Num<R>::max(e2[q], e2[q + o2])));
+  }
+  const bool fb = riemann<R, SOLVER>(wl, wr, c.arr(A_BH + D)[q], p.gam, p.gm1inv, F, etah);
   if (fb) count_event(p.stats + 2);
 #pragma unroll
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[q] = F[v];
 }
-template <class R, int SOLVER, int LIMVAR, int SC>
+template <class R, int SOLVER, int LIMVAR, int SC, bool HC = false>
 __global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux2_vl(const KParamsSC<R, SC> p, const Box3x3 bx) {
   switch (blockIdx.y) {
-    case 0: flux2_vl_dir<R, SOLVER, LIMVAR, 0>(p, bx.b[0]); break;
-    case 1: flux2_vl_dir<R, SOLVER, LIMVAR, 1>(p, bx.b[1]); break;
-    default: flux2_vl_dir<R, SOLVER, LIMVAR, 2>(p, bx.b[2]); break;
+    case 0: flux2_vl_dir<R, SOLVER, LIMVAR, 0, HC>(p, bx.b[0]); break;
+    case 1: flux2_vl_dir<R, SOLVER, LIMVAR, 1, HC>(p, bx.b[1]); break;
+    default: flux2_vl_dir<R, SOLVER, LIMVAR, 2, HC>(p, bx.b[2]); break;
+  }
+}
+// H-correction (R19): eta of every pass-2 face and of the transverse faces around them (the same PLM states, floors not counted twice)
+template <class R, int LIMVAR, int D, class KP>
+__device__ __forceinline__ void eta2_vl_dir(const KP& p, const Box3& box) {
+  Ctx<R, KP> c(p, box);
+  if (!c.ok) return;
+  R wl[7], wr[7];
+  plm_states_vl<R, LIMVAR, D, false>(c, p, wl, wr);
+  c.arr(A_ETA + D)[c.q] = eta_face(wl, wr, c.arr(A_BH + D)[c.q], p.gam);
+}
+template <class R, int LIMVAR, int SC>
+__global__ void __launch_bounds__(256, Occ<R>::minb) k_eta2_vl(const KParamsSC<R, SC> p, const Box3x3 bx) {
+  switch (blockIdx.y) {
+    case 0: eta2_vl_dir<R, LIMVAR, 0>(p, bx.b[0]); break;
+    case 1: eta2_vl_dir<R, LIMVAR, 1>(p, bx.b[1]); break;
+    default: eta2_vl_dir<R, LIMVAR, 2>(p, bx.b[2]); break;
   }
 }
 

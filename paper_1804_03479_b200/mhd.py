@@ -29,7 +29,7 @@ EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance
 class Config(C.Structure):
     _fields_ = [("ps2", C.c_int), ("nghost", C.c_int), ("gamma", C.c_double), ("scheme", C.c_int),
                 ("recon", C.c_int), ("riemann", C.c_int), ("limvar", C.c_int), ("prec", C.c_int),
-                ("min_dens", C.c_double), ("min_pres", C.c_double), ("emf_tie", C.c_double), ("max_groups", C.c_int), ("device", C.c_int), ("limiter", C.c_int)]
+                ("min_dens", C.c_double), ("min_pres", C.c_double), ("emf_tie", C.c_double), ("max_groups", C.c_int), ("device", C.c_int), ("limiter", C.c_int), ("hcorr", C.c_int)]
 
 
 class MHDError(RuntimeError):
@@ -145,10 +145,10 @@ def _stream_ptr(stream):
 
 
 def make_config(N=16, g=3, gamma=5.0 / 3.0, scheme=VL, recon=PLM, riemann=HLLD, limvar=None, prec=FP64,
-                min_dens=1e-10, min_pres=1e-10, emf_tie=0.0, max_groups=512, device=0, limiter=0) -> Config:
+                min_dens=1e-10, min_pres=1e-10, emf_tie=0.0, max_groups=512, device=0, limiter=0, hcorr=0) -> Config:
     if limvar is None:
         limvar = LIM_PRIM if scheme == VL else LIM_CHAR
-    return Config(N, g, gamma, scheme, recon, riemann, limvar, prec, min_dens, min_pres, emf_tie, max_groups, device, limiter)
+    return Config(N, g, gamma, scheme, recon, riemann, limvar, prec, min_dens, min_pres, emf_tie, max_groups, device, limiter, hcorr)
 
 
 class Solver:

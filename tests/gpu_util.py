@@ -11,13 +11,13 @@ def np_dtype(prec):
 class GpuRunner:
     """advance_fn-compatible wrapper (see tests/harness.py) around paper_1804_03479_b200.mhd.Solver."""
 
-    def __init__(self, N=16, g=3, scheme=0, recon=0, riemann=1, limvar=None, prec=1, max_groups=512, planes=True, limiter=0):
+    def __init__(self, N=16, g=3, scheme=0, recon=0, riemann=1, limvar=None, prec=1, max_groups=512, planes=True, limiter=0, hcorr=0, gamma=5.0 / 3.0):
         import torch
         from paper_1804_03479_b200 import mhd
         self.torch = torch
         self.mhd = mhd
         self.cfg = mhd.make_config(N=N, g=g, scheme=scheme, recon=recon, riemann=riemann, limvar=limvar, prec=prec,
-                                   max_groups=max_groups, limiter=limiter)
+                                   max_groups=max_groups, limiter=limiter, hcorr=hcorr, gamma=gamma)
         self.solver = mhd.Solver(self.cfg)
         self.planes = planes
         self.dtype = np_dtype(prec)

@@ -103,3 +103,73 @@ def test_shock_tubes_ctu_ppm_roe(oracle, name, prec):
         errs[nm] = float(np.abs(Pd[v] - Pr[v]).max() / den)
     assert not bad_fields(errs, TOL[prec]), errs
     assert np.array_equal(dev[1], np.full_like(dev[1], dtp(inputs.RIEMANN_PROBLEMS[name]["Bn"])))      # B_n untouched
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Roe solver with H-correction (R19): device path for VL + PLM (the combination of the paper's Fig. 18)
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("limvar", [0, 1])
+@pytest.mark.parametrize("prec", [1, 0])
+def test_h_correction_one_step_and_ten_steps(oracle, limvar, prec):
+    N, G, g = 16, 5, 4
+    dtp = GU.np_dtype(prec)
+    U_in, B_in, dh = inputs.config2_batch(G, N=N, g=g, dtype=dtp)
+    U64, B64 = U_in.astype(np.float64), B_in.astype(np.float64)
+    cfg = oracle.make_config(N=N, g=g, scheme=0, recon=0, riemann=2, limvar=limvar, emf_tie=EMF_TIE[prec], hcorr=1)
+    dt, _ = oracle.dt_reduce(cfg, U64, B64, g, dh, 0.3)
+    ref = oracle.advance(cfg, U64, B64, dt, dh)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=0, recon=0, riemann=2, limvar=limvar, prec=prec, max_groups=8, hcorr=1)
+    out = gpu(U_in, B_in, dt, dh)
+    errs = GU.field_errors(out, ref, N)
+    assert not bad_fields(errs, TOL_ONE_STEP[prec]), errs
+    # and it is the H-correction that was compared: the plain Roe solver differs on this transonic state
+    plain = oracle.advance(oracle.make_config(N=N, g=g, scheme=0, recon=0, riemann=2, limvar=limvar, emf_tie=EMF_TIE[prec]), U64, B64, dt, dh)
+    assert np.abs(plain["U"] - ref["U"]).max() > 1e-6
+    assert all(a <= b for a, b in zip(gpu.stats(), ref["stats"]))
+    # ten steps on a periodic 32^3 grid: shared faces bitwise, div B, parity
+    n = 32
+    U, bx, by, bz, dh = inputs.random_group_grid(n, 77)
+    adv = lambda Ui, Bi, dt_, dh_: oracle.advance(cfg, Ui, Bi, dt_, dh_)
+    r = [a.astype(dtp).astype(np.float64) for a in (U, bx, by, bz)]
+    d = [a.astype(dtp) for a in (U, bx, by, bz)]
+    for _ in range(10):
+        Ui, Bi = inputs.pack_groups(*r, n, 0)
+        dt, _ = oracle.dt_reduce(oracle.make_config(N=n, g=3), Ui, Bi, 0, dh, 0.3)
+        r = list(H.step_grid(adv, *r, dt, dh, N, g)[:4])
+        o = H.step_grid(gpu, *d, dt, dh, N, g, dtype=dtp)
+        assert o[5] == 0.0
+        d = list(o[:4])
+    for a, b in zip(d, r):
+        assert H.field_err(a, b) <= TOL[prec]
+    assert H.rel_divb(*(np.asarray(a, dtype=np.float64) for a in d[1:]), dh) < (1e-13 if prec == 1 else 2e-5)
+
+
+def test_expansion_shock_dissolves_on_the_device(oracle):
+    """the textbook failure of the plain Roe flux (tests/test_oracle_hcorr.py) through the CUDA path: 8^3 patch groups along the tube"""
+    from test_oracle_hcorr import _tube_with_expansion_shock, _expansion_shock, GAM
+    res = {}
+    for hc in (0, 1):
+        U, bx, by, bz, dh, xc = _tube_with_expansion_shock(64)
+        U, bx, by, bz = (np.tile(a, (1, 2, 2, 1)) if a.ndim == 4 else a for a in (U, bx, by, bz))     # 8 cells across for 8^3 groups
+        bx = np.zeros((8, 8, 129)); by = np.zeros((8, 9, 128)); bz = np.zeros((9, 8, 128))
+        gpu = GU.GpuRunner(N=8, g=3 + hc, scheme=0, recon=0, riemann=2, prec=1, max_groups=16, hcorr=hc, gamma=GAM)
+        ref_cfg = oracle.make_config(N=8, g=3 + hc, gamma=GAM, scheme=0, recon=0, riemann=2, hcorr=hc)
+        Ur, br = U.copy(), (bx.copy(), by.copy(), bz.copy())
+        for _ in range(40):
+            U, bx, by, bz, _, _ = H.step_grid(gpu, U, bx, by, bz, 0.3 * dh / 3.6, dh, 8, 3 + hc)
+            Ur, b0, b1, b2, _, _ = H.step_grid(lambda a, b, c, d_: oracle.advance(ref_cfg, a, b, c, d_), Ur, *br, 0.3 * dh / 3.6, dh, 8, 3 + hc)
+            br = (b0, b1, b2)
+        w = np.abs(xc - 0.5) < 0.2
+        res[hc] = np.abs(np.diff(U[0][0, 0, :][w])).max()
+        assert H.field_err(U[0], Ur[0]) < 1e-11, hc
+    jump = _expansion_shock()[0][0] - _expansion_shock()[1][0]
+    assert res[0] > 0.95 * jump and res[1] < 0.5 * jump, res
+
+
+def test_h_correction_argument_checks():
+    from paper_1804_03479_b200 import mhd
+    for kw in (dict(riemann=mhd.HLLD, g=4), dict(riemann=mhd.ROE, g=3), dict(riemann=mhd.ROE, g=5, scheme=mhd.CTU, recon=mhd.PPM),
+               dict(riemann=mhd.ROE, g=5, scheme=mhd.VL, recon=mhd.PPM)):
+        with pytest.raises(mhd.MHDError) as ei:
+            mhd.Solver(mhd.make_config(hcorr=1, max_groups=2, **kw))
+        assert ei.value.code == mhd.EINVAL

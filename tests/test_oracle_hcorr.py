@@ -181,3 +181,20 @@ def test_linear_wave_stays_second_order_with_h_correction(oracle):
         adv = lambda Ui, Bi, dt, dh_: oracle.advance(cfg, Ui, Bi, dt, dh_)
         errs.append(waves.run_period(adv, lambda *a: 0.3 * a[4] / 2.0, U, bx, by, bz, dh, 1.0 / spd, 4, 4)[0])
     assert np.log2(errs[0] / errs[1]) > 1.5, errs
+
+
+def test_supersonic_shortcut_is_continuous_with_the_h_correction(oracle):
+    """plain Roe returns F_L as soon as the slowest wave moves right (lambda_min >= 0), and the dissipation formula tends to F_L
+    there.  With eta > 0 the formula gives F_L only for lambda_min >= eta, so R19 takes the shortcut only there: the flux is a
+    continuous function of eta (and of the states) across the switch."""
+    WL = np.array([1.0, 0.0, 0.1, -0.2, 0.6, np.sqrt(2.0), 0.5])       # P5 background: c_f = 2 along n with B_n = 1
+    WR = WL * np.array([1.02, 1.0, 0.9, 1.1, 0.97, 1.01, 0.98])
+    WL[1] = WR[1] = 2.2                                                 # slightly supersonic to the right
+    rc, lam, _, _, _ = oracle.eig_roe(WL, WR, 1.0)
+    assert rc == 0 and 0.05 < lam[0] < 0.4
+    FL = oracle.physflux(WL, 1.0)
+    assert np.array_equal(oracle.roe_eta(WL, WR, 1.0, 0.0)[0], FL)
+    assert np.array_equal(oracle.roe_eta(WL, WR, 1.0, 0.99 * lam[0])[0], FL)
+    just_above = oracle.roe_eta(WL, WR, 1.0, lam[0] * (1 + 1e-9))[0]
+    assert 0 < np.abs(just_above - FL).max() < 1e-8
+    assert np.abs(oracle.roe_eta(WL, WR, 1.0, 3.0 * lam[0])[0] - FL).max() > 1e-4
