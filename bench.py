@@ -297,7 +297,12 @@ def measure(args, prec_name, rank, world, dist, scheme=None, riemann=None, steps
                     "traffic_unit": "bytes per launch: ncu dram__bytes_read.sum + dram__bytes_write.sum, read at run time from "
                                     "profiles/r02_dram_traffic.csv (a %d-group launch)" % int(round(G / max(n_launch, 1))),
                     "avg_launch_ms": dur * 1e3, "launches_per_step": n_launch,
-                    "share_of_step": units[top]["ms_per_step"] / (prof_ms / steps)}
+                    "share_of_step": units[top]["ms_per_step"] / (prof_ms / steps),
+                    # the same arithmetic for every kernel of the step (the dominant one is the headline of this object)
+                    "all_kernels": {k: {"steps_covered": list(u["steps"]), "ms_per_step": u["ms_per_step"],
+                                        "achieved": sum(step_flops[i - 1] for i in u["steps"]) * G / (u["ms_per_step"] * 1e-3) / 1e12,
+                                        "frac": sum(step_flops[i - 1] for i in u["steps"]) * G / (u["ms_per_step"] * 1e-3) / 1e12 / peak}
+                                    for k, u in units.items() if u["steps"]}}
     # HBM view of the whole step: algorithmic bytes = read the ghost-zoned tile once, write the results once (the CFL
     # reduction is fused into the final update: no second read of the new state)
     sz = solver.sizes()
