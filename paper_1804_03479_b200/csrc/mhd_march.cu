@@ -56,12 +56,21 @@ cudaError_t launch_solver(const KParamsSC<R, 23>& p, int ng, int lim, int pass, 
 
 }  // namespace
 
-template <class R> bool vl_march_supports(int solver) { return solver == kHLLD; }
+// Roe: FP32 only (in FP64 the solver alone needs ~220 registers, a 484-thread block has 128 per thread); MHD_MARCH_ROE=0 keeps the
+// fused first pass + staged kernels of round 1 for A/B runs
+template <class R> bool vl_march_supports(int solver) {
+  if (solver == kHLLD) return true;
+  if (solver == kROE && sizeof(R) == 4) { const char* e = getenv("MHD_MARCH_ROE"); return !(e && e[0] == '0'); }
+  return false;
+}
 
 template <class R>
 cudaError_t launch_vl_march(const KParams<R>& p0, int ng, int solver, int lim, int pass, cudaStream_t st) {
   const KParamsSC<R, 23> p(p0);
   if (solver == kHLLD) return launch_solver<R, kHLLD>(p, ng, lim, pass, st);
+  if constexpr (sizeof(R) == 4) {
+    if (solver == kROE) return launch_solver<R, kROE>(p, ng, lim, pass, st);
+  }
   return cudaErrorInvalidValue;
 }
 

@@ -118,7 +118,7 @@ template <class R, bool TMA> constexpr size_t march1_smem() {
 // primitives and x / y face data), so every chunk repeats two planes of solves; the values it produces are those of the whole march,
 // bit for bit (same operations on the same operands), whatever the number of chunks.
 template <class R, int SOLVER, bool TMA>
-__global__ void __launch_bounds__(kMP, sizeof(R) == 4 ? 2 : 1) k_vl_march1(const KParamsSC<R, 23> p, const int per) {
+__global__ void __launch_bounds__(kMP, (sizeof(R) == 4 && SOLVER != kROE) ? 2 : 1) k_vl_march1(const KParamsSC<R, 23> p, const int per) {
   constexpr int T = kMT, P = kMP, T3 = T * T * T, XP = T * (T + 1);
   extern __shared__ __align__(16) unsigned char march_smem[];
   R* sW = reinterpret_cast<R*>(march_smem);     // [2][11][P]: primitives (8) and reference EMFs (3) of planes k, k-1
@@ -271,17 +271,24 @@ __global__ void __launch_bounds__(kMP, sizeof(R) == 4 ? 2 : 1) k_vl_march1(const
 // ring of three whole 22 x 22 planes of the 8 half-step primitives (k-1, k, k+1), filled by 1-D bulk copies (TMA) one
 // plane ahead: every slope operand comes from shared memory, and the plane is read from memory once.
 // ---------------------------------------------------------------------------------------------------------------------
+// FP32 also stages the time-n planes the update of cell plane k-1 reads (U, x / y faces of plane k-1, z faces of level k): 6 planes of
+// 484 + 2 x 508 values; in FP64 the block is at the 227 KB limit without them and reads them from memory
+template <class R> constexpr bool march2_stage_in() { return sizeof(R) == 4; }
+constexpr int kMXS = 508;                          // 22 x 23 face values + 2 of alignment slack
 template <class R> constexpr size_t march2_smem() {
-  return (size_t)((2 * 4 + 21 + 3 + 7 + 2) * kM2P + 3 * 8 * kMP) * sizeof(R) + 16;
+  return (size_t)((2 * 4 + 21 + 3 + 7 + 2) * kM2P + 3 * 8 * kMP + (march2_stage_in<R>() ? 6 * kMP + 2 * kMXS : 0)) * sizeof(R) + 32;
 }
 
 #ifndef MHD_M2_MINB
 #define MHD_M2_MINB 2
 #endif
+#ifndef MHD_M2_MINB_ROE
+#define MHD_M2_MINB_ROE 1
+#endif
 // S9 (p.red set: mhd_advance_dt) is a run-time branch, not a template flag: the two instantiations compiled the energy flux of
 // the Riemann solve to different last bits in FP32, and mhd_advance_dt must equal mhd_advance + mhd_dt_reduce bit for bit
 template <class R, int SOLVER, int LIM>
-__global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_march2(const KParamsSC<R, 23> p, const int per) {
+__global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? (SOLVER != kROE ? MHD_M2_MINB : MHD_M2_MINB_ROE) : 1) k_vl_march2(const KParamsSC<R, 23> p, const int per) {
   constexpr int T = kMT, PT = kMT * kMT, T3 = T * T * T, P = kM2P, W = kM2W, N = 16, M = N + 1, g = 3;
   extern __shared__ __align__(16) unsigned char march_smem[];
   R* sR = reinterpret_cast<R*>(march_smem);     // [3][8][PT]: half-step primitives of planes k-1, k, k+1 (plane kp in slot kp % 3)
@@ -290,7 +297,13 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
   R* sE = sF + 21 * P;                           // [3][P]
   R* sZ = sE + 3 * P;                            // [7][P]: W(k-1) + slope_z(k-1)/2 of the thread's own column
   R* sX = sZ + 7 * P;                            // [2][P]: new lower x / y faces of plane k-1 (DT)
-  unsigned long long* bar = reinterpret_cast<unsigned long long*>(sX + 2 * P);
+  constexpr bool SIN = march2_stage_in<R>();
+  R* sUt = sX + 2 * P;                           // SIN: [5][PT] U of plane k-1, then x faces [kMXS], y faces [kMXS] of plane k-1, z faces [PT] of level k
+  R* sBxt = sUt + 5 * PT;
+  R* sByt = sBxt + kMXS;
+  R* sBzt = sByt + kMXS;
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(SIN ? sBzt + PT : sX + 2 * P);
+  unsigned long long* bar2 = bar + 1;
   const int t = threadIdx.x, i = t % W + 2, j = t / W + 2, grp = blockIdx.x;
   const int c = j * T + i;
   const R* ws = p.ws + (size_t)grp * kMWS;
@@ -326,10 +339,26 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
 #pragma unroll
     for (int v = 0; v < 8; ++v) bulk_load(sR + ((kp % 3) * 8 + v) * PT, Wh + v * T3 + kp * PT, PB, bar);
   };
+  // SIN: the time-n planes that iteration kn + 1 reads: U, x / y faces of plane kn, z faces of level kn + 1 (alignment as in pass 1)
+  auto stage_in = [&](int kn) {
+    constexpr unsigned PB = PT * sizeof(R);
+    constexpr int XP = T * (T + 1);
+    const unsigned mis = (unsigned)((size_t)kn * XP * sizeof(R)) & 15u;
+    const unsigned XB = (unsigned)(XP * sizeof(R) + mis + 15u) & ~15u;
+    mbar_expect_tx(bar2, 6u * PB + 2u * XB);
+#pragma unroll
+    for (int v = 0; v < 5; ++v) bulk_load(sUt + v * PT, U + v * T3 + kn * PT, PB, bar2);
+    bulk_load(sBxt, reinterpret_cast<const char*>(Bx + kn * XP) - mis, XB, bar2);
+    bulk_load(sByt, reinterpret_cast<const char*>(By + kn * XP) - mis, XB, bar2);
+    bulk_load(sBzt, Bz + (kn + 1) * PT, PB, bar2);
+  };
+  const bool sin = SIN && ((reinterpret_cast<size_t>(p.Uin) | reinterpret_cast<size_t>(p.Bin)) & 15) == 0;   // bulk copies need 16-byte aligned planes
   if (t == 0) {
     mbar_init(bar, 1);
+    if (SIN) mbar_init(bar2, 1);
     mbar_expect_tx(bar, 3u * 8u * PT * sizeof(R));
     stage(kb - 1, false); stage(kb, false); stage(kb + 1, false);
+    if (sin) stage_in(kb);
   }
   __syncthreads();
   mbar_wait(bar, 0);
@@ -395,16 +424,26 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
     if (t == 0 && k + 2 <= k1 + 1) stage(k + 2, true);                    // into the slot of plane k-1: nobody reads it any more
     // time-n data of cell (i, j, k-1), its lower x / y faces and the lower z face of level k-1/2: asked for here, used below
     R Ut[5] = { R(0), R(0), R(0), R(0), R(0) }, bxo = R(0), byo = R(0), bzo = R(0);
-    if (k >= kb + 2) {
-      const int cq = ((k - 1) * T + j) * T + i;
-      if (in) {
+    if (sin) {
+      if (k > kb) {
+        mbar_wait(bar2, (unsigned)(k - kb - 1) & 1u);
+        const int sh = (int)((((size_t)(k - 1) * T * (T + 1) * sizeof(R)) & 15u) / sizeof(R));
 #pragma unroll
-        for (int v = 0; v < 5; ++v) Ut[v] = U[v * T3 + cq];
+        for (int v = 0; v < 5; ++v) Ut[v] = sUt[v * PT + c];
+        bxo = sBxt[sh + j * (T + 1) + i]; byo = sByt[sh + c]; bzo = sBzt[c];
       }
-      if (fx) bxo = Bx[((k - 1) * T + j) * (T + 1) + i];
-      if (fy) byo = By[((k - 1) * (T + 1) + j) * T + i];
+    } else {
+      if (k >= kb + 2) {
+        const int cq = ((k - 1) * T + j) * T + i;
+        if (in) {
+#pragma unroll
+          for (int v = 0; v < 5; ++v) Ut[v] = U[v * T3 + cq];
+        }
+        if (fx) bxo = Bx[((k - 1) * T + j) * (T + 1) + i];
+        if (fy) byo = By[((k - 1) * (T + 1) + j) * T + i];
+      }
+      if (in && k > kb) bzo = Bz[(k * T + j) * T + i];
     }
-    if (in && k > kb) bzo = Bz[(k * T + j) * T + i];
     if (k < k1) {
       const int qn = (k + 1) * PT + c;
       bhn[0] = bh[qn]; bhn[1] = bh[T3 + qn]; bhn[2] = bh[2 * T3 + qn];
@@ -465,6 +504,7 @@ __global__ void __launch_bounds__(kM2P, sizeof(R) == 4 ? MHD_M2_MINB : 1) k_vl_m
       }
     }
     __syncthreads();
+    if (sin && t == 0 && k > kb && k + 1 <= k1) stage_in(k);               // every thread has taken the planes of this iteration
     // ---- CT (Eq. 13): lower z face of level k-1/2; lower x / y faces of plane k-1 ----
     R bzn = R(0), bxn = R(0), byn = R(0);
     if (in && k > kb) {
