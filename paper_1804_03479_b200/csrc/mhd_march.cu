@@ -31,7 +31,7 @@ template <class R, int SOLVER>
 cudaError_t launch_solver(const KParamsSC<R, 23>& p, int ng, int lim, int pass, cudaStream_t st) {
   if (pass == 1) {
     // bulk copies need 16-byte aligned planes: the group strides are multiples of 16 bytes, the base pointers must be
-    static const bool no_tma = getenv("MHD_NO_TMA") != nullptr;
+    const bool no_tma = getenv("MHD_NO_TMA") != nullptr;      // read at every launch (tests switch it within one process)
     const bool tma = !no_tma && ((reinterpret_cast<size_t>(p.Uin) | reinterpret_cast<size_t>(p.Bin)) & 15) == 0;
     const int chunks = std::max(1, std::min(10, kMarchSlots / ng)), per = (20 + chunks - 1) / chunks;   // 20 half-step planes
     cudaError_t e;

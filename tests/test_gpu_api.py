@@ -469,3 +469,38 @@ def test_march_chunks_give_the_same_bits(prec, monkeypatch):
     for r in res[1:]:
         for k in ("U", "B", "flux", "emf", "dt"):
             assert np.array_equal(res[0][k], r[k]), k
+
+
+@pytest.mark.parametrize("prec", [1, 0])
+def test_march_without_tma_and_with_misaligned_inputs_gives_the_same_bits(prec, monkeypatch):
+    """The marching kernels stage their input planes by 1-D bulk copies (TMA), which need 16-byte aligned planes.  Input
+    arrays that start 4 / 8 bytes off a 16-byte boundary (a view into a larger tensor) take the direct-load instantiation
+    of pass 1 and the direct loads of pass 2; so does MHD_NO_TMA=1.  All three give bitwise the same outputs and CFL speed."""
+    import torch
+    from paper_1804_03479_b200 import mhd
+    dtp = GU.np_dtype(prec)
+    G = 6
+    U, B, dh = small_batch(G, g=3, dtype=dtp)
+    s = mhd.Solver(mhd.make_config(N=16, g=3, prec=prec, max_groups=G))
+
+    def run(dU, dB):
+        out = s.alloc_outputs(G)
+        dt, sm = s.advance_dt(dU, dB, out["U"], out["B"], out["flux"], out["emf"], G, 2e-3, dh, 0.3)
+        r = {k: v.cpu().numpy() for k, v in out.items()}
+        r["dt"] = np.array([dt, sm])
+        return r
+    ref = run(torch.from_numpy(U).cuda(), torch.from_numpy(B).cuda())
+    # misaligned: element 1 of a larger allocation (cudaMalloc returns 256-byte aligned blocks)
+    bigU = torch.empty(U.size + 1, dtype=torch.float32 if prec == 0 else torch.float64, device="cuda")
+    bigB = torch.empty(B.size + 1, dtype=bigU.dtype, device="cuda")
+    mU, mB = bigU[1:], bigB[1:]
+    mU.copy_(torch.from_numpy(U.ravel())); mB.copy_(torch.from_numpy(B.ravel()))
+    assert mU.data_ptr() % 16 != 0 and mB.data_ptr() % 16 != 0
+    mis = run(mU, mB)
+    monkeypatch.setenv("MHD_NO_TMA", "1")
+    notma = run(torch.from_numpy(U).cuda(), torch.from_numpy(B).cuda())
+    monkeypatch.delenv("MHD_NO_TMA")
+    for k in ref:
+        assert np.array_equal(ref[k], mis[k]), ("misaligned", k)
+        assert np.array_equal(ref[k], notma[k]), ("MHD_NO_TMA", k)
+    s.destroy()
