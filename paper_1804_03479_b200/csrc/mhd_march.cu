@@ -8,10 +8,15 @@ namespace mhd {
 
 namespace {
 
-// block slots of the marching kernels on one B200 (two resident blocks on each of 148 SMs); MHD_MARCH_SLOTS overrides (tests: 1 = never
+// block slots of the marching kernels on one B200 (two resident blocks on each of 148 SMs in FP32 with HLLD); MHD_MARCH_SLOTS overrides (tests: 1 = never
 // chunk, a large value = always the finest chunks)
-inline int march_slots() { const char* e = getenv("MHD_MARCH_SLOTS"); const int v = e ? atoi(e) : 0; return v > 0 ? v : 296; }
-#define kMarchSlots march_slots()
+// one_per_sm: FP64 and Roe run one block per SM
+inline int march_slots(bool one_per_sm) {
+  const char* e = getenv("MHD_MARCH_SLOTS");
+  const int v = e ? atoi(e) : 0;
+  return v > 0 ? v : (one_per_sm ? 148 : 296);
+}
+#define kMarchSlots march_slots(sizeof(R) == 8 || SOLVER == kROE)
 
 template <class K> cudaError_t big_smem(K kernel, size_t bytes) {
   return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
