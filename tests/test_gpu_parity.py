@@ -182,3 +182,41 @@ def test_config4_blast_ctu_ppm_fp64_10_steps(oracle):
     assert H.rel_divb(res[1], res[2], res[3], dh) < 1e-13
     t0, t1 = H.totals(U), H.totals(res[0])
     assert abs(t1[4] - t0[4]) / t0[4] < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# degenerate states through the plane-marching VL kernels: B = 0 (HLLD's double-star state collapses, every EMF is zero), the
+# static blast (zero velocity: every mass flux sits inside the dead zone of the CT switch; strong shock; floors)
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [1, 0])
+@pytest.mark.parametrize("which", ["hydro", "blast"])
+def test_vl_march_on_degenerate_states(oracle, which, prec):
+    n, N, g = 32, 16, 3
+    dtp = GU.np_dtype(prec)
+    if which == "hydro":
+        U, bx, by, bz, dh = inputs.random_group_grid(n, 99)
+        bx, by, bz = np.zeros_like(bx), np.zeros_like(by), np.zeros_like(bz)
+        rho = U[0]
+        v = U[1:4] / rho
+        U = inputs.conserved(rho, v[0], v[1], v[2], 0.6 + 0.0 * rho, bx, by, bz)
+    else:
+        U, bx, by, bz, dh = inputs.blast_grid(n)
+    state0 = tuple(a.astype(dtp).astype(np.float64) for a in (U, bx, by, bz))
+    cfg, adv = oracle_fn(oracle, N, g, 0, 0, 1, 0, prec)
+    dts, ref, ref_out = PC.run_grid_oracle(oracle, adv, state0, dh, N, g)
+    gpu = GU.GpuRunner(N=N, g=g, scheme=0, recon=0, riemann=1, prec=prec, max_groups=8)
+    res, gpu_out = PC.run_grid(gpu, state0, dts, dh, N, g, dtype=dtp)
+    errs = PC.grid_errors(res, ref)
+    if which == "hydro":
+        for k in ("Bx", "By", "Bz"):
+            assert errs.pop(k) == 0.0 and not np.any(res[1:][("Bx", "By", "Bz").index(k)])      # B stays exactly zero
+    if prec == 1:
+        assert_fields(errs, TOL[1], f"{which} FP64")
+    else:
+        s32, _ = PC.run_grid(_fp32_reference(oracle, cfg), state0, dts, dh, N, g, dtype=np.float32)
+        e32 = PC.grid_errors(s32, ref)
+        gate = PC.fp32_gate({k: e32[k] for k in errs})
+        bad = {k: (v, gate[k]) for k, v in errs.items() if not v <= gate[k]}
+        assert not bad, f"{which} FP32 over the gate (R14b): {bad}; oracle-FP32 {e32}"
+    t0, t1 = H.totals(state0[0]), H.totals(res[0].astype(np.float64))
+    assert abs(t1[0] - t0[0]) / t0[0] < (1e-13 if prec == 1 else 2e-6) and abs(t1[4] - t0[4]) / t0[4] < (1e-13 if prec == 1 else 2e-6)
