@@ -186,34 +186,32 @@ __device__ __forceinline__ void riemann_hlld(const R (&wl)[7], const R (&wr)[7],
   const R bn2 = bn * bn;
   R irL, irR;
   frcp2(wl[0], wr[0], irL, irR);
-  R pT[2], vB[2], en[2], cf[2], gg[2], root[2], xx[2];
+  R pT[2], pmag[2], cf[2], root[2], a2[2], ca2[2], ct2[2];
 #pragma unroll
   for (int a = 0; a < 2; ++a) {
     const R (&w)[7] = a ? wr : wl;
     const R ir = a ? irR : irL;
     const R bt2 = w[5] * w[5] + w[6] * w[6];
-    const R pmag = R(0.5) * (bn2 + bt2);
-    pT[a] = w[4] + pmag;
-    vB[a] = bn * w[1] + w[5] * w[2] + w[6] * w[3];
-    en[a] = w[4] * gm1inv + R(0.5) * w[0] * (w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) + pmag;
+    pmag[a] = R(0.5) * (bn2 + bt2);
+    pT[a] = w[4] + pmag[a];
     // c_f^2 = 1/2 [ (a^2+ca^2+ct^2) + sqrt( (ca^2+ct^2-a^2)^2 + 4 a^2 ct^2 ) ]   (R1, R18)
-    const R a2 = gam * w[4] * ir, ca2 = bn2 * ir, ct2 = bt2 * ir;
-    const R sum = a2 + ca2 + ct2, dif = ca2 + ct2 - a2;
-    root[a] = Num<R>::sqrt(dif * dif + R(4) * a2 * ct2);
+    a2[a] = gam * w[4] * ir; ca2[a] = bn2 * ir; ct2[a] = bt2 * ir;
+    const R sum = a2[a] + ca2[a] + ct2[a], dif = ca2[a] + ct2[a] - a2[a];
+    root[a] = Num<R>::sqrt(dif * dif + R(4) * a2[a] * ct2[a]);
     cf[a] = Num<R>::sqrt(R(0.5) * (sum + root[a]));
-    // cf^2 - ca^2 = 1/2 (x + root), x = a^2 + ct^2 - ca^2 (root^2 = x^2 + 4 ca^2 ct^2); rationalised where x < 0
-    xx[a] = a2 + ct2 - ca2;
-    gg[a] = R(2) * ca2 * ct2;                 // numerator of the rationalised form
-  }
-  {
-    R i0, i1;
-    frcp2(xx[0] < R(0) ? root[0] - xx[0] : R(1), xx[1] < R(0) ? root[1] - xx[1] : R(1), i0, i1);
-    gg[0] = xx[0] < R(0) ? gg[0] * i0 : R(0.5) * (xx[0] + root[0]);
-    gg[1] = xx[1] < R(0) ? gg[1] * i1 : R(0.5) * (xx[1] + root[1]);
   }
   const R uL = wl[1], uR = wr[1];
   const bool lmax = cf[0] >= cf[1];
   const R cmax = lmax ? cf[0] : cf[1];
+  // cf^2 - ca^2 of the faster side = 1/2 (x + root), x = a^2 + ct^2 - ca^2 (root^2 = x^2 + 4 ca^2 ct^2); rationalised where x < 0
+  R gm;
+  {
+    const R a2m = lmax ? a2[0] : a2[1], ca2m = lmax ? ca2[0] : ca2[1], ct2m = lmax ? ct2[0] : ct2[1], rootm = lmax ? root[0] : root[1];
+    const R xx = a2m + ct2m - ca2m;
+    const R gnum = R(2) * ca2m * ct2m;          // numerator of the rationalised form
+    const R inv = frcp(xx < R(0) ? rootm - xx : R(1));
+    gm = xx < R(0) ? gnum * inv : R(0.5) * (xx + rootm);
+  }
   const R SL = Num<R>::min(uL, uR) - cmax, SR = Num<R>::max(uL, uR) + cmax;
   const R sL = (SL - uL) * wl[0], sR = (SR - uR) * wr[0];
   const R idn = frcp(sR - sL);
@@ -225,24 +223,26 @@ __device__ __forceinline__ void riemann_hlld(const R (&wl)[7], const R (&wr)[7],
   const R SM = uL - uLmSM;
   const R pTs = (sR * pT[0] - sL * pT[1] + sL * sR * (uR - uL)) * idn;
   const R tiny = R(1e-12) * pTs;
+  // the side of the contact the face lies on: S_L <= S*_L <= S_M in floating point too (S*_L = S_M - |Bn| / sqrt(rho*_L))
+  const bool left = (SL >= R(0)) || (SM >= R(0));
   // rho (S-u)^2 - Bn^2 of each side without cancellation: (S-u)^2 = (cmax + delta)^2, cmax^2 = ca_m^2 + g_m
   const R delta = Num<R>::max(du, R(0));
-  const R gm = lmax ? gg[0] : gg[1], rhom = lmax ? wl[0] : wr[0], irm = lmax ? irL : irR;
+  const R rhom = lmax ? wl[0] : wr[0], irm = lmax ? irL : irR;
   const R grow = gm + delta * (R(2) * cmax + delta);
   const R bfac = bn2 * irm;
 
-  // star states of both sides (the double-star state needs both)
+  // star states of both sides (the double-star state needs both); total energy and v.B only of the side the face lies on
   const R dSML = (SL - uL) + uLmSM, dSMR = (SR - uR) + uRmSM;               // S_alpha - S_M
   const R NbL = wl[0] * grow + bfac * (wl[0] - rhom), NbR = wr[0] * grow + bfac * (wr[0] - rhom);   // rho (S-u)^2 - Bn^2
   const R DL = NbL + sL * uLmSM, DR = NbR + sR * uRmSM;                     // rho (S-u)(S-S_M) - Bn^2
   const bool degL = Num<R>::abs(DL) < tiny, degR = Num<R>::abs(DR) < tiny;
   R idSML, idSMR, iDL, iDR;
   frcp4(dSML, dSMR, degL ? R(1) : DL, degR ? R(1) : DR, idSML, idSMR, iDL, iDR);
-  R rs[2], v1s[2], v2s[2], b1s[2], b2s[2], es[2], vBs[2], sq[2], isq[2];
+  R rs[2], v1s[2], v2s[2], b1s[2], b2s[2], sq[2], isq[2];
 #pragma unroll
   for (int a = 0; a < 2; ++a) {
     const R (&w)[7] = a ? wr : wl;
-    const R Sa = a ? SR : SL, sa = a ? sR : sL, umSM = a ? uRmSM : uLmSM;
+    const R sa = a ? sR : sL, umSM = a ? uRmSM : uLmSM;
     const R idSM = a ? idSMR : idSML, iD = a ? iDR : iDL, Nb = a ? NbR : NbL;
     const bool degen = a ? degR : degL;
     rs[a] = sa * idSM;
@@ -250,28 +250,30 @@ __device__ __forceinline__ void riemann_hlld(const R (&wl)[7], const R (&wr)[7],
     const R fb = degen ? R(1) : Nb * iD;
     v1s[a] = w[2] - w[5] * fv; v2s[a] = w[3] - w[6] * fv;
     b1s[a] = w[5] * fb; b2s[a] = w[6] * fb;
-    vBs[a] = bn * SM + b1s[a] * v1s[a] + b2s[a] * v2s[a];
-    es[a] = ((Sa - w[1]) * en[a] - pT[a] * w[1] + pTs * SM + bn * (vB[a] - vBs[a])) * idSM;
     sqrt_and_inverse(rs[a], sq[a], isq[a]);
   }
   const R abn = Num<R>::abs(bn);
-  const R SsL = SM - abn * isq[0], SsR = SM + abn * isq[1];
-
-  // which side of the contact the face lies on, and in which region of that side
-  const bool left = (SL >= R(0)) || (SsL >= R(0)) || (SM >= R(0));
-  const bool outer = left ? (SL >= R(0)) : !(SR >= R(0));           // plain F_L / F_R
-  const bool star = left ? (SsL >= R(0)) : !(SsR >= R(0));          // single-star region (if not outer)
-  const R Sa = left ? SL : SR, Ssa = left ? SsL : SsR;
+  // the chosen side: input state, conserved state and physical flux (Eq. 5, 7), star state
+  R wa[7];
+#pragma unroll
+  for (int c = 0; c < 7; ++c) wa[c] = left ? wl[c] : wr[c];
+  const R pTa = left ? pT[0] : pT[1], pma = left ? pmag[0] : pmag[1];
+  const R Sa = left ? SL : SR, idSMa = left ? idSML : idSMR, isqa = left ? isq[0] : isq[1];
   const R r_s = left ? rs[0] : rs[1], sq_a = left ? sq[0] : sq[1];
   const R v1a = left ? v1s[0] : v1s[1], v2a = left ? v2s[0] : v2s[1];
   const R b1a = left ? b1s[0] : b1s[1], b2a = left ? b2s[0] : b2s[1];
-  const R esa = left ? es[0] : es[1], vBa = left ? vBs[0] : vBs[1];
-  R Us[7] = { r_s, r_s * SM, r_s * v1a, r_s * v2a, esa, b1a, b2a };
+  const R vBa0 = bn * wa[1] + wa[5] * wa[2] + wa[6] * wa[3];
+  const R ena = wa[4] * gm1inv + R(0.5) * wa[0] * (wa[1] * wa[1] + wa[2] * wa[2] + wa[3] * wa[3]) + pma;
+  const R vBa = bn * SM + b1a * v1a + b2a * v2a;
+  const R esa = ((Sa - wa[1]) * ena - pTa * wa[1] + pTs * SM + bn * (vBa0 - vBa)) * idSMa;
+  const R Ssa = left ? SM - abn * isqa : SM + abn * isqa;
+  // region of that side: plain F_L / F_R, single star, double star
+  const bool outer = left ? (SL >= R(0)) : !(SR >= R(0));
+  const bool star = left ? (Ssa >= R(0)) : !(Ssa >= R(0));
+  const R Us[7] = { r_s, r_s * SM, r_s * v1a, r_s * v2a, esa, b1a, b2a };
+  // double-star state (transverse components and energy; U** = U* where Bn vanishes: no rotational waves)
   R Uss[7];
-  if (R(0.5) * bn2 < tiny) {
-#pragma unroll
-    for (int c = 0; c < 7; ++c) Uss[c] = Us[c];
-  } else {
+  {
     const R sg = bn > R(0) ? R(1) : R(-1);
     const R ir = frcp(sq[0] + sq[1]);
     const R v1 = (sq[0] * v1s[0] + sq[1] * v1s[1] + (b1s[1] - b1s[0]) * sg) * ir;
@@ -284,20 +286,18 @@ __device__ __forceinline__ void riemann_hlld(const R (&wl)[7], const R (&wr)[7],
     Uss[4] = esa + pm * sq_a * (vBa - vBss) * sg;
     Uss[5] = b1; Uss[6] = b2;
   }
-  // conserved state and physical flux (Eq. 5, 7) of the chosen side only
-  R wa[7];
-#pragma unroll
-  for (int c = 0; c < 7; ++c) wa[c] = left ? wl[c] : wr[c];
-  const R pTa = left ? pT[0] : pT[1], vBa0 = left ? vB[0] : vB[1], ena = left ? en[0] : en[1];
   const R mn = wa[0] * wa[1];
   const R Ua[7] = { wa[0], mn, wa[0] * wa[2], wa[0] * wa[3], ena, wa[5], wa[6] };
   const R Fa[7] = { mn, mn * wa[1] + pTa - bn2, mn * wa[2] - bn * wa[5], mn * wa[3] - bn * wa[6],
                     (ena + pTa) * wa[1] - bn * vBa0, wa[5] * wa[1] - bn * wa[2], wa[6] * wa[1] - bn * wa[3] };
+  // F* = F_a + S_a (U* - U_a);  F** = F_a + S* U** - (S* - S_a) U* - S_a U_a = F* + S* (U** - U*): one expression for both regions with
+  // S* := 0 in the single-star region and where Bn vanishes (rho and the normal momentum are the same in U* and U**)
+  const R Sse = (star || R(0.5) * bn2 < tiny) ? R(0) : Ssa;
 #pragma unroll
   for (int c = 0; c < 7; ++c) {
-    const R f_star = Fa[c] + Sa * (Us[c] - Ua[c]);
-    const R f_dstar = Fa[c] + Ssa * Uss[c] - (Ssa - Sa) * Us[c] - Sa * Ua[c];
-    F[c] = outer ? Fa[c] : (star ? f_star : f_dstar);
+    R f = Fa[c] + Sa * (Us[c] - Ua[c]);
+    if (c >= 2) f += Sse * (Uss[c] - Us[c]);
+    F[c] = outer ? Fa[c] : f;
   }
 }
 

@@ -266,14 +266,15 @@ def test_fused_pass1_agrees_with_the_staged_kernels(scheme, recon, g, monkeypatc
     """The first pass of the standard FP32 patch group runs in one kernel (CTU steps 1 + 2: csrc/mhd_ctu_pass1.cuh; VL
     S0-S2: csrc/mhd_vl_pass1.cuh); with MHD_NO_FUSED_PASS1 the same solver runs the staged kernels.  Same functions, same
     operands, but the compiler orders / contracts the arithmetic inside a stage differently, so the two agree to the last
-    bits only: a few FP32 ulp of each field's scale (measured 1e-7 U, 8e-7 B, 5e-7 fluxes, 8e-6 EMFs)"""
+    bits only: a few FP32 ulp of each field's scale (measured 1e-7 U, 1.4e-6 B, 5e-7 fluxes; EMFs 5e-7 ... 3.3e-5: an edge whose mass
+    flux lies in the ramp of the CT switch, R10a, turns an ulp of that flux into a visible change of its weight)"""
     U, B, dh = small_batch(5, g=g, dtype=np.float32)
     kw = dict(N=16, g=g, scheme=scheme, recon=recon, riemann=1, prec=0, max_groups=5)
     fused = GU.GpuRunner(**kw)
     monkeypatch.setenv("MHD_NO_FUSED_PASS1", "1")
     staged = GU.GpuRunner(**kw)
     monkeypatch.delenv("MHD_NO_FUSED_PASS1")
-    tol = {"U": 5e-7, "B": 3e-6, "flux": 3e-6, "emf": 3e-5}
+    tol = {"U": 5e-7, "B": 5e-6, "flux": 3e-6, "emf": 1e-4}
     for dt in (1e-3, 2e-3, 3e-3):
         a, b = fused(U, B, dt, dh), staged(U, B, dt, dh)
         for k in ("U", "B", "flux", "emf"):
