@@ -69,7 +69,8 @@ typedef struct {
 /* MHD_ESTATE: a call that returns a time step (mhd_dt_reduce, mhd_advance_dt, mhd_advance_host_dt, mhd_grid_dt,
  * mhd_grid_advance_dt) found no finite positive signal speed -- the state holds NaN or infinite values (a cell with a NaN
  * input reports an infinite speed, so the maximum cannot drop it).  The arrays have been written; *dt_out is not usable. */
-enum { MHD_OK = 0, MHD_EINVAL = -1, MHD_ECUDA = -2, MHD_ENOMEM = -3, MHD_ESTATE = -4 };
+enum { MHD_OK = 0, MHD_EINVAL = -1, MHD_ECUDA = -2, MHD_ENOMEM = -3, MHD_ESTATE = -4, MHD_ELIMIT = -5 };
+/* MHD_ELIMIT: the call needs more than the fixed capacity of a no-allocation entry point (mhd_dt_reduce_noalloc). */
 
 /* Create a solver.  Allocates the device workspace (for min(max_groups, what fits a 6 GB budget) groups: larger
  * batches are processed in equal slices).  Returns MHD_EINVAL for a bad configuration (incl. too small a ghost width), MHD_ECUDA /
@@ -119,6 +120,24 @@ int mhd_dt_reduce(mhd_solver* s, const void* U, const void* B, int ngroups, int 
 int mhd_advance_dt(mhd_solver* s, const void* U_in, const void* B_in, void* U_out, void* B_out, void* flux_out,
                    void* emf_out, int ngroups, double dt, double dh, double cfl, double* dt_out, double* maxspeed_out,
                    void* cuda_stream);
+
+/* mhd_dt_reduce for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same CFL reduction (R13) with NO solver object, no cudaMalloc / cudaFree / allocating
+ * library call, and no host synchronisation.  The scratch memory of the reduction (one partial maximum per 256-cell block and an
+ * arrival counter) is a fixed array of the library's device image: (MHD_NOALLOC_MAX_BLOCKS + 32) * 8 bytes = 513 KB, held on
+ * every GPU that loads the library until the process exits.  It runs on the CURRENT device.
+ *   prec: MHD_FP32 / MHD_FP64, the element type of U and B (DEVICE arrays, layouts of mhd_dt_reduce: ps2 interior cells per
+ *   side, nghost_of_arrays ghost cells in the arrays, 0 ... 8); gamma, min_dens, min_pres as in mhd_config (no defaults here).
+ *   dt_speed_out: DEVICE pointer to two doubles, written by the kernel: [0] = dt = cfl * dh / maxspeed, [1] = maxspeed -- the bits
+ *   that mhd_dt_reduce returns for the same arguments.  A state with NaN / infinite values gives maxspeed = +inf and dt = 0 (the
+ *   call is asynchronous and cannot return MHD_ESTATE): the caller checks.
+ * Limit: ngroups * ceil(ps2^3 / 256) <= MHD_NOALLOC_MAX_BLOCKS and ngroups <= 65535 (4096 groups of 16^3), else MHD_ELIMIT and
+ * nothing is launched.  Asynchronous on cuda_stream: one memset node (the counter) and one kernel, both capturable.  The first call
+ * on a device asks the driver for the array's address (cudaGetSymbolAddress): make it outside a capture.
+ * All calls share the one array: calls that overlap on the GPU (other streams, concurrently replayed graphs) race -- serialise. */
+#define MHD_NOALLOC_MAX_BLOCKS 65536
+int mhd_dt_reduce_noalloc(int prec, const void* U, const void* B, int ngroups, int ps2, int nghost_of_arrays, double gamma,
+                          double min_dens, double min_pres, double dh, double cfl, double* dt_speed_out, void* cuda_stream);
 
 /* Cumulative event counters since creation (density floors, pressure floors, Roe->HLLE fallbacks).
  * Synchronises the device; asynchronous kernel faults surface here as MHD_ECUDA. */

@@ -20,6 +20,8 @@ UNITS = {
     "mhd_api.cu": COMMON + ["mhd_api_host.inl", "mhd_api_grid.inl", "mhd_api_amr.inl", "mhd_grid.cuh", "mhd_amr.cuh", "mhd_prolong.cuh",
                             os.path.join("..", "..", "include", "mhd.h")],
     "mhd_march.cu": COMMON + ["mhd_vl_march.cuh"],
+    "mhd_noalloc.cu": ["mhd_physics.cuh", "mhd_eigen.cuh", "mhd_recon.cuh", "mhd_kernels.cuh", "mhd_kernels2.cuh", "mhd_kernels3.cuh",
+                       os.path.join("..", "..", "include", "mhd.h")],
 }
 OBJDIR = os.path.join(HERE, "build")
 

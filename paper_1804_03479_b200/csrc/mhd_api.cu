@@ -412,6 +412,11 @@ static void free_lanes(mhd_solver* s) {
   s->lane_groups = 0; s->lane_count = 0;
 }
 
+// for the other translation units of the library (mhd_noalloc.cu): a CUDA failure recorded for mhd_strerror(MHD_ECUDA)
+namespace mhd {
+int note_cuda_failure(cudaError_t e, const char* where) { return cuda_fail(e, where); }
+}
+
 extern "C" {
 
 int mhd_create(const mhd_config* cfg, mhd_solver** out) {

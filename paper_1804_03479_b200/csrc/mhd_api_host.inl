@@ -181,6 +181,7 @@ const char* mhd_strerror(int code) {
     case MHD_ECUDA: return g_cuda_err.c_str();
     case MHD_ENOMEM: return "out of device memory";
     case MHD_ESTATE: return "the state has no finite positive signal speed (NaN or infinite values): no time step";
+    case MHD_ELIMIT: return "size beyond the fixed capacity of a no-allocation entry point (MHD_NOALLOC_MAX_BLOCKS, include/mhd.h)";
     default: return "unknown error code";
   }
 }

@@ -19,9 +19,10 @@ PLM, PPM = 0, 1
 HLLE, HLLD, ROE = 0, 1, 2
 LIM_PRIM, LIM_CHAR = 0, 1
 MC, MINMOD, VANLEER = 0, 1, 2
-OK, EINVAL, ECUDA, ENOMEM, ESTATE = 0, -1, -2, -3, -4
+OK, EINVAL, ECUDA, ENOMEM, ESTATE, ELIMIT = 0, -1, -2, -3, -4, -5
+NOALLOC_MAX_BLOCKS = 65536      # include/mhd.h MHD_NOALLOC_MAX_BLOCKS
 
-EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance_host", "mhd_advance_host_dt", "mhd_dt_reduce", "mhd_advance_dt",
+EXPORTS = ["mhd_create", "mhd_destroy", "mhd_sizes", "mhd_advance", "mhd_advance_host", "mhd_advance_host_dt", "mhd_dt_reduce", "mhd_dt_reduce_noalloc", "mhd_advance_dt",
            "mhd_get_stats", "mhd_launch_count", "mhd_grid_pack", "mhd_grid_unpack", "mhd_grid_advance", "mhd_grid_advance_dt", "mhd_grid_dt", "mhd_amr_restrict", "mhd_amr_fixup", "mhd_amr_prolong", "mhd_set_profiling", "mhd_get_profile", "mhd_profile_stage_name",
            "mhd_measure_fma_peak", "mhd_strerror"]
 
@@ -57,6 +58,8 @@ def lib():
         L.mhd_advance_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int]
         L.mhd_dt_reduce.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_double),
                                     C.POINTER(C.c_double), vp]
+        L.mhd_dt_reduce_noalloc.argtypes = [C.c_int, vp, vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double,
+                                            C.c_double, vp, vp]
         L.mhd_advance_host_dt.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int,
                                           C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.mhd_advance_dt.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_double, C.c_double, C.c_double,
@@ -142,6 +145,23 @@ def _stream_ptr(stream):
         import torch
         stream = torch.cuda.current_stream()
     return C.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def dt_reduce_noalloc(prec, U, B, ngroups, ps2, nghost_of_arrays, gamma, min_dens, min_pres, dh, cfl, dt_speed_out, stream=None):
+    """mhd_dt_reduce_noalloc: the CFL reduction with no solver object and no allocation (scratch = a fixed array of the library's
+    device image), asynchronous on `stream`; dt_speed_out = CUDA float64 tensor of >= 2 elements that receives (dt, maxspeed).
+    Raises MHDError(ELIMIT) beyond ngroups * ceil(ps2^3 / 256) = NOALLOC_MAX_BLOCKS.  Runs on the current device."""
+    import torch
+    dev = torch.cuda.current_device()
+    T = int(ps2) + 2 * int(nghost_of_arrays)
+    G = max(int(ngroups), 0)
+    if G * ((int(ps2) ** 3 + 255) // 256) > NOALLOC_MAX_BLOCKS or G > 65535:
+        G = 0                          # the library rejects the call (MHD_ELIMIT); no size to check against
+    _checked(U, prec, G * 5 * T ** 3, "U", dev)
+    _checked(B, prec, G * 3 * T * T * (T + 1), "B", dev)
+    _checked(dt_speed_out, FP64, 2, "dt_speed_out", dev)
+    _check(lib().mhd_dt_reduce_noalloc(int(prec), _ptr(U), _ptr(B), int(ngroups), int(ps2), int(nghost_of_arrays), float(gamma),
+                                       float(min_dens), float(min_pres), float(dh), float(cfl), _ptr(dt_speed_out), _stream_ptr(stream)))
 
 
 def make_config(N=16, g=3, gamma=5.0 / 3.0, scheme=VL, recon=PLM, riemann=HLLD, limvar=None, prec=FP64,
