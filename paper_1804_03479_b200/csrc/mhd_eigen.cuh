@@ -89,8 +89,15 @@ __device__ __forceinline__ void riemann_hlle(const R (&wl)[7], const R (&wr)[7],
 
 // Roe: F = 1/2 (F_L + F_R) - 1/2 sum_k |lambda_k| (L_k . dU) R_k on the conserved eigen-system of the Roe average;
 // HLLE where a~^2 <= 0 or an intermediate state has rho <= 0 or P <= 0.  Returns true if it fell back.
-template <class R>
 // etah (R19, H-correction): every wave speed of the dissipation term is max(|lam_k|, etah); 0: the plain solver
+//
+// Evaluation: the left-going and the right-going wave of a family (fast, Alfven, slow) have left / right eigenvectors E +- O with a
+// common even part E and an odd part O (the terms that carry the direction sign s).  The amplitudes L_k . dU are therefore E.dU +- O.dU
+// with sums shared by all families (v.dM, B.dB, beta.dB, beta.dM), and the right vectors Re +- Ro are built once per family: no
+// vector L_k is ever formed.  The intermediate states are still accumulated wave by wave in the order of the speeds (the
+// positivity test of R7 needs them); their pressure test is the division-free rho (E - B^2/2) - M^2/2 > 0 (rho > 0 is tested first).
+// The HLLE flux (and the fast speeds of the two sides it needs) is evaluated only where the solver falls back.
+template <class R>
 __device__ __forceinline__ bool riemann_roe(const R (&wl)[7], const R (&wr)[7], R bn, R gam, R gm1inv, R (&F)[7], R etah = R(0)) {
   const R bn2 = bn * bn;
   Side<R> L, Rr;
@@ -115,69 +122,69 @@ __device__ __forceinline__ bool riemann_roe(const R (&wl)[7], const R (&wr)[7], 
   R dU[7], Ui[7], diss[7];
 #pragma unroll
   for (int c = 0; c < 7; ++c) { dU[c] = Rr.U[c] - L.U[c]; Ui[c] = L.U[c]; diss[c] = R(0); }
+  // ---- amplitudes a_k = L_k . dU: even part + s * odd part, s = +1 for the left-going wave of a family ----
+  R ak[7];
+  {
+    const R vdM = r.vn * dU[1] + r.v1 * dU[2] + r.v2 * dU[3];          // v . dM
+    const R BdB = r.B1 * dU[5] + r.B2 * dU[6];                         // B_t . dB_t
+    const R bdB = w.b1 * dU[5] + w.b2 * dU[6];                         // beta . dB_t
+    const R bdM = w.b1 * dU[2] + w.b2 * dU[3];                         // beta . dM_t
+    const R Y = dU[4] - vdM - BdB;
+    const R G = g * ((vsq - Hp) * dU[0] + Y);
+    const R Q = nn * (r.rho * bdB - bt * dU[0]);
+    const R un = nn * (r.vn * dU[0] - dU[1]);
+    const R tv = nn * (bdM - vb * dU[0]);
+    const R Ef = w.af * (G + nn * w.cf * w.cf * dU[0]) + Asp * Q, Of = w.af * w.cf * un + Qs * tv;
+    const R Es = w.as * (G + nn * w.cs * w.cs * dU[0]) - Afp * Q, Os = w.as * w.cs * un - Qf * tv;
+    const R Ea = R(0.5) * srho * w.S * (w.b1 * dU[6] - w.b2 * dU[5]), Oa = R(0.5) * (vxb * dU[0] - w.b2 * dU[2] + w.b1 * dU[3]);
+    ak[0] = Ef + Of; ak[6] = Ef - Of;
+    ak[1] = Ea + Oa; ak[5] = Ea - Oa;
+    ak[2] = Es + Os; ak[4] = Es - Os;
+    ak[3] = dU[0] - R(2) * g * ((R(0.5) * vsq - xt) * dU[0] + Y);
+  }
+  // ---- right eigenvectors R_k = Re + s * Ro of each family (Ro has the components 1 .. 4 only) ----
+  const R ReF[7] = { w.af, w.af * r.vn, w.af * r.v1, w.af * r.v2, w.af * Hp + Asp * bt, Asp * w.b1, Asp * w.b2 };
+  const R RoF[4] = { -w.af * w.cf, Qs * w.b1, Qs * w.b2, Qs * vb - w.af * r.vn * w.cf };
+  const R ReS[7] = { w.as, w.as * r.vn, w.as * r.v1, w.as * r.v2, w.as * Hp - Afp * bt, -Afp * w.b1, -Afp * w.b2 };
+  const R RoS[4] = { -w.as * w.cs, -Qf * w.b1, -Qf * w.b2, -w.as * r.vn * w.cs - Qf * vb };
+  const R ReA5 = -w.b2 * w.S * isrho, ReA6 = w.b1 * w.S * isrho;
   bool bad = false;
 #pragma unroll
   for (int k = 0; k < 7; ++k) {
-    const R s = (k < 3) ? R(1) : R(-1);      // s = +1: the left-going ("-") wave, s = -1: the right-going one
-    R Lk[7], Rk[7];
+    const R s = (k < 3) ? R(1) : R(-1);
+    R Rk[7];
     if (k == 0 || k == 6) {                  // fast
-      Lk[0] = g * w.af * (vsq - Hp) + nn * w.af * w.cf * (w.cf + s * r.vn) - s * nn * Qs * vb - nn * Asp * bt;
-      Lk[1] = -g * w.af * r.vn - s * nn * w.af * w.cf;
-      Lk[2] = -g * w.af * r.v1 + s * nn * Qs * w.b1;
-      Lk[3] = -g * w.af * r.v2 + s * nn * Qs * w.b2;
-      Lk[4] = g * w.af;
-      Lk[5] = nn * Asp * r.rho * w.b1 - g * w.af * r.B1;
-      Lk[6] = nn * Asp * r.rho * w.b2 - g * w.af * r.B2;
-      Rk[0] = w.af; Rk[1] = w.af * (r.vn - s * w.cf);
-      Rk[2] = w.af * r.v1 + s * Qs * w.b1; Rk[3] = w.af * r.v2 + s * Qs * w.b2;
-      Rk[4] = w.af * (Hp - s * r.vn * w.cf) + s * Qs * vb + Asp * bt;
-      Rk[5] = Asp * w.b1; Rk[6] = Asp * w.b2;
+      Rk[0] = ReF[0]; Rk[5] = ReF[5]; Rk[6] = ReF[6];
+#pragma unroll
+      for (int c = 1; c < 5; ++c) Rk[c] = ReF[c] + s * RoF[c - 1];
     } else if (k == 1 || k == 5) {           // Alfven
-      Lk[0] = s * R(0.5) * vxb; Lk[1] = R(0); Lk[2] = -s * R(0.5) * w.b2; Lk[3] = s * R(0.5) * w.b1; Lk[4] = R(0);
-      Lk[5] = -R(0.5) * srho * w.b2 * w.S; Lk[6] = R(0.5) * srho * w.b1 * w.S;
-      Rk[0] = R(0); Rk[1] = R(0); Rk[2] = -s * w.b2; Rk[3] = s * w.b1; Rk[4] = -s * vxb;
-      Rk[5] = -w.b2 * w.S * isrho; Rk[6] = w.b1 * w.S * isrho;
+      Rk[0] = R(0); Rk[1] = R(0); Rk[2] = -s * w.b2; Rk[3] = s * w.b1; Rk[4] = -s * vxb; Rk[5] = ReA5; Rk[6] = ReA6;
     } else if (k == 2 || k == 4) {           // slow
-      Lk[0] = g * w.as * (vsq - Hp) + nn * w.as * w.cs * (w.cs + s * r.vn) + s * nn * Qf * vb + nn * Afp * bt;
-      Lk[1] = -g * w.as * r.vn - s * nn * w.as * w.cs;
-      Lk[2] = -g * w.as * r.v1 - s * nn * Qf * w.b1;
-      Lk[3] = -g * w.as * r.v2 - s * nn * Qf * w.b2;
-      Lk[4] = g * w.as;
-      Lk[5] = -nn * Afp * r.rho * w.b1 - g * w.as * r.B1;
-      Lk[6] = -nn * Afp * r.rho * w.b2 - g * w.as * r.B2;
-      Rk[0] = w.as; Rk[1] = w.as * (r.vn - s * w.cs);
-      Rk[2] = w.as * r.v1 - s * Qf * w.b1; Rk[3] = w.as * r.v2 - s * Qf * w.b2;
-      Rk[4] = w.as * (Hp - s * r.vn * w.cs) - s * Qf * vb - Afp * bt;
-      Rk[5] = -Afp * w.b1; Rk[6] = -Afp * w.b2;
+      Rk[0] = ReS[0]; Rk[5] = ReS[5]; Rk[6] = ReS[6];
+#pragma unroll
+      for (int c = 1; c < 5; ++c) Rk[c] = ReS[c] + s * RoS[c - 1];
     } else {                                  // entropy
-      Lk[0] = R(1) - R(2) * g * (R(0.5) * vsq - xt);
-      Lk[1] = R(2) * g * r.vn; Lk[2] = R(2) * g * r.v1; Lk[3] = R(2) * g * r.v2; Lk[4] = -R(2) * g;
-      Lk[5] = R(2) * g * r.B1; Lk[6] = R(2) * g * r.B2;
       Rk[0] = R(1); Rk[1] = r.vn; Rk[2] = r.v1; Rk[3] = r.v2; Rk[4] = R(0.5) * vsq + xt; Rk[5] = R(0); Rk[6] = R(0);
     }
-    R ak = R(0);
+    const R wk = Num<R>::max(Num<R>::abs(lam[k]), etah) * ak[k];
 #pragma unroll
-    for (int c = 0; c < 7; ++c) ak += Lk[c] * dU[c];
-    const R wk = Num<R>::max(Num<R>::abs(lam[k]), etah) * ak;
-#pragma unroll
-    for (int c = 0; c < 7; ++c) { diss[c] += wk * Rk[c]; Ui[c] += ak * Rk[c]; }
+    for (int c = 0; c < 7; ++c) { diss[c] += wk * Rk[c]; Ui[c] += ak[k] * Rk[c]; }
     if (k < 6) {
       if (lam[k + 1] > lam[k]) {
-        const R Pi = (gam - R(1)) * (Ui[4] - R(0.5) * fdiv(sqr(Ui[1]) + sqr(Ui[2]) + sqr(Ui[3]), Ui[0])
-                                      - R(0.5) * (bn2 + sqr(Ui[5]) + sqr(Ui[6])));
-        bad = bad || !(Ui[0] > R(0)) || !(Pi > R(0));
+        // rho > 0 and P > 0 <=> rho (E - B^2/2) - M^2/2 > 0
+        const R t = Ui[0] * (Ui[4] - R(0.5) * (bn2 + sqr(Ui[5]) + sqr(Ui[6]))) - R(0.5) * (sqr(Ui[1]) + sqr(Ui[2]) + sqr(Ui[3]));
+        bad = bad || !(Ui[0] > R(0)) || !(t > R(0));
       }
     }
   }
-  R Fh[7];
-  hlle_flux(wl, wr, L, Rr, a2ok, r.vn, w.cf, Fh);
   const bool superL = lam[0] >= etah, superR = lam[6] <= -etah;     // R19: the shortcuts only where every wave is faster than etah
   const bool fallback = !a2ok || (!superL && !superR && bad);
 #pragma unroll
   for (int c = 0; c < 7; ++c) {
     const R roe = R(0.5) * (L.F[c] + Rr.F[c]) - R(0.5) * diss[c];
-    F[c] = fallback ? Fh[c] : (superL ? L.F[c] : (superR ? Rr.F[c] : roe));
+    F[c] = superL ? L.F[c] : (superR ? Rr.F[c] : roe);
   }
+  if (fallback) hlle_flux(wl, wr, L, Rr, a2ok, r.vn, w.cf, F);
   return fallback;
 }
 
