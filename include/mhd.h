@@ -62,8 +62,8 @@ typedef struct {
   int limiter;      /* mhd_limiter (0 = MC) */
   int hcorr;        /* NEXT-4 variant, 0 / 1: H-correction of the Roe solver (R19: every dissipation speed of the corrector
                        pass raised to eta^H, the largest fast-characteristic jump over the face and the 8 transverse faces of its two
-                       cells).  Needs riemann = MHD_ROE and nghost one larger than the scheme alone.  Device path: VL + PLM (the
-                       combination of the paper's Fig. 18); other schemes: MHD_EINVAL (the oracle covers them) */
+                       cells).  Needs riemann = MHD_ROE and nghost one larger than the scheme alone (4 with PLM, 5 with PPM), else
+                       MHD_EINVAL.  Every scheme: VL / CTU with PLM / PPM */
 } mhd_config;
 
 /* MHD_ESTATE: a call that returns a time step (mhd_dt_reduce, mhd_advance_dt, mhd_advance_host_dt, mhd_grid_dt,

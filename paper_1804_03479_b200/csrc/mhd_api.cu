@@ -231,9 +231,16 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
     } else {
       // VL + PPM (NEXT-4): limited slopes of the half-step primitives (parked in the dead pass-1 flux arrays), the
       // monotonised parabola's interface values as L/R states, then the plain L/R Riemann kernel of CTU
-      const Box3x3 bsl = dir_boxes(g - 2, g + N + 2, g - 1, g + N + 1), brc = dir_boxes(g - 1, g + N + 1, g - 1, g + N + 1);
+      // (H-correction: eta also on the faces one further along the normal, hence states and slopes of one more cell)
+      const int hp = s->cfg.hcorr ? 1 : 0;
+      const Box3x3 bsl = dir_boxes(g - 2 - hp, g + N + 2 + hp, g - 1, g + N + 1), brc = dir_boxes(g - 1 - hp, g + N + 1 + hp, g - 1, g + N + 1);
       LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_slope_ctu<R, LIM, SC><<<GRID3(bsl), blk, 0, st>>>(p, bsl, A_WH))));
       LIM_SWITCH(lim, LAUNCH(ST_RECON, (k_recon_ctu<R, kPPMNoTrace, LIM, SC><<<GRID3(brc), blk, 0, st>>>(p, brc, A_WH))));
+      if (hp) {
+        const Box3x3 bet = dir_boxes(g - 1, g + N + 2, g - 1, g + N + 1);
+        LAUNCH(ST_RECON, (k_flux_lr<R, kROE, SC, kHcEta><<<GRID3(bet), blk, 0, st>>>(p, bet, A_BH)));
+        LAUNCH(ST_FLUX2, (k_flux_lr<R, kROE, SC, kHcOn><<<GRID3(bf2), blk, 0, st>>>(p, bf2, A_BH)));
+      } else
       LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux_lr<R, SOLVER, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2, A_BH))));
     }
     LAUNCH(ST_EMF2, (k_emf<R, A_F, SC><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                                     // step 6
@@ -241,7 +248,10 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
     // everything is derived from the cells whose half-step state the second pass needs, [lo, hi)^3 = interior + 1:
     // pass-1 fluxes on their faces and on the faces their edge EMFs touch, face states one cell further, PPM slopes
     // one more (the oracle evaluates these stages on the whole tile; what it computes outside is never used)
-    const int lo = g - 1, hi = g + N + 1;
+    // (H-correction, R19: eta of the corrected states also on the transverse faces around the pass-2 faces: everything of the first
+    // pass one cell further out, which is the one more ghost cell the switch asks for)
+    const int hp = s->cfg.hcorr ? 1 : 0;
+    const int lo = g - 1 - hp, hi = g + N + 1 + hp;
     const Box3x3 brc = dir_boxes(lo - 1, hi + 1, lo - 1, hi + 1), bf1 = dir_boxes(lo, hi + 1, lo - 1, hi + 1);
     const Box3x3 be1 = edge_boxes(lo, hi, lo, hi);
     const Box3 bh = box(lo, hi, lo, hi, lo, hi);
@@ -271,6 +281,11 @@ int run_slice_sc(mhd_solver* s, const KParams<R>& p0, int ng, cudaStream_t st) {
     }
     LAUNCH(ST_EMF1, (k_emf<R, A_F, SC><<<GRID3(be1), blk, 0, st>>>(p, be1, A_W)));                                      // step 3
     LAUNCH(ST_HALF, (k_half<R, SC><<<GRID1(bh), blk, 0, st>>>(p, bh, 0)));                                         // step 4
+    if (hp) {
+      const Box3x3 bet = dir_boxes(g - 1, g + N + 2, g - 1, g + N + 1);
+      LAUNCH(ST_RECON, (k_flux2_ctu<R, kROE, SC, kHcEta><<<GRID3(bet), blk, 0, st>>>(p, bet)));
+      LAUNCH(ST_FLUX2, (k_flux2_ctu<R, kROE, SC, kHcOn><<<GRID3(bf2), blk, 0, st>>>(p, bf2)));
+    } else
     LAUNCH(ST_FLUX2, SOLVER_SWITCH(sol, (k_flux2_ctu<R, SOLVER, SC><<<GRID3(bf2), blk, 0, st>>>(p, bf2))));        // steps 5 + 6
     LAUNCH(ST_EMF2, (k_emf<R, A_F2, SC><<<GRID3(be2), blk, 0, st>>>(p, be2, A_WH)));                               // step 7
     f2 = A_F2;
@@ -389,8 +404,8 @@ int check_config(const mhd_config* c) {
   if (c->limiter < MHD_LIMITER_MC || c->limiter > MHD_LIMITER_VANLEER) return MHD_EINVAL;
   int need = c->recon == MHD_PPM ? 4 : 3;           // DESIGN.md R8
   if (c->hcorr != 0 && c->hcorr != 1) return MHD_EINVAL;
-  if (c->hcorr) {                                   // DESIGN.md R19: Roe only, one more ghost cell; device path for VL + PLM
-    if (c->riemann != MHD_ROE || c->scheme != MHD_VL || c->recon != MHD_PLM) return MHD_EINVAL;
+  if (c->hcorr) {                                   // DESIGN.md R19: Roe only, one more ghost cell
+    if (c->riemann != MHD_ROE) return MHD_EINVAL;
     need += 1;
   }
   if (c->nghost < need || c->nghost > 8) return MHD_EINVAL;
@@ -437,6 +452,7 @@ int mhd_create(const mhd_config* cfg, mhd_solver** out) {
   s->no_fused_pass1 = getenv("MHD_NO_FUSED_PASS1") != nullptr;
   s->no_march = s->no_fused_pass1 || getenv("MHD_NO_MARCH") != nullptr;
   s->narr = (cfg->scheme == MHD_VL && cfg->recon == MHD_PLM) ? A_VL_END : A_CTU_END;   // face-state arrays: CTU, VL + PPM
+  if (cfg->scheme == MHD_CTU && cfg->hcorr) s->narr = A_CTU_HC_END;                     // + eta of the pass-2 faces
   s->esz = cfg->prec == MHD_FP32 ? 4 : 8;
   const size_t N = s->N, T = s->T;
   s->nUi = 5 * T * T * T; s->nBi = 3 * T * T * (T + 1);

@@ -31,8 +31,24 @@ enum : int {
   A_LO = 49,    // 21: CTU state at the lower d-face of each cell, [d][v]
   A_UP = 70,    // 21: CTU state at the upper d-face
   A_F2 = 91,    // 21: CTU pass-2 fluxes (the fused correction + Riemann kernel still reads the pass-1 fluxes while it writes)
-  A_CTU_END = 112
+  A_CTU_END = 112,
+  A_ETAC = 112, // 3: H-correction of CTU: eta of the pass-2 faces (the time-n velocities are still read by the correction step)
+  A_CTU_HC_END = 115
 };
+// H-correction (R19) in the pass-2 face kernels: kHcOff the plain solver, kHcEta only eta of the face is written, kHcOn the solver
+// with eta^H = max over the face and the eight transverse faces of its two cells
+enum : int { kHcOff = 0, kHcEta = 1, kHcOn = 2 };
+// eta^H of the D face q from the eta arrays at `base`
+template <class R, int D, class C>
+__device__ __forceinline__ R eta_h(const C& c, int base, int q) {
+  constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
+  R etah = c.arr(base + D)[q];
+  const R* e1 = c.arr(base + T1); const R* e2 = c.arr(base + T2);
+  const int o1 = c.off(T1), o2 = c.off(T2), ql = q - c.off(D);
+  etah = Num<R>::max(etah, Num<R>::max(Num<R>::max(e1[ql], e1[ql + o1]), Num<R>::max(e1[q], e1[q + o1])));
+  etah = Num<R>::max(etah, Num<R>::max(Num<R>::max(e2[ql], e2[ql + o2]), Num<R>::max(e2[q], e2[q + o2])));
+  return etah;
+}
 
 template <class R> struct KParams {
   const R* Uin; const R* Bin;       // first group of the slice

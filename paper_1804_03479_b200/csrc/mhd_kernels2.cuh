@@ -23,21 +23,13 @@ __device__ __forceinline__ void plm_states_vl(const Ctx<R, KP>& c, const KP& p, 
 }
 template <class R, int SOLVER, int LIMVAR, int D, bool HC, class KP>
 __device__ __forceinline__ void flux2_vl_dir(const KP& p, const Box3& box) {
-  constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
   Ctx<R, KP> c(p, box);
   if (!c.ok) return;
-  const int o = c.off(D), q = c.q;
+  const int q = c.q;
   R wl[7], wr[7], F[7];
   plm_states_vl<R, LIMVAR, D, true>(c, p, wl, wr);
-  R etah = R(0);
-  if (HC) {
-    // eta^H: this face and the lower / upper T1 and T2 faces of its two cells (k_eta2_vl wrote them on a box one face wider)
-    etah = c.arr(A_ETA + D)[q];
-    const R* e1 = c.arr(A_ETA + T1); const R* e2 = c.arr(A_ETA + T2);
-    const int o1 = c.off(T1), o2 = c.off(T2), ql = q - o;
-    etah = Num<R>::max(etah, Num<R>::max(Num<R>::max(e1[ql], e1[ql + o1]), Num<R>::max(e1[q], e1[q + o1])));
-    etah = Num<R>::max(etah, Num<R>::max(Num<R>::max(e2[ql], e2[ql + o2]), Num<R>::max(e2[q], e2[q + o2])));
-  }
+  // eta^H: this face and the lower / upper T1 and T2 faces of its two cells (k_eta2_vl wrote them on a box one face wider)
+  const R etah = HC ? eta_h<R, D>(c, A_ETA, q) : R(0);
   const bool fb = riemann<R, SOLVER>(wl, wr, c.arr(A_BH + D)[q], p.gam, p.gm1inv, F, etah);
   if (fb) count_event(p.stats + 2);
 #pragma unroll
@@ -151,7 +143,8 @@ __global__ void __launch_bounds__(256, Occ<R>::minb) k_recon_ctu(const KParamsSC
 }
 
 // ---- CTU steps 2 and 6: Riemann solve between the upper state of cell i-1 and the lower of i ----
-template <class R, int SOLVER, int D, class KP>
+// HC (kHcOff / kHcEta / kHcOn) and etabase: H-correction of VL + PPM, whose pass 2 runs through this kernel
+template <class R, int SOLVER, int D, int HC, class KP>
 __device__ __forceinline__ void flux_lr_dir(const KP& p, const Box3& box, int bbase) {
   Ctx<R, KP> c(p, box);
   if (!c.ok) return;
@@ -159,17 +152,19 @@ __device__ __forceinline__ void flux_lr_dir(const KP& p, const Box3& box, int bb
   R wl[7], wr[7], F[7];
 #pragma unroll
   for (int v = 0; v < 7; ++v) { wl[v] = c.arr(A_UP + 7 * D + v)[ql]; wr[v] = c.arr(A_LO + 7 * D + v)[q]; }
-  const bool fb = riemann<R, SOLVER>(wl, wr, c.arr(bbase + D)[q], p.gam, p.gm1inv, F);
+  if (HC == kHcEta) { c.arr(A_ETA + D)[q] = eta_face(wl, wr, c.arr(bbase + D)[q], p.gam); return; }
+  const R etah = HC == kHcOn ? eta_h<R, D>(c, A_ETA, q) : R(0);
+  const bool fb = riemann<R, SOLVER>(wl, wr, c.arr(bbase + D)[q], p.gam, p.gm1inv, F, etah);
   if (fb) count_event(p.stats + 2);
 #pragma unroll
   for (int v = 0; v < 7; ++v) c.arr(A_F + 7 * D + v)[q] = F[v];
 }
-template <class R, int SOLVER, int SC>
+template <class R, int SOLVER, int SC, int HC = kHcOff>
 __global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux_lr(const KParamsSC<R, SC> p, const Box3x3 bx, int bbase) {
   switch (blockIdx.y) {
-    case 0: flux_lr_dir<R, SOLVER, 0>(p, bx.b[0], bbase); break;
-    case 1: flux_lr_dir<R, SOLVER, 1>(p, bx.b[1], bbase); break;
-    default: flux_lr_dir<R, SOLVER, 2>(p, bx.b[2], bbase); break;
+    case 0: flux_lr_dir<R, SOLVER, 0, HC>(p, bx.b[0], bbase); break;
+    case 1: flux_lr_dir<R, SOLVER, 1, HC>(p, bx.b[1], bbase); break;
+    default: flux_lr_dir<R, SOLVER, 2, HC>(p, bx.b[2], bbase); break;
   }
 }
 
@@ -212,7 +207,7 @@ __device__ __forceinline__ void ctu_corr_cell(const Ctx<R, KP>& c, const KP& p, 
 }
 // one state w of the cell (at the face whose time-n normal field is bnn and half-step normal field bh): to conserved
 // variables, correct, back to primitive variables with the floors of R9
-template <class R, class KP>
+template <bool COUNT = true, class R, class KP>
 __device__ __forceinline__ void ctu_corr_apply(const KP& p, const CtuCorr<R>& k, R hdt, R qh, R bnn, R bh, R (&w)[7]) {
   R u[7];
   u[0] = w[0]; u[1] = w[0] * w[1]; u[2] = w[0] * w[2]; u[3] = w[0] * w[3];
@@ -224,13 +219,14 @@ __device__ __forceinline__ void ctu_corr_apply(const KP& p, const CtuCorr<R>& k,
   u[5] += hdt * k.v1 * k.m1; u[6] += hdt * k.v2 * k.m2;
   u[4] += hdt * (k.Bc1 * k.v1 * k.m1 + k.Bc2 * k.v2 * k.m2);
   R rho = u[0];
-  if (rho < p.min_dens) { rho = p.min_dens; count_event(p.stats + 0); }
+  if (rho < p.min_dens) { rho = p.min_dens; if (COUNT) count_event(p.stats + 0); }
   const R ir = frcp(rho);
   w[0] = rho; w[1] = u[1] * ir; w[2] = u[2] * ir; w[3] = u[3] * ir; w[5] = u[5]; w[6] = u[6];
   w[4] = p.gm1 * (u[4] - R(0.5) * rho * (sqr(w[1]) + sqr(w[2]) + sqr(w[3])) - R(0.5) * (sqr(bh) + sqr(w[5]) + sqr(w[6])));
-  if (w[4] < p.min_pres) { w[4] = p.min_pres; count_event(p.stats + 1); }
+  if (w[4] < p.min_pres) { w[4] = p.min_pres; if (COUNT) count_event(p.stats + 1); }
 }
-template <class R, int SOLVER, int D, class KP>
+// HC = kHcEta: the corrected states only, for eta of the face (floors not counted twice); kHcOn: the Roe solver with eta^H
+template <class R, int SOLVER, int D, int HC, class KP>
 __device__ __forceinline__ void flux2_ctu_dir(const KP& p, const Box3& box) {
   Ctx<R, KP> c(p, box);
   if (!c.ok) return;
@@ -242,20 +238,22 @@ __device__ __forceinline__ void flux2_ctu_dir(const KP& p, const Box3& box) {
   const R bnn = c.arr(A_B + D)[q], bh = c.arr(A_BH + D)[q];
   CtuCorr<R> k;
   ctu_corr_cell<R, D>(c, p, ql, qh, k);
-  ctu_corr_apply(p, k, hdt, qh, bnn, bh, wl);
+  ctu_corr_apply<HC != kHcEta>(p, k, hdt, qh, bnn, bh, wl);
   ctu_corr_cell<R, D>(c, p, q, qh, k);
-  ctu_corr_apply(p, k, hdt, qh, bnn, bh, wr);
-  const bool fb = riemann<R, SOLVER>(wl, wr, bh, p.gam, p.gm1inv, F);
+  ctu_corr_apply<HC != kHcEta>(p, k, hdt, qh, bnn, bh, wr);
+  if (HC == kHcEta) { c.arr(A_ETAC + D)[q] = eta_face(wl, wr, bh, p.gam); return; }
+  const R etah = HC == kHcOn ? eta_h<R, D>(c, A_ETAC, q) : R(0);
+  const bool fb = riemann<R, SOLVER>(wl, wr, bh, p.gam, p.gm1inv, F, etah);
   if (fb) count_event(p.stats + 2);
 #pragma unroll
   for (int v = 0; v < 7; ++v) c.arr(A_F2 + 7 * D + v)[q] = F[v];
 }
-template <class R, int SOLVER, int SC>
+template <class R, int SOLVER, int SC, int HC = kHcOff>
 __global__ void __launch_bounds__(256, OccFlux<R, SOLVER>::minb) k_flux2_ctu(const KParamsSC<R, SC> p, const Box3x3 bx) {
   switch (blockIdx.y) {
-    case 0: flux2_ctu_dir<R, SOLVER, 0>(p, bx.b[0]); break;
-    case 1: flux2_ctu_dir<R, SOLVER, 1>(p, bx.b[1]); break;
-    default: flux2_ctu_dir<R, SOLVER, 2>(p, bx.b[2]); break;
+    case 0: flux2_ctu_dir<R, SOLVER, 0, HC>(p, bx.b[0]); break;
+    case 1: flux2_ctu_dir<R, SOLVER, 1, HC>(p, bx.b[1]); break;
+    default: flux2_ctu_dir<R, SOLVER, 2, HC>(p, bx.b[2]); break;
   }
 }
 

@@ -166,10 +166,49 @@ def test_expansion_shock_dissolves_on_the_device(oracle):
     assert res[0] > 0.95 * jump and res[1] < 0.5 * jump, res
 
 
+@pytest.mark.parametrize("scheme,recon,g", [(1, 1, 5), (1, 0, 4), (0, 1, 5)])
+@pytest.mark.parametrize("prec", [1, 0])
+def test_h_correction_ctu_and_ppm_one_step_and_ten_steps(oracle, scheme, recon, g, prec):
+    """the other schemes (the paper's own test combination CTU + PPM + Roe; CTU + PLM; VL + PPM): eta of the corrected /
+    parabola states, one more ghost cell, against the oracle"""
+    N, G = 16, 4
+    dtp = GU.np_dtype(prec)
+    limvar = 1 if scheme == 1 else 0
+    U_in, B_in, dh = inputs.config2_batch(G, N=N, g=g, dtype=dtp)
+    U64, B64 = U_in.astype(np.float64), B_in.astype(np.float64)
+    kw = dict(N=N, g=g, scheme=scheme, recon=recon, riemann=2, limvar=limvar)
+    cfg = oracle.make_config(emf_tie=EMF_TIE[prec], hcorr=1, **kw)
+    dt, _ = oracle.dt_reduce(cfg, U64, B64, g, dh, 0.3)
+    ref = oracle.advance(cfg, U64, B64, dt, dh)
+    gpu = GU.GpuRunner(prec=prec, max_groups=8, hcorr=1, **kw)
+    out = gpu(U_in, B_in, dt, dh)
+    errs = GU.field_errors(out, ref, N)
+    assert not bad_fields(errs, TOL_ONE_STEP[prec]), errs
+    plain = oracle.advance(oracle.make_config(emf_tie=EMF_TIE[prec], **kw), U64, B64, dt, dh)
+    assert np.abs(plain["U"] - ref["U"]).max() > 1e-6               # it is the corrected solver that was compared
+    assert all(a <= b for a, b in zip(gpu.stats(), ref["stats"]))
+    n = 32
+    U, bx, by, bz, dh = inputs.random_group_grid(n, 78)
+    adv = lambda Ui, Bi, dt_, dh_: oracle.advance(cfg, Ui, Bi, dt_, dh_)
+    r = [a.astype(dtp).astype(np.float64) for a in (U, bx, by, bz)]
+    d = [a.astype(dtp) for a in (U, bx, by, bz)]
+    for _ in range(10):
+        Ui, Bi = inputs.pack_groups(*r, n, 0)
+        dt, _ = oracle.dt_reduce(oracle.make_config(N=n, g=3), Ui, Bi, 0, dh, 0.3)
+        r = list(H.step_grid(adv, *r, dt, dh, N, g)[:4])
+        o = H.step_grid(gpu, *d, dt, dh, N, g, dtype=dtp)
+        assert o[5] == 0.0                                            # shared faces of neighbouring groups bitwise equal
+        d = list(o[:4])
+    for a, b in zip(d, r):
+        assert H.field_err(a, b) <= TOL[prec]
+    assert H.rel_divb(*(np.asarray(a, dtype=np.float64) for a in d[1:]), dh) < (1e-13 if prec == 1 else 2e-5)
+
+
 def test_h_correction_argument_checks():
     from paper_1804_03479_b200 import mhd
-    for kw in (dict(riemann=mhd.HLLD, g=4), dict(riemann=mhd.ROE, g=3), dict(riemann=mhd.ROE, g=5, scheme=mhd.CTU, recon=mhd.PPM),
-               dict(riemann=mhd.ROE, g=5, scheme=mhd.VL, recon=mhd.PPM)):
+    for kw in (dict(riemann=mhd.HLLD, g=4), dict(riemann=mhd.ROE, g=3), dict(riemann=mhd.ROE, g=4, scheme=mhd.CTU, recon=mhd.PPM),
+               dict(riemann=mhd.ROE, g=4, scheme=mhd.VL, recon=mhd.PPM), dict(riemann=mhd.ROE, g=3, scheme=mhd.CTU, recon=mhd.PLM),
+               dict(riemann=mhd.HLLE, g=5, scheme=mhd.CTU, recon=mhd.PPM)):
         with pytest.raises(mhd.MHDError) as ei:
             mhd.Solver(mhd.make_config(hcorr=1, max_groups=2, **kw))
         assert ei.value.code == mhd.EINVAL
