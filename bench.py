@@ -47,7 +47,9 @@ STAGE_STEPS = {"march_pass1": (1, 2, 3, 4), "march_pass2": (5, 6, 7), "emf_pass1
                "final_update": (7,)}
 NOMINAL_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
 TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_dram_traffic.csv")
-E2E_CHUNK, E2E_STREAMS = 32, 4                  # measured best of chunk x streams on this box (PCIe-bound)
+# host path: groups per chunk and streams, the measured best of 16 ... 256 x 2 ... 8 on this box (PCIe-bound; CTU's longer kernels want
+# the shorter pipeline fill of smaller chunks)
+E2E_CHUNK, E2E_STREAMS = {"vl": 64, "ctu": 32}, 4
 
 
 def ncu_traffic():
@@ -330,7 +332,7 @@ def measure(args, prec_name, rank, world, dist, scheme=None, riemann=None, steps
         pin = lambda a: torch.from_numpy(a).pin_memory()
         pU, pB = pin(hU), pin(hB)
         hout = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
-        chunk, nstr = max(1, min(G, E2E_CHUNK)), E2E_STREAMS
+        chunk, nstr = max(1, min(G, E2E_CHUNK[a2.scheme])), E2E_STREAMS
         ksteps = max(3, steps // 4)
         for _ in range(2):
             solver.advance_host_dt(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], G, dt0, dh, chunk, nstr, 0.3)
@@ -379,7 +381,7 @@ def measure_config5(args, scheme_name, pool=None):
     out = solver.alloc_outputs(P, planes=True)
     hout = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
     passes = total // P
-    chunk, nstr = E2E_CHUNK, E2E_STREAMS
+    chunk, nstr = E2E_CHUNK[scheme_name], E2E_STREAMS
     solver.advance_host(pU, pB, hout["U"], hout["B"], hout["flux"], hout["emf"], P, dt0, dh, chunk, nstr)
     sampler = ClockSampler(torch.cuda.current_device())
     torch.cuda.synchronize()
