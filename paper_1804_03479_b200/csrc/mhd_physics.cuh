@@ -41,9 +41,17 @@ template <class R> struct OccHalf  { static constexpr int minb = sizeof(R) == 8 
 template <class R> struct OccFinal { static constexpr int minb = sizeof(R) == 8 ? MHD_OCC_FINAL64 : MHD_OCC_FINAL32; };
 template <class R> struct OccEmf   { static constexpr int minb = sizeof(R) == 8 ? MHD_OCC_EMF64 : MHD_OCC_EMF32; };
 template <class R> struct Occ { static constexpr int minb = sizeof(R) == 8 ? MHD_MINB64 : MHD_MINB32; };          // reconstruction
-// Riemann kernels (measured: HLLD FP64 3 > 2 > 4 blocks; Roe needs ~220 FP64 / ~120 FP32 registers and must not be capped)
+// Riemann kernels (measured: HLLD FP64 3 > 2 > 4 blocks.  Roe, since the solver forms no left eigenvectors any more (mhd_eigen.cuh): FP64
+// 2 blocks of 128 registers with ~220 bytes of spills beat 1 block of 190 registers, VL+PLM+Roe 5.5e8 -> 6.9e8; 3 blocks: 4.6e8.
+// FP32 3 blocks of 85 registers beat 2 of 96, CTU+PPM+Roe 9.4e8 -> 1.00e9; 4 blocks: 9.0e8)
+#ifndef MHD_OCC_ROE64
+#define MHD_OCC_ROE64 2
+#endif
+#ifndef MHD_OCC_ROE32
+#define MHD_OCC_ROE32 3
+#endif
 template <class R, int SOLVER> struct OccFlux {
-  static constexpr int minb = SOLVER == 2 ? (sizeof(R) == 8 ? 1 : 2) : (sizeof(R) == 8 ? MHD_MINB64_FLUX : MHD_MINB32);
+  static constexpr int minb = SOLVER == 2 ? (sizeof(R) == 8 ? MHD_OCC_ROE64 : MHD_OCC_ROE32) : (sizeof(R) == 8 ? MHD_MINB64_FLUX : MHD_MINB32);
 };
 enum : int { kPLM = 0, kPPM = 1, kPPMNoTrace = 2 };   // kPPMNoTrace: the PPM parabola at the half step of VL (NEXT-4)
 enum : int { kLimPrim = 0, kLimChar = 1 };   // kernels take LIM = limvar + 2 * limiter (limiter: 0 MC, 1 minmod, 2 van Leer)
