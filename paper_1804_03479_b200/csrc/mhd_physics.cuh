@@ -116,6 +116,15 @@ __device__ __forceinline__ void frcp4(double a, double b, double c, double d, do
 }
 
 // monotonised-central limiter (R5)
+// FP32: the same value in 7 instructions instead of 13: min(|a|, |b|) with the sign sign(a) xor sign(b) in ONE instruction
+// (min.xorsign.abs), so opposite signs give a value <= 0 that the clamp at zero removes (a zero operand gives 0 by itself);
+// min(|s| / 2, 2 q) = 2 min(|s| / 4, q) exactly; the sign of the result is that of a (= that of a + b where the signs agree)
+__device__ __forceinline__ float lim_mc(float a, float b) {
+  float q;
+  asm("min.xorsign.abs.f32 %0, %1, %2;" : "=f"(q) : "f"(a), "f"(b));
+  const float r = fmaxf(fminf(q, 0.25f * fabsf(a + b)), 0.0f);
+  return copysignf(r + r, a);
+}
 template <class R> __device__ __forceinline__ R lim_mc(R a, R b) {
   R s = a + b;
   R m = Num<R>::min(R(0.5) * Num<R>::abs(s), R(2) * Num<R>::min(Num<R>::abs(a), Num<R>::abs(b)));
