@@ -70,6 +70,13 @@ def test_strerror_and_null_argument_checks_need_no_device(libpath):
     assert L.mhd_destroy(None) == mhd.EINVAL
     assert L.mhd_advance(None, None, None, None, None, None, None, 1, 0.1, 0.1, None) == mhd.EINVAL
     assert L.mhd_launch_count(None) == 0
+    # the no-allocation entry point checks its arguments and its size limit before it touches the device
+    one = C.c_double()
+    ptr = C.cast(C.pointer(one), C.c_void_p)
+    assert L.mhd_dt_reduce_noalloc(0, None, ptr, 1, 16, 0, 5.0 / 3.0, 1e-10, 1e-10, 0.1, 0.3, ptr, None) == mhd.EINVAL
+    assert L.mhd_dt_reduce_noalloc(0, ptr, ptr, 1, 15, 0, 5.0 / 3.0, 1e-10, 1e-10, 0.1, 0.3, ptr, None) == mhd.EINVAL
+    assert L.mhd_dt_reduce_noalloc(0, ptr, ptr, mhd.NOALLOC_MAX_BLOCKS // 16 + 1, 16, 0, 5.0 / 3.0, 1e-10, 1e-10, 0.1, 0.3, ptr, None) == mhd.ELIMIT
+    assert "MHD_NOALLOC_MAX_BLOCKS" in mhd.strerror(mhd.ELIMIT)
 
 
 def test_no_cpu_fallback_create_fails_loudly_without_a_device(libpath):
